@@ -1,0 +1,168 @@
+"""ctypes front end of the fp64 CPU oracle (oracle/oracle.cpp).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this.  It never imports the CUDA package and the CUDA package never imports it.
+
+All fields are canonical real arrays: float64, C-contiguous, shape [V,4,nc,nc,2] (links) or
+[V,nc,nc,2] (per-site matrices); site s = x0 + N0*(x1 + N1*(x2 + N2*x3)).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle.cpp -> liboracle.so with g++ -O2 (no fast-math), OpenMP if available."""
+    if not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC):
+        return _LIB
+    base = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-o", _LIB, _SRC]
+    try:
+        subprocess.run(base[:1] + ["-fopenmp"] + base[1:], check=True, capture_output=True)
+    except subprocess.CalledProcessError:
+        subprocess.run(base, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    build()
+    lib = ctypes.CDLL(_LIB)
+    i32p = ctypes.POINTER(ctypes.c_int32)
+    dp = ctypes.POINTER(ctypes.c_double)
+    lib.oracle_set_threads.argtypes = [ctypes.c_int]
+    lib.oracle_set_threads.restype = ctypes.c_int
+    lib.oracle_max_threads.restype = ctypes.c_int
+    lib.oracle_su2_pow.argtypes = [dp, ctypes.c_double, dp]
+    lib.oracle_K.argtypes = [i32p, ctypes.c_int, dp, dp]
+    lib.oracle_site_G.argtypes = [ctypes.c_int, dp, ctypes.c_double, dp]
+    lib.oracle_subgroup_step.argtypes = [ctypes.c_int, dp, ctypes.c_int, ctypes.c_int,
+                                         ctypes.c_double, dp]
+    lib.oracle_subgroup_step.restype = ctypes.c_int
+    lib.oracle_or_sweep.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double]
+    lib.oracle_functional.argtypes = [i32p, ctypes.c_int, dp]
+    lib.oracle_functional.restype = ctypes.c_double
+    lib.oracle_delta.argtypes = [i32p, ctypes.c_int, dp, dp]
+    lib.oracle_gauge_precision.argtypes = [i32p, ctypes.c_int, dp]
+    lib.oracle_gauge_precision.restype = ctypes.c_double
+    lib.oracle_gauge_transform.argtypes = [i32p, ctypes.c_int, dp, dp]
+    lib.oracle_plaquette.argtypes = [i32p, ctypes.c_int, dp]
+    lib.oracle_plaquette.restype = ctypes.c_double
+    lib.oracle_reconstruct12.argtypes = [ctypes.c_int64, dp]
+    _lib = lib
+    return lib
+
+
+def _dims(dims):
+    arr = (ctypes.c_int32 * 4)(*[int(d) for d in dims])
+    return arr
+
+
+def _dp(a: np.ndarray):
+    if a.dtype != np.float64 or not a.flags["C_CONTIGUOUS"]:
+        raise TypeError("oracle arrays must be C-contiguous float64")
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _check_links(dims, u: np.ndarray) -> int:
+    v = int(np.prod([int(d) for d in dims]))
+    if u.ndim != 5 or u.shape[0] != v or u.shape[1] != 4 or u.shape[2] != u.shape[3] or u.shape[4] != 2:
+        raise ValueError(f"links must be [V,4,nc,nc,2], got {u.shape}")
+    if u.shape[2] not in (2, 3):
+        raise ValueError("nc must be 2 or 3")
+    return u.shape[2]
+
+
+def set_threads(n: int) -> int:
+    return _load().oracle_set_threads(int(n))
+
+
+def max_threads() -> int:
+    return _load().oracle_max_threads()
+
+
+def su2_pow(q, omega: float) -> np.ndarray:
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    out = np.empty(4)
+    _load().oracle_su2_pow(_dp(q), float(omega), _dp(out))
+    return out
+
+
+def K_field(dims, u: np.ndarray) -> np.ndarray:
+    nc = _check_links(dims, u)
+    out = np.empty((u.shape[0], nc, nc, 2))
+    _load().oracle_K(_dims(dims), nc, _dp(u), _dp(out))
+    return out
+
+
+def site_G(K: np.ndarray, omega: float) -> np.ndarray:
+    """K real [nc,nc,2] -> G real [nc,nc,2]."""
+    K = np.ascontiguousarray(K, dtype=np.float64)
+    out = np.empty_like(K)
+    _load().oracle_site_G(K.shape[0], _dp(K), float(omega), _dp(out))
+    return out
+
+
+def subgroup_step(K: np.ndarray, i: int, j: int, omega: float):
+    K = np.ascontiguousarray(K, dtype=np.float64)
+    out = np.empty_like(K)
+    ok = _load().oracle_subgroup_step(K.shape[0], _dp(K), int(i), int(j), float(omega), _dp(out))
+    return out, bool(ok)
+
+
+def or_sweep(dims, u: np.ndarray, parity: int, omega: float) -> None:
+    """One half-sweep, in place."""
+    nc = _check_links(dims, u)
+    _load().oracle_or_sweep(_dims(dims), nc, _dp(u), int(parity), float(omega))
+
+
+def full_sweep(dims, u: np.ndarray, omega: float) -> None:
+    """Black (parity 0) then white (parity 1) half-sweep, in place."""
+    or_sweep(dims, u, 0, omega)
+    or_sweep(dims, u, 1, omega)
+
+
+def functional(dims, u: np.ndarray) -> float:
+    nc = _check_links(dims, u)
+    return float(_load().oracle_functional(_dims(dims), nc, _dp(u)))
+
+
+def delta_field(dims, u: np.ndarray) -> np.ndarray:
+    nc = _check_links(dims, u)
+    out = np.empty((u.shape[0], nc, nc, 2))
+    _load().oracle_delta(_dims(dims), nc, _dp(u), _dp(out))
+    return out
+
+
+def gauge_precision(dims, u: np.ndarray) -> float:
+    nc = _check_links(dims, u)
+    return float(_load().oracle_gauge_precision(_dims(dims), nc, _dp(u)))
+
+
+def gauge_transform(dims, u: np.ndarray, g: np.ndarray) -> None:
+    nc = _check_links(dims, u)
+    if g.shape != (u.shape[0], nc, nc, 2):
+        raise ValueError("g must be [V,nc,nc,2]")
+    _load().oracle_gauge_transform(_dims(dims), nc, _dp(u), _dp(g))
+
+
+def plaquette(dims, u: np.ndarray) -> float:
+    nc = _check_links(dims, u)
+    return float(_load().oracle_plaquette(_dims(dims), nc, _dp(u)))
+
+
+def reconstruct12(m: np.ndarray) -> None:
+    """In place: rebuild row 2 = conj(row0 x row1) of every 3x3 matrix in real [...,3,3,2]."""
+    if m.shape[-3:] != (3, 3, 2):
+        raise ValueError("need [...,3,3,2]")
+    _load().oracle_reconstruct12(int(m.size // 18), _dp(m))

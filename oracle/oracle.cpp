@@ -1,0 +1,408 @@
+// oracle/oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// A plain, slow, obviously-correct fp64 CPU implementation of the checkerboard overrelaxation
+// sweep for lattice Landau gauge fixing (arXiv:1412.3655, "cuLGT: Lattice Gauge Fixing on
+// GPUs"), written from the paper's text.  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may call it.  It shares no code with the CUDA path under
+// paper_1412_3655_b200/ (no headers, helpers, tables, pre- or post-processing) and neither
+// imports the other.
+//
+// Citations: P:Lnn = /root/reference/PAPER.md line nn.  "C-n" = reading n in DESIGN.md
+// (points where the paper is silent / ambiguous).
+//
+// Layout (canonical): site s = x0 + N0*(x1 + N1*(x2 + N2*x3)), periodic,
+// parity(x) = (x0+x1+x2+x3)&1, black = 0 (C-1).  U is double[V][4][nc][nc][2], i.e. full
+// nc x nc complex matrices, re/im interleaved, row-major.  nc = 2 or 3.
+//
+// There is no blocking, fusion or reordering: every function is the paper's formula looped
+// over sites.  Sums over the lattice are Neumaier-compensated so the oracle is the trustworthy
+// side of a reduction comparison.  OpenMP is used only across the independent sites of one
+// parity ("only transformations at neighboring sites interfere") and across sites in the
+// per-site terms of a reduction; the arithmetic per site is unchanged by it.
+//
+// Pins (tests/test_oracle_*.py, run with -m "not gpu"): see DESIGN.md "Oracle pins".
+// Every exported function below is pinned by at least one of them; none is "parity unpinned".
+
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef std::complex<double> cd;
+
+namespace {
+
+int g_threads = 1;
+
+struct Lat {
+  int N[4];
+  int64_t V;
+  int nc;
+};
+
+Lat make_lat(const int32_t* dims, int nc) {
+  Lat L;
+  for (int i = 0; i < 4; ++i) L.N[i] = dims[i];
+  L.V = (int64_t)dims[0] * dims[1] * dims[2] * dims[3];
+  L.nc = nc;
+  return L;
+}
+
+void coords_of(const Lat& L, int64_t s, int x[4]) {
+  x[0] = (int)(s % L.N[0]); s /= L.N[0];
+  x[1] = (int)(s % L.N[1]); s /= L.N[1];
+  x[2] = (int)(s % L.N[2]); s /= L.N[2];
+  x[3] = (int)s;
+}
+
+int64_t index_of(const Lat& L, const int x[4]) {
+  return x[0] + (int64_t)L.N[0] * (x[1] + (int64_t)L.N[1] * (x[2] + (int64_t)L.N[2] * x[3]));
+}
+
+// site index of x + step*mu_hat with periodic wrap (C-2)
+int64_t neighbour(const Lat& L, int64_t s, int mu, int step) {
+  int x[4];
+  coords_of(L, s, x);
+  x[mu] = ((x[mu] + step) % L.N[mu] + L.N[mu]) % L.N[mu];
+  return index_of(L, x);
+}
+
+int parity_of(const Lat& L, int64_t s) {
+  int x[4];
+  coords_of(L, s, x);
+  return (x[0] + x[1] + x[2] + x[3]) & 1;
+}
+
+struct Mat {
+  cd e[3][3];
+};
+
+Mat zero_mat() {
+  Mat m;
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b) m.e[a][b] = cd(0.0, 0.0);
+  return m;
+}
+
+Mat unit_mat(int nc) {
+  Mat m = zero_mat();
+  for (int a = 0; a < nc; ++a) m.e[a][a] = cd(1.0, 0.0);
+  return m;
+}
+
+Mat load_mat(const double* base, int nc) {
+  Mat m = zero_mat();
+  for (int a = 0; a < nc; ++a)
+    for (int b = 0; b < nc; ++b) m.e[a][b] = cd(base[2 * (a * nc + b)], base[2 * (a * nc + b) + 1]);
+  return m;
+}
+
+void store_mat(double* base, int nc, const Mat& m) {
+  for (int a = 0; a < nc; ++a)
+    for (int b = 0; b < nc; ++b) {
+      base[2 * (a * nc + b)] = m.e[a][b].real();
+      base[2 * (a * nc + b) + 1] = m.e[a][b].imag();
+    }
+}
+
+const double* link_ptr(const double* U, const Lat& L, int64_t s, int mu) {
+  return U + ((s * 4 + mu) * L.nc * L.nc) * 2;
+}
+double* link_ptr(double* U, const Lat& L, int64_t s, int mu) {
+  return U + ((s * 4 + mu) * L.nc * L.nc) * 2;
+}
+
+Mat mul(const Mat& A, const Mat& B, int nc) {
+  Mat C = zero_mat();
+  for (int a = 0; a < nc; ++a)
+    for (int b = 0; b < nc; ++b) {
+      cd acc(0.0, 0.0);
+      for (int k = 0; k < nc; ++k) acc += A.e[a][k] * B.e[k][b];
+      C.e[a][b] = acc;
+    }
+  return C;
+}
+
+Mat dagger(const Mat& A, int nc) {
+  Mat C = zero_mat();
+  for (int a = 0; a < nc; ++a)
+    for (int b = 0; b < nc; ++b) C.e[a][b] = std::conj(A.e[b][a]);
+  return C;
+}
+
+Mat add(const Mat& A, const Mat& B, int nc) {
+  Mat C = zero_mat();
+  for (int a = 0; a < nc; ++a)
+    for (int b = 0; b < nc; ++b) C.e[a][b] = A.e[a][b] + B.e[a][b];
+  return C;
+}
+
+cd trace(const Mat& A, int nc) {
+  cd t(0.0, 0.0);
+  for (int a = 0; a < nc; ++a) t += A.e[a][a];
+  return t;
+}
+
+// Neumaier-compensated sum of n doubles, in index order.
+double neumaier_sum(const double* v, int64_t n) {
+  double sum = 0.0, comp = 0.0;
+  for (int64_t i = 0; i < n; ++i) {
+    double t = sum + v[i];
+    if (std::fabs(sum) >= std::fabs(v[i])) comp += (sum - t) + v[i];
+    else comp += (v[i] - t) + sum;
+    sum = t;
+  }
+  return sum + comp;
+}
+
+// K(x) = sum_mu [ U_mu(x) + U_mu(x - mu)^dagger ]   -- eq. (3).  mu ascending, up then down (C-17).
+Mat gather_K(const double* U, const Lat& L, int64_t s) {
+  Mat K = zero_mat();
+  for (int mu = 0; mu < 4; ++mu) {
+    K = add(K, load_mat(link_ptr(U, L, s, mu), L.nc), L.nc);
+    int64_t sd = neighbour(L, s, mu, -1);
+    K = add(K, dagger(load_mat(link_ptr(U, L, sd, mu), L.nc), L.nc), L.nc);
+  }
+  return K;
+}
+
+// Exact group power q^omega of a unit quaternion q = (c, v) = cos(alpha) + i sin(alpha) n.sigma on
+// the principal branch alpha in [0, pi] (reading C-8 of "replacing g(x) by g^omega(x)").
+// alpha = atan2(|v|, c), never acos(c).
+void su2_pow(const double q[4], double omega, double out[4]) {
+  double c = q[0];
+  double r = std::hypot(q[1], q[2], q[3]);
+  if (r < 1e-150) {
+    if (c > 0.0) { out[0] = 1.0; out[1] = out[2] = out[3] = 0.0; }
+    else { out[0] = std::cos(omega * M_PI); out[1] = 0.0; out[2] = 0.0; out[3] = std::sin(omega * M_PI); }
+    return;
+  }
+  double alpha = std::atan2(r, c);
+  double f = std::sin(omega * alpha) / r;
+  out[0] = std::cos(omega * alpha);
+  out[1] = q[1] * f;
+  out[2] = q[2] * f;
+  out[3] = q[3] * f;
+}
+
+// SU(2) convention C-7: (a0,a1,a2,a3) <-> [[a0 + i a3, a2 + i a1], [-a2 + i a1, a0 - i a3]].
+// Embeds the quaternion q into rows/cols (i,j) of an nc x nc identity.
+Mat embed_su2(const double q[4], int i, int j, int nc) {
+  Mat g = unit_mat(nc);
+  g.e[i][i] = cd(q[0], q[3]);
+  g.e[i][j] = cd(q[2], q[1]);
+  g.e[j][i] = cd(-q[2], q[1]);
+  g.e[j][j] = cd(q[0], -q[3]);
+  return g;
+}
+
+// One subgroup step (readings C-6, C-9, C-10): project the (i,j) 2x2 block of K onto
+// its real-quaternion part p (twice the SU(2)-proportional part), g = p^dagger/|p| which is
+// K_block^dagger / sqrt(det K_block^dagger) for an SU(2)-proportional block, raise it to
+// the power omega.  Returns false (g_s = 1) when |p| = 0.
+bool subgroup_step(const Mat& K, int i, int j, double omega, int nc, Mat* gs) {
+  double p0 = K.e[i][i].real() + K.e[j][j].real();
+  double p1 = K.e[i][j].imag() + K.e[j][i].imag();
+  double p2 = K.e[i][j].real() - K.e[j][i].real();
+  double p3 = K.e[i][i].imag() - K.e[j][j].imag();
+  double n = std::sqrt(p0 * p0 + p1 * p1 + p2 * p2 + p3 * p3);
+  if (n == 0.0) { *gs = unit_mat(nc); return false; }
+  double g[4] = {p0 / n, -p1 / n, -p2 / n, -p3 / n};
+  double q[4];
+  su2_pow(g, omega, q);
+  *gs = embed_su2(q, i, j, nc);
+  return true;
+}
+
+// The site's gauge transformation G from K(x).  SU(2): one step.  SU(3): the three SU(2)
+// subgroups (0,1),(0,2),(1,2) in this order, one pass, each seeing K already rotated by the
+// previous ones (C-6), omega applied per subgroup (C-10).
+Mat site_G(Mat K, double omega, int nc) {
+  Mat G = unit_mat(nc);
+  static const int pairs[3][2] = {{0, 1}, {0, 2}, {1, 2}};
+  int npairs = (nc == 2) ? 1 : 3;
+  for (int t = 0; t < npairs; ++t) {
+    Mat gs;
+    if (!subgroup_step(K, pairs[t][0], pairs[t][1], omega, nc, &gs)) continue;
+    K = mul(gs, K, nc);
+    G = mul(gs, G, nc);
+  }
+  return G;
+}
+
+}  // namespace
+
+extern "C" {
+
+// Number of OpenMP threads used across independent sites (1 = serial).  Returns the value set.
+int oracle_set_threads(int n) {
+#ifdef _OPENMP
+  g_threads = n < 1 ? 1 : n;
+#else
+  (void)n;
+  g_threads = 1;
+#endif
+  return g_threads;
+}
+
+int oracle_max_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+void oracle_su2_pow(const double* q, double omega, double* out) { su2_pow(q, omega, out); }
+
+// K(x) for every site: out is double[V][nc][nc][2].  eq. (3).
+void oracle_K(const int32_t* dims, int nc, const double* U, double* out) {
+  Lat L = make_lat(dims, nc);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) store_mat(out + s * nc * nc * 2, nc, gather_K(U, L, s));
+}
+
+// G for a given K (one site): K, G are double[nc][nc][2].  P:L50-54.
+void oracle_site_G(int nc, const double* K, double omega, double* G) {
+  store_mat(G, nc, site_G(load_mat(K, nc), omega, nc));
+}
+
+// One subgroup step on a given K: gs = embedded q^omega, returns 1 if |p| > 0.
+int oracle_subgroup_step(int nc, const double* K, int i, int j, double omega, double* gs) {
+  Mat g;
+  bool ok = subgroup_step(load_mat(K, nc), i, j, omega, nc, &g);
+  store_mat(gs, nc, g);
+  return ok ? 1 : 0;
+}
+
+// One HALF sweep over the sites of `parity`, in place (P:L54 checkerboard; C-12).
+//   K = sum_mu U_mu(x) + U_mu(x-mu)^dagger                        eq. (3)
+//   G = site_G(K, omega)
+//   U_mu(x) <- G U_mu(x);  U_mu(x-mu) <- U_mu(x-mu) G^dagger      P:L19-21 with g = 1 elsewhere
+void oracle_or_sweep(const int32_t* dims, int nc, double* U, int parity, double omega) {
+  Lat L = make_lat(dims, nc);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    if (parity_of(L, s) != parity) continue;
+    Mat G = site_G(gather_K(U, L, s), omega, nc);
+    Mat Gd = dagger(G, nc);
+    for (int mu = 0; mu < 4; ++mu) {
+      double* up = link_ptr(U, L, s, mu);
+      store_mat(up, nc, mul(G, load_mat(up, nc), nc));
+      double* dn = link_ptr(U, L, neighbour(L, s, mu, -1), mu);
+      store_mat(dn, nc, mul(load_mat(dn, nc), Gd, nc));
+    }
+  }
+}
+
+// F^U = 1/(N_d N_c V) sum_x sum_mu Re tr U_mu(x)     eq. (2) at g = 1; N_d = 4.
+double oracle_functional(const int32_t* dims, int nc, const double* U) {
+  Lat L = make_lat(dims, nc);
+  std::vector<double> term(L.V);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    double t = 0.0;
+    for (int mu = 0; mu < 4; ++mu) t += trace(load_mat(link_ptr(U, L, s, mu), nc), nc).real();
+    term[s] = t;
+  }
+  return neumaier_sum(term.data(), L.V) / (4.0 * nc * (double)L.V);
+}
+
+namespace {
+// A_mu(x) = [ (U - U^dagger) / (2i) ]_traceless with a*g = 1 (C-4).   P:L31-33.
+Mat gauge_field_A(const Mat& Um, int nc) {
+  Mat Ud = dagger(Um, nc);
+  Mat A = zero_mat();
+  const cd two_i(0.0, 2.0);
+  for (int a = 0; a < nc; ++a)
+    for (int b = 0; b < nc; ++b) A.e[a][b] = (Um.e[a][b] - Ud.e[a][b]) / two_i;
+  cd tr = trace(A, nc) / (double)nc;
+  for (int a = 0; a < nc; ++a) A.e[a][a] -= tr;
+  return A;
+}
+// Delta(x) = sum_mu ( A_mu(x) - A_mu(x - mu) )     eq. (1).
+Mat delta_at(const double* U, const Lat& L, int64_t s) {
+  Mat D = zero_mat();
+  for (int mu = 0; mu < 4; ++mu) {
+    Mat Ax = gauge_field_A(load_mat(link_ptr(U, L, s, mu), L.nc), L.nc);
+    Mat Ad = gauge_field_A(load_mat(link_ptr(U, L, neighbour(L, s, mu, -1), mu), L.nc), L.nc);
+    for (int a = 0; a < L.nc; ++a)
+      for (int b = 0; b < L.nc; ++b) D.e[a][b] += Ax.e[a][b] - Ad.e[a][b];
+  }
+  return D;
+}
+}  // namespace
+
+// Delta(x) for every site: out is double[V][nc][nc][2].
+void oracle_delta(const int32_t* dims, int nc, const double* U, double* out) {
+  Lat L = make_lat(dims, nc);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) store_mat(out + s * nc * nc * 2, nc, delta_at(U, L, s));
+}
+
+// theta = 1/(N_c V) sum_x tr[ Delta(x) Delta(x)^dagger ]   (BASELINE.json north_star; C-5).
+double oracle_gauge_precision(const int32_t* dims, int nc, const double* U) {
+  Lat L = make_lat(dims, nc);
+  std::vector<double> term(L.V);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    Mat D = delta_at(U, L, s);
+    term[s] = trace(mul(D, dagger(D, nc), nc), nc).real();
+  }
+  return neumaier_sum(term.data(), L.V) / ((double)nc * (double)L.V);
+}
+
+// U_mu(x) <- g(x) U_mu(x) g(x+mu)^dagger for all x, mu.  g is double[V][nc][nc][2], read-only.
+void oracle_gauge_transform(const int32_t* dims, int nc, double* U, const double* g) {
+  Lat L = make_lat(dims, nc);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    Mat gx = load_mat(g + s * nc * nc * 2, nc);
+    for (int mu = 0; mu < 4; ++mu) {
+      Mat gf = load_mat(g + neighbour(L, s, mu, +1) * nc * nc * 2, nc);
+      double* p = link_ptr(U, L, s, mu);
+      store_mat(p, nc, mul(mul(gx, load_mat(p, nc), nc), dagger(gf, nc), nc));
+    }
+  }
+}
+
+// Average plaquette 1/(6 N_c V) sum_x sum_{mu<nu} Re tr[U_mu(x) U_nu(x+mu) U_mu(x+nu)^dagger U_nu(x)^dagger].
+// Test-only gauge-invariant observable (not on the hot path).
+double oracle_plaquette(const int32_t* dims, int nc, const double* U) {
+  Lat L = make_lat(dims, nc);
+  std::vector<double> term(L.V);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    double t = 0.0;
+    for (int mu = 0; mu < 4; ++mu)
+      for (int nu = mu + 1; nu < 4; ++nu) {
+        Mat a = load_mat(link_ptr(U, L, s, mu), nc);
+        Mat b = load_mat(link_ptr(U, L, neighbour(L, s, mu, +1), nu), nc);
+        Mat c = dagger(load_mat(link_ptr(U, L, neighbour(L, s, nu, +1), mu), nc), nc);
+        Mat d = dagger(load_mat(link_ptr(U, L, s, nu), nc), nc);
+        t += trace(mul(mul(a, b, nc), mul(c, d, nc), nc), nc).real();
+      }
+    term[s] = t;
+  }
+  return neumaier_sum(term.data(), L.V) / (6.0 * nc * (double)L.V);
+}
+
+// 12-parameter representation: keep rows 0,1 of every SU(3) link, rebuild
+// row 2 = conj(row0 x row1) in fp64.  n = number of 3x3 matrices in `M` (double[n][3][3][2]).
+// Used to give the oracle exactly the field a 12-parameter store holds.
+void oracle_reconstruct12(int64_t n, double* M) {
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t k = 0; k < n; ++k) {
+    Mat m = load_mat(M + k * 18, 3);
+    m.e[2][0] = std::conj(m.e[0][1] * m.e[1][2] - m.e[0][2] * m.e[1][1]);
+    m.e[2][1] = std::conj(m.e[0][2] * m.e[1][0] - m.e[0][0] * m.e[1][2]);
+    m.e[2][2] = std::conj(m.e[0][0] * m.e[1][1] - m.e[0][1] * m.e[1][0]);
+    store_mat(M + k * 18, 3, m);
+  }
+}
+
+}  // extern "C"
