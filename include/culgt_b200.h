@@ -1,0 +1,136 @@
+/* culgt_b200.h -- C ABI of libculgt_b200.so: the checkerboard overrelaxation sweep for lattice
+ * Landau gauge fixing (arXiv:1412.3655 "cuLGT: Lattice Gauge Fixing on GPUs"), hand-written
+ * CUDA for sm_100a (NVIDIA B200).
+ *
+ * Citations: P:Lnn = PAPER.md line nn of the reference text; C-n = reading n in DESIGN.md.
+ *
+ * General rules
+ *   - Every function returns an int status (CULGT_OK = 0, errors < 0) unless it returns a size.
+ *     Nothing throws, aborts, prints or allocates device memory.
+ *   - "device pointer" = address in the current CUDA device's global memory, 16-byte aligned,
+ *     owned (allocated and freed) by the caller.  "host pointer" = ordinary host memory owned
+ *     by the caller (pinned memory makes the *_host calls faster but is not required).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls
+ *     taking a stream only ENQUEUE work and return without synchronising, except where stated.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns CULGT_ERR_CUDA.
+ *   - Non-unitary input is not detected (garbage in, garbage out).
+ *
+ * Lattice and layouts
+ *   dims = {N0,N1,N2,N3} = x,y,z,t extents, periodic in all directions (C-2); every extent must
+ *   be even and >= 2 (an odd extent breaks the checkerboard across the wrap).
+ *   Canonical site index  s = x0 + N0*(x1 + N1*(x2 + N2*x3));  parity(x) = (x0+x1+x2+x3)&1,
+ *   0 = "black", 1 = "white" (C-1); mu = 0..3 <-> x,y,z,t (C-3).
+ *   CANONICAL field  : real[V][4][Nc][Nc][2]  site-major, full Nc x Nc complex matrices,
+ *                      row-major, re/im interleaved (the interchange format a host framework
+ *                      hands over, "linear float or double array of length V*Nd*2Nc^2").
+ *   CANONICAL g field: real[V][Nc][Nc][2].
+ *   INTERNAL field   : links[parity][mu][j][h], parity-split, site-fastest structure of arrays
+ *                      ("site index runs faster than Lorentz and matrix indices") of
+ *                      vectors: SU(3) 12-parameter fp32 = 3 x float4, fp64 = 6 x double2;
+ *                      18-parameter fp32 = 9 x float2, fp64 = 9 x double2; SU(2) 4-parameter
+ *                      fp32 = 1 x float4 (a0,a1,a2,a3), fp64 = 2 x double2.  h = s>>1 is the
+ *                      index of the site inside its parity.  Opaque to the caller: use
+ *                      culgt_pack / culgt_unpack.  `real` = float (precision 32) or double (64)
+ *                      for BOTH the canonical and the internal field.
+ */
+#ifndef CULGT_B200_H
+#define CULGT_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CULGT_OK            0
+#define CULGT_ERR_NULL     -1  /* a required pointer is NULL                                  */
+#define CULGT_ERR_DIMS     -2  /* an extent is odd, < 2, or the volume overflows int32 indices */
+#define CULGT_ERR_DESC     -3  /* group / precision / params combination not provided         */
+#define CULGT_ERR_PARITY   -4  /* parity is not 0 or 1                                         */
+#define CULGT_ERR_OMEGA    -5  /* omega is NaN or outside [1,2)                        */
+#define CULGT_ERR_ALIGN    -6  /* a device pointer is not 16-byte aligned                      */
+#define CULGT_ERR_CUDA     -7  /* CUDA runtime / launch failure (see culgt_last_cuda_error)    */
+#define CULGT_ERR_ARG      -8  /* another argument is out of range                             */
+
+typedef struct {
+  int32_t dims[4];    /* N0..N3, x fastest in the canonical site index                        */
+  int32_t group;      /* 2 = SU(2), 3 = SU(3)                                                 */
+  int32_t precision;  /* 32 or 64                                                             */
+  int32_t params;     /* SU(3): 18 (full) or 12 (first two rows); SU(2): 4             */
+} culgt_lattice;
+
+/* Sizes in bytes; 0 if the descriptor is invalid. */
+size_t culgt_links_bytes(const culgt_lattice* lat);      /* internal field: 4*V*params*sizeof(real) */
+size_t culgt_canonical_bytes(const culgt_lattice* lat);  /* V*4*Nc*Nc*2*sizeof(real)                */
+size_t culgt_gfield_bytes(const culgt_lattice* lat);     /* V*Nc*Nc*2*sizeof(real)                  */
+size_t culgt_workspace_bytes(const culgt_lattice* lat);  /* reductions: block partials + 2 scalars   */
+
+/* Validate a descriptor: CULGT_OK, CULGT_ERR_NULL, CULGT_ERR_DIMS or CULGT_ERR_DESC. */
+int culgt_validate(const culgt_lattice* lat);
+
+/* a0: canonical <-> internal (P:L64 reordering into black/white sublattices; "discarding
+ * the third line" on pack, implicit reconstruction row2 = conj(row0 x row1) on unpack).
+ * canonical, links: device pointers (distinct buffers).  Asynchronous on `stream`. */
+int culgt_pack(const culgt_lattice* lat, const void* canonical, void* links, void* stream);
+int culgt_unpack(const culgt_lattice* lat, const void* links, void* canonical, void* stream);
+
+/* a1-a6: ONE HALF sweep of overrelaxation over all sites x of `parity`, in place:
+ *   K(x) = sum_mu [ U_mu(x) + U_mu(x-mu)^dagger ]                         eq. (3)
+ *   SU(2): g = K^dagger/sqrt(det K^dagger), G = g^omega
+ *   SU(3): for the subgroups (0,1),(0,2),(1,2): g_s from the block of the current K, raised to
+ *          omega, K <- g_s K, G <- g_s G  (C-6, C-10); g^omega is the exact group power (C-8)
+ *   U_mu(x) <- G U_mu(x),  U_mu(x-mu) <- U_mu(x-mu) G^dagger
+ * links: device pointer to the internal field.  omega in [1,2).  Asynchronous on `stream`.
+ * Arithmetic: precision 64 -> all fp64.  precision 32 -> link storage, reconstruction and the 8
+ * link products in fp32; K accumulation and the subgroup solve in fp64 (C-15). */
+int culgt_or_sweep(const culgt_lattice* lat, void* links, int parity, double omega, void* stream);
+
+/* n_sweeps full sweeps (black then white half-sweep each; C-12), enqueued back to back. */
+int culgt_or_sweeps(const culgt_lattice* lat, void* links, int n_sweeps, double omega, void* stream);
+
+/* a8: theta = 1/(Nc V) sum_x tr[Delta(x) Delta(x)^dagger],  Delta = sum_mu A_mu(x) - A_mu(x-mu),
+ * A_mu = [(U_mu - U_mu^dagger)/(2i)]_traceless with a*g = 1 (eq. (1); C-4, C-5).
+ * a7: F = 1/(4 Nc V) sum_x sum_mu Re tr U_mu(x) (eq. (2) at g = 1).
+ * workspace: device pointer, >= culgt_workspace_bytes.  The fp64 scalar is written to the DEVICE
+ * address *_dev; the reduction is deterministic (fixed order, fp64).  Asynchronous on `stream`. */
+int culgt_gauge_precision(const culgt_lattice* lat, const void* links, void* workspace,
+                          double* theta_dev, void* stream);
+int culgt_functional(const culgt_lattice* lat, const void* links, void* workspace,
+                     double* F_dev, void* stream);
+
+/* a9: U_mu(x) <- g(x) U_mu(x) g(x+mu)^dagger for all x, mu (the paper's worked code
+ * example P:L105-118).  g: device pointer to a canonical g field (read-only); links in place. */
+int culgt_gauge_transform(const culgt_lattice* lat, void* links, const void* g, void* stream);
+
+/* The paper's driver loop ("iterated until the discrete gauge condition (1) is satisfied
+ * up to a given numerical precision"): full sweeps until theta < theta_target or max_sweeps,
+ * theta checked every check_every sweeps (and before the first).  SYNCHRONISES the stream at
+ * each check.  Outputs are HOST pointers (any may be NULL). */
+int culgt_landau_fix(const culgt_lattice* lat, void* links, void* workspace, double omega,
+                     double theta_target, int max_sweeps, int check_every,
+                     int* sweeps_done, double* theta_out, double* F_out, void* stream);
+
+/* End-to-end call with HOST buffers: copies the canonical field host->device, packs, runs
+ * n_sweeps full sweeps, computes theta and F, unpacks and copies the fixed field back to the
+ * host (canonical_host is updated in place).  Device scratch is supplied by the caller:
+ * canonical_dev >= culgt_canonical_bytes, links_dev >= culgt_links_bytes, workspace >=
+ * culgt_workspace_bytes.  SYNCHRONISES before returning.  theta_out / F_out: host pointers. */
+int culgt_fix_host(const culgt_lattice* lat, void* canonical_host, void* canonical_dev,
+                   void* links_dev, void* workspace, int n_sweeps, double omega,
+                   double* theta_out, double* F_out, void* stream);
+
+/* Kernel-variant selection for measurement: variant 0 = the default chosen
+ * by measurement; other values select alternative thread-to-site mappings where provided.
+ * Returns CULGT_OK or CULGT_ERR_ARG.  Process-global; not thread-safe. */
+int culgt_set_sweep_variant(int variant);
+int culgt_get_sweep_variant(void);
+
+const char* culgt_strerror(int status);
+const char* culgt_last_cuda_error(void);
+int culgt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CULGT_B200_H */

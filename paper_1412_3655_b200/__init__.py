@@ -1,0 +1,256 @@
+"""paper_1412_3655_b200 -- B200-native checkerboard overrelaxation for lattice Landau gauge fixing.
+
+Thin Python binding of the C-ABI library libculgt_b200.so (include/culgt_b200.h): the functions
+here have the same names as the C entry points and only marshal arguments (torch tensors ->
+device pointers, the current torch stream -> cudaStream_t).  Every step of the method runs in
+the CUDA kernels under csrc/.  PyTorch is used for device memory and streams only.
+
+There is NO CPU fallback: importing works anywhere (so the ABI can be inspected), but the
+library must have been built (python -m paper_1412_3655_b200.build) and every compute call
+needs a CUDA device, else it raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libculgt_b200.so")
+
+CULGT_OK = 0
+ERRORS = {
+    "CULGT_ERR_NULL": -1, "CULGT_ERR_DIMS": -2, "CULGT_ERR_DESC": -3, "CULGT_ERR_PARITY": -4,
+    "CULGT_ERR_OMEGA": -5, "CULGT_ERR_ALIGN": -6, "CULGT_ERR_CUDA": -7, "CULGT_ERR_ARG": -8,
+}
+FLOPS_PER_SITE = {3: 2304, 2: 278}   # fixed algorithmic counts, DESIGN.md "Measurement"
+
+
+class CulgtError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().culgt_strerror(status).decode()
+        if status == ERRORS["CULGT_ERR_CUDA"]:
+            msg += ": " + lib().culgt_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} ({status})")
+
+
+class culgt_lattice(ctypes.Structure):
+    _fields_ = [("dims", ctypes.c_int32 * 4), ("group", ctypes.c_int32),
+                ("precision", ctypes.c_int32), ("params", ctypes.c_int32)]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libculgt_b200.so (fails loudly if it has not been built)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with "
+                          "`python -m paper_1412_3655_b200.build` (there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    latp = ctypes.POINTER(culgt_lattice)
+    vp = ctypes.c_void_p
+    dp = ctypes.POINTER(ctypes.c_double)
+    for name in ("culgt_links_bytes", "culgt_canonical_bytes", "culgt_gfield_bytes", "culgt_workspace_bytes"):
+        getattr(L, name).argtypes = [latp]
+        getattr(L, name).restype = ctypes.c_size_t
+    L.culgt_validate.argtypes = [latp]
+    L.culgt_pack.argtypes = [latp, vp, vp, vp]
+    L.culgt_unpack.argtypes = [latp, vp, vp, vp]
+    L.culgt_or_sweep.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
+    L.culgt_or_sweeps.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
+    L.culgt_gauge_precision.argtypes = [latp, vp, vp, vp, vp]
+    L.culgt_functional.argtypes = [latp, vp, vp, vp, vp]
+    L.culgt_gauge_transform.argtypes = [latp, vp, vp, vp]
+    L.culgt_landau_fix.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+                                   ctypes.c_int, ctypes.POINTER(ctypes.c_int), dp, dp, vp]
+    L.culgt_fix_host.argtypes = [latp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_double, dp, dp, vp]
+    L.culgt_set_sweep_variant.argtypes = [ctypes.c_int]
+    L.culgt_strerror.argtypes = [ctypes.c_int]
+    L.culgt_strerror.restype = ctypes.c_char_p
+    L.culgt_last_cuda_error.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+@dataclass(frozen=True)
+class Lattice:
+    """Python mirror of the C `culgt_lattice` descriptor."""
+    dims: tuple
+    group: int = 3
+    precision: int = 32
+    params: int = 12
+
+    def c(self) -> culgt_lattice:
+        return culgt_lattice((ctypes.c_int32 * 4)(*[int(d) for d in self.dims]),
+                             int(self.group), int(self.precision), int(self.params))
+
+    @property
+    def volume(self) -> int:
+        v = 1
+        for d in self.dims:
+            v *= int(d)
+        return v
+
+    @property
+    def torch_dtype(self):
+        import torch
+        return torch.float32 if self.precision == 32 else torch.float64
+
+
+def _check(status: int, where: str) -> None:
+    if status != CULGT_OK:
+        raise CulgtError(status, where)
+
+
+def _ptr(t) -> int:
+    """Device (or host) address of a torch tensor / numpy array / raw int / None."""
+    if t is None:
+        return 0
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    if hasattr(t, "ctypes"):
+        return t.ctypes.data
+    raise TypeError(f"cannot take the address of {type(t)}")
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _require_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1412_3655_b200 needs a CUDA device; there is no CPU fallback")
+
+
+# ---- sizes -----------------------------------------------------------------------------------
+
+def culgt_validate(lat: Lattice) -> int:
+    return lib().culgt_validate(ctypes.byref(lat.c()))
+
+
+def culgt_links_bytes(lat: Lattice) -> int:
+    return lib().culgt_links_bytes(ctypes.byref(lat.c()))
+
+
+def culgt_canonical_bytes(lat: Lattice) -> int:
+    return lib().culgt_canonical_bytes(ctypes.byref(lat.c()))
+
+
+def culgt_gfield_bytes(lat: Lattice) -> int:
+    return lib().culgt_gfield_bytes(ctypes.byref(lat.c()))
+
+
+def culgt_workspace_bytes(lat: Lattice) -> int:
+    return lib().culgt_workspace_bytes(ctypes.byref(lat.c()))
+
+
+# ---- device-memory helpers (torch is the allocator) -------------------------------------------
+
+def alloc_links(lat: Lattice, device="cuda"):
+    import torch
+    n = culgt_links_bytes(lat)
+    if n == 0:
+        _check(culgt_validate(lat), "alloc_links")
+    return torch.empty(n // (lat.precision // 8), dtype=lat.torch_dtype, device=device)
+
+
+def alloc_workspace(lat: Lattice, device="cuda"):
+    import torch
+    return torch.empty(culgt_workspace_bytes(lat) // 8, dtype=torch.float64, device=device)
+
+
+# ---- the C entry points, same names ------------------------------------------------------------
+
+def culgt_pack(lat: Lattice, canonical, links, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_pack(ctypes.byref(lat.c()), _ptr(canonical), _ptr(links), _stream(stream)), "culgt_pack")
+
+
+def culgt_unpack(lat: Lattice, links, canonical, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_unpack(ctypes.byref(lat.c()), _ptr(links), _ptr(canonical), _stream(stream)), "culgt_unpack")
+
+
+def culgt_or_sweep(lat: Lattice, links, parity: int, omega: float, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_or_sweep(ctypes.byref(lat.c()), _ptr(links), int(parity), float(omega),
+                                _stream(stream)), "culgt_or_sweep")
+
+
+def culgt_or_sweeps(lat: Lattice, links, n_sweeps: int, omega: float, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_or_sweeps(ctypes.byref(lat.c()), _ptr(links), int(n_sweeps), float(omega),
+                                 _stream(stream)), "culgt_or_sweeps")
+
+
+def culgt_gauge_precision(lat: Lattice, links, workspace, theta_dev, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_gauge_precision(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace),
+                                       _ptr(theta_dev), _stream(stream)), "culgt_gauge_precision")
+
+
+def culgt_functional(lat: Lattice, links, workspace, F_dev, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_functional(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace),
+                                  _ptr(F_dev), _stream(stream)), "culgt_functional")
+
+
+def culgt_gauge_transform(lat: Lattice, links, g, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_gauge_transform(ctypes.byref(lat.c()), _ptr(links), _ptr(g), _stream(stream)),
+           "culgt_gauge_transform")
+
+
+def culgt_landau_fix(lat: Lattice, links, workspace, omega: float, theta_target: float,
+                     max_sweeps: int, check_every: int = 1, stream=None):
+    """Returns (sweeps_done, theta, F)."""
+    _require_cuda()
+    done = ctypes.c_int(0)
+    theta = ctypes.c_double(0.0)
+    F = ctypes.c_double(0.0)
+    _check(lib().culgt_landau_fix(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace), float(omega),
+                                  float(theta_target), int(max_sweeps), int(check_every),
+                                  ctypes.byref(done), ctypes.byref(theta), ctypes.byref(F),
+                                  _stream(stream)), "culgt_landau_fix")
+    return done.value, theta.value, F.value
+
+
+def culgt_fix_host(lat: Lattice, canonical_host, canonical_dev, links_dev, workspace,
+                   n_sweeps: int, omega: float, stream=None):
+    """Host-buffer end-to-end call; canonical_host is updated in place. Returns (theta, F)."""
+    _require_cuda()
+    theta = ctypes.c_double(0.0)
+    F = ctypes.c_double(0.0)
+    _check(lib().culgt_fix_host(ctypes.byref(lat.c()), _ptr(canonical_host), _ptr(canonical_dev),
+                                _ptr(links_dev), _ptr(workspace), int(n_sweeps), float(omega),
+                                ctypes.byref(theta), ctypes.byref(F), _stream(stream)), "culgt_fix_host")
+    return theta.value, F.value
+
+
+def culgt_set_sweep_variant(variant: int) -> None:
+    _check(lib().culgt_set_sweep_variant(int(variant)), "culgt_set_sweep_variant")
+
+
+def culgt_get_sweep_variant() -> int:
+    return lib().culgt_get_sweep_variant()
+
+
+def culgt_version() -> int:
+    return lib().culgt_version()
+
+
+def culgt_strerror(status: int) -> str:
+    return lib().culgt_strerror(int(status)).decode()

@@ -1,0 +1,265 @@
+// api.cu -- the C ABI of libculgt_b200.so (include/culgt_b200.h): descriptor validation, error
+// codes and dispatch to the kernel launchers.  No compute happens here.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+#include "../../include/culgt_b200.h"
+#include "kernels.h"
+
+using namespace culgt;
+
+namespace {
+
+char g_cuda_err[256] = "";
+int g_variant = 0;
+
+int cuda_fail(cudaError_t e) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+  return CULGT_ERR_CUDA;
+}
+
+int describe(const culgt_lattice* lat, LatticeDesc* d) {
+  if (!lat) return CULGT_ERR_NULL;
+  long long v = 1;
+  for (int i = 0; i < 4; ++i) {
+    const int n = lat->dims[i];
+    if (n < 2 || (n & 1)) return CULGT_ERR_DIMS;
+    v *= n;
+    if (v > (1ll << 30)) return CULGT_ERR_DIMS;   // 32-bit site indices, 8*V thread indices in 64-bit
+  }
+  const bool prec_ok = lat->precision == 32 || lat->precision == 64;
+  const bool su3 = lat->group == 3 && (lat->params == 18 || lat->params == 12);
+  const bool su2 = lat->group == 2 && lat->params == 4;
+  if (!prec_ok || !(su3 || su2)) return CULGT_ERR_DESC;
+  if (d) {
+    d->geom = make_geom(lat->dims);
+    d->group = lat->group;
+    d->precision = lat->precision;
+    d->params = lat->params;
+    d->V = v;
+  }
+  return CULGT_OK;
+}
+
+bool misaligned(const void* p) { return ((uintptr_t)p & 15u) != 0; }
+
+}  // namespace
+
+extern "C" {
+
+int culgt_validate(const culgt_lattice* lat) { return describe(lat, nullptr); }
+
+size_t culgt_links_bytes(const culgt_lattice* lat) {
+  LatticeDesc d;
+  if (describe(lat, &d) != CULGT_OK) return 0;
+  return (size_t)4 * (size_t)d.V * (size_t)d.params * (size_t)(d.precision / 8);
+}
+
+size_t culgt_canonical_bytes(const culgt_lattice* lat) {
+  LatticeDesc d;
+  if (describe(lat, &d) != CULGT_OK) return 0;
+  return (size_t)4 * (size_t)d.V * (size_t)(2 * d.group * d.group) * (size_t)(d.precision / 8);
+}
+
+size_t culgt_gfield_bytes(const culgt_lattice* lat) {
+  LatticeDesc d;
+  if (describe(lat, &d) != CULGT_OK) return 0;
+  return (size_t)d.V * (size_t)(2 * d.group * d.group) * (size_t)(d.precision / 8);
+}
+
+size_t culgt_workspace_bytes(const culgt_lattice* lat) {
+  if (describe(lat, nullptr) != CULGT_OK) return 0;
+  return (size_t)(kMaxReduceBlocks + 2) * sizeof(double);   // block partials + {theta, F} scalars
+}
+
+int culgt_pack(const culgt_lattice* lat, const void* canonical, void* links, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!canonical || !links) return CULGT_ERR_NULL;
+  if (misaligned(canonical) || misaligned(links)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_pack(d, canonical, links, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_unpack(const culgt_lattice* lat, const void* links, void* canonical, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!canonical || !links) return CULGT_ERR_NULL;
+  if (misaligned(canonical) || misaligned(links)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_unpack(d, links, canonical, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+static int check_omega(double omega) {
+  if (!(omega >= 1.0 && omega < 2.0)) return CULGT_ERR_OMEGA;   // NaN fails the comparison
+  return CULGT_OK;
+}
+
+int culgt_or_sweep(const culgt_lattice* lat, void* links, int parity, double omega, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (parity != 0 && parity != 1) return CULGT_ERR_PARITY;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  cudaError_t e = launch_or_sweep(d, links, parity, omega, g_variant, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_or_sweeps(const culgt_lattice* lat, void* links, int n_sweeps, double omega, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (n_sweeps < 0) return CULGT_ERR_ARG;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  for (int i = 0; i < n_sweeps; ++i)
+    for (int parity = 0; parity < 2; ++parity) {
+      cudaError_t e = launch_or_sweep(d, links, parity, omega, g_variant, (cudaStream_t)stream);
+      if (e != cudaSuccess) return cuda_fail(e);
+    }
+  return CULGT_OK;
+}
+
+int culgt_gauge_precision(const culgt_lattice* lat, const void* links, void* workspace,
+                          double* theta_dev, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !workspace || !theta_dev) return CULGT_ERR_NULL;
+  if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_gauge_precision(d, links, (double*)workspace, theta_dev, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_functional(const culgt_lattice* lat, const void* links, void* workspace,
+                     double* F_dev, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !workspace || !F_dev) return CULGT_ERR_NULL;
+  if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_functional(d, links, (double*)workspace, F_dev, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_gauge_transform(const culgt_lattice* lat, void* links, const void* g, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !g) return CULGT_ERR_NULL;
+  if (misaligned(links) || misaligned(g)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_gauge_transform(d, links, g, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+// theta and F into the two doubles that follow the block partials in the workspace, read back.
+static int read_theta_F(const LatticeDesc& d, const void* links, void* workspace, cudaStream_t st,
+                        double* theta, double* F) {
+  double* ws = (double*)workspace;
+  double* scal = ws + kMaxReduceBlocks;
+  cudaError_t e = launch_gauge_precision(d, links, ws, scal, st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  if (F) {
+    e = launch_functional(d, links, ws, scal + 1, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+  }
+  double host[2] = {0, 0};
+  e = cudaMemcpyAsync(host, scal, (F ? 2 : 1) * sizeof(double), cudaMemcpyDeviceToHost, st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  *theta = host[0];
+  if (F) *F = host[1];
+  return CULGT_OK;
+}
+
+int culgt_landau_fix(const culgt_lattice* lat, void* links, void* workspace, double omega,
+                     double theta_target, int max_sweeps, int check_every,
+                     int* sweeps_done, double* theta_out, double* F_out, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !workspace) return CULGT_ERR_NULL;
+  if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
+  if (max_sweeps < 0 || check_every < 1) return CULGT_ERR_ARG;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  double theta = 0, F = 0;
+  int done = 0;
+  if ((rc = read_theta_F(d, links, workspace, st, &theta, nullptr)) != CULGT_OK) return rc;
+  while (theta >= theta_target && done < max_sweeps) {
+    int n = check_every;
+    if (done + n > max_sweeps) n = max_sweeps - done;
+    for (int i = 0; i < n; ++i)
+      for (int parity = 0; parity < 2; ++parity) {
+        cudaError_t e = launch_or_sweep(d, links, parity, omega, g_variant, st);
+        if (e != cudaSuccess) return cuda_fail(e);
+      }
+    done += n;
+    if ((rc = read_theta_F(d, links, workspace, st, &theta, nullptr)) != CULGT_OK) return rc;
+  }
+  if ((rc = read_theta_F(d, links, workspace, st, &theta, &F)) != CULGT_OK) return rc;
+  if (sweeps_done) *sweeps_done = done;
+  if (theta_out) *theta_out = theta;
+  if (F_out) *F_out = F;
+  return CULGT_OK;
+}
+
+int culgt_fix_host(const culgt_lattice* lat, void* canonical_host, void* canonical_dev,
+                   void* links_dev, void* workspace, int n_sweeps, double omega,
+                   double* theta_out, double* F_out, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!canonical_host || !canonical_dev || !links_dev || !workspace) return CULGT_ERR_NULL;
+  if (misaligned(canonical_dev) || misaligned(links_dev) || misaligned(workspace)) return CULGT_ERR_ALIGN;
+  if (n_sweeps < 0) return CULGT_ERR_ARG;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t cbytes = culgt_canonical_bytes(lat);
+  cudaError_t e = cudaMemcpyAsync(canonical_dev, canonical_host, cbytes, cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  if ((e = launch_pack(d, canonical_dev, links_dev, st)) != cudaSuccess) return cuda_fail(e);
+  for (int i = 0; i < n_sweeps; ++i)
+    for (int parity = 0; parity < 2; ++parity)
+      if ((e = launch_or_sweep(d, links_dev, parity, omega, g_variant, st)) != cudaSuccess) return cuda_fail(e);
+  if ((e = launch_unpack(d, links_dev, canonical_dev, st)) != cudaSuccess) return cuda_fail(e);
+  e = cudaMemcpyAsync(canonical_host, canonical_dev, cbytes, cudaMemcpyDeviceToHost, st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  double theta = 0, F = 0;
+  if ((rc = read_theta_F(d, links_dev, workspace, st, &theta, &F)) != CULGT_OK) return rc;
+  if (theta_out) *theta_out = theta;
+  if (F_out) *F_out = F;
+  return CULGT_OK;
+}
+
+int culgt_set_sweep_variant(int variant) {
+  if (variant < 0 || variant > 99) return CULGT_ERR_ARG;
+  g_variant = variant;
+  return CULGT_OK;
+}
+int culgt_get_sweep_variant(void) { return g_variant; }
+
+const char* culgt_strerror(int status) {
+  switch (status) {
+    case CULGT_OK: return "ok";
+    case CULGT_ERR_NULL: return "null pointer";
+    case CULGT_ERR_DIMS: return "lattice extents must be even, >= 2, volume <= 2^30";
+    case CULGT_ERR_DESC: return "unsupported group/precision/params combination";
+    case CULGT_ERR_PARITY: return "parity must be 0 or 1";
+    case CULGT_ERR_OMEGA: return "omega must be in [1,2)";
+    case CULGT_ERR_ALIGN: return "device pointer not 16-byte aligned";
+    case CULGT_ERR_CUDA: return "CUDA error (see culgt_last_cuda_error)";
+    case CULGT_ERR_ARG: return "argument out of range";
+    default: return "unknown status";
+  }
+}
+const char* culgt_last_cuda_error(void) { return g_cuda_err; }
+int culgt_version(void) { return 100; }
+
+}  // extern "C"

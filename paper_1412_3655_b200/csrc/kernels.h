@@ -1,0 +1,29 @@
+// kernels.h -- internal (C++) interface between the C-ABI layer (api.cu) and the kernel files.
+#pragma once
+#include <cuda_runtime.h>
+#include "lattice.cuh"
+
+namespace culgt {
+
+struct LatticeDesc {
+  Geom geom;
+  int group;      // 2 or 3
+  int precision;  // 32 or 64
+  int params;     // 18, 12 or 4
+  long long V;
+};
+
+constexpr int kReduceBlock = 256;       // threads per block of the reduction kernels
+constexpr int kMaxReduceBlocks = 4096;  // block partials kept in the workspace
+
+cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
+                            int variant, cudaStream_t st);
+cudaError_t launch_pack(const LatticeDesc& d, const void* canonical, void* links, cudaStream_t st);
+cudaError_t launch_unpack(const LatticeDesc& d, const void* links, void* canonical, cudaStream_t st);
+cudaError_t launch_gauge_precision(const LatticeDesc& d, const void* links, double* workspace,
+                                   double* out, cudaStream_t st);
+cudaError_t launch_functional(const LatticeDesc& d, const void* links, double* workspace,
+                              double* out, cudaStream_t st);
+cudaError_t launch_gauge_transform(const LatticeDesc& d, void* links, const void* g, cudaStream_t st);
+
+}  // namespace culgt

@@ -1,0 +1,192 @@
+// or_sweep.cu -- the checkerboard overrelaxation half-sweep kernels.
+//
+// For every site x of one parity:
+//   gather the 8 links touching x, K = sum_mu U_mu(x) + U_mu(x-mu)^dagger      (eq. 3)
+//   G from K by the SU(2) closed form / the SU(3) subgroup loop with g^omega   (L50-54)
+//   U_mu(x) <- G U_mu(x),  U_mu(x-mu) <- U_mu(x-mu) G^dagger                   (L19-21, L48)
+// Sites of one parity are independent (L54), so there is no synchronisation inside a launch.
+//
+// Thread-to-site mapping (the paper's 1 / 4 / 8 threads per site, L62-72, L122) is the template
+// parameter TPS: each of the TPS cooperating lanes owns 8/TPS links, the partial K are summed by
+// xor-shuffles (the warp-level analogue of the paper's shared-memory exchange) and every lane
+// then holds the same K and computes the same G.  Which TPS each storage uses is chosen by
+// measurement (profiles/).
+#include "lattice.cuh"
+#include "su_math.cuh"
+#include "kernels.h"
+
+namespace culgt {
+
+template <typename T>
+__device__ __forceinline__ T shfl_xor_t(T v, int mask);
+template <>
+__device__ __forceinline__ float shfl_xor_t<float>(float v, int mask) { return __shfl_xor_sync(0xffffffffu, v, mask); }
+template <>
+__device__ __forceinline__ double shfl_xor_t<double>(double v, int mask) { return __shfl_xor_sync(0xffffffffu, v, mask); }
+
+// ---------------------------------------------------------------------------------------------
+// SU(3).  S = storage traits, Acc = type of K and of the subgroup solve, TPS threads per site.
+// ---------------------------------------------------------------------------------------------
+template <typename S, typename Acc, int TPS, int BLOCK>
+__global__ void __launch_bounds__(BLOCK)
+or_sweep_su3_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity, const Acc omega) {
+  typedef typename S::Real Real;
+  constexpr int LPT = 8 / TPS;   // links per thread
+  const int tid = blockIdx.x * BLOCK + threadIdx.x;
+  int h = tid / TPS;
+  const int q = tid % TPS;
+  const bool active = h < g.vh;
+  if (!active) h = g.vh - 1;     // keep the lane alive for the shuffles; it stores nothing
+  const SiteCoord sc = decode_site(g, h, parity);
+
+  Real U[LPT][18];
+  typename S::Vec* ptr[LPT];
+#pragma unroll
+  for (int l = 0; l < LPT; ++l) {
+    const int slot = q * LPT + l;          // slot = 2*mu + (0: U_mu(x), 1: U_mu(x-mu))
+    const int mu = slot >> 1;
+    const bool dn = slot & 1;
+    const int idx = dn ? down_index(g, h, sc, mu) : h;
+    ptr[l] = link_base<S>(links, g, dn ? 1 - parity : parity, mu, idx);
+  }
+#pragma unroll
+  for (int l = 0; l < LPT; ++l) load_params<S>(ptr[l], g.vh, U[l]);
+  if (S::NP == 12) {
+#pragma unroll
+    for (int l = 0; l < LPT; ++l) reconstruct_row2(U[l]);
+  }
+
+  Acc K[18];
+#pragma unroll
+  for (int i = 0; i < 18; ++i) K[i] = 0;
+#pragma unroll
+  for (int l = 0; l < LPT; ++l) accumulate(K, U[l], ((q * LPT + l) & 1) != 0);
+#pragma unroll
+  for (int m = 1; m < TPS; m <<= 1) {
+#pragma unroll
+    for (int i = 0; i < 18; ++i) K[i] += shfl_xor_t<Acc>(K[i], m);
+  }
+
+  Acc Ga[18];
+  su3_site_G(K, Ga, omega);
+  Real G[18];
+#pragma unroll
+  for (int i = 0; i < 18; ++i) G[i] = (Real)Ga[i];
+
+  if (!active) return;
+  constexpr int NR = (S::NP == 12) ? 2 : 3;   // rows that are stored
+#pragma unroll
+  for (int l = 0; l < LPT; ++l) {
+    Real R[18];
+    if (((q * LPT + l) & 1) == 0) mul_ab<NR>(G, U[l], R);
+    else mul_abd<NR>(U[l], G, R);
+    store_params<S>(ptr[l], g.vh, R);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// SU(2), 4-parameter storage, one thread per site, all arithmetic in Real.
+// ---------------------------------------------------------------------------------------------
+template <typename S, int BLOCK>
+__global__ void __launch_bounds__(BLOCK)
+or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
+                    const typename S::Real omega) {
+  typedef typename S::Real Real;
+  const int h = blockIdx.x * BLOCK + threadIdx.x;
+  if (h >= g.vh) return;
+  const SiteCoord sc = decode_site(g, h, parity);
+  Real U[8][4];
+  typename S::Vec* ptr[8];
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) {
+    ptr[2 * mu] = link_base<S>(links, g, parity, mu, h);
+    ptr[2 * mu + 1] = link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu));
+  }
+#pragma unroll
+  for (int l = 0; l < 8; ++l) load_params<S>(ptr[l], g.vh, U[l]);
+  // K = k0 + i k.sigma = sum_mu u_up + conj(u_dn)
+  Real k[4] = {0, 0, 0, 0};
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) {
+    k[0] += U[2 * mu][0] + U[2 * mu + 1][0];
+#pragma unroll
+    for (int i = 1; i < 4; ++i) k[i] += U[2 * mu][i] - U[2 * mu + 1][i];
+  }
+  const Real n2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3];
+  if (n2 == 0) return;                               // K = 0: skip the update (C-9)
+  const Real ninv = rsqrt_t(n2);
+  Real G[4] = {k[0] * ninv, -k[1] * ninv, -k[2] * ninv, -k[3] * ninv};   // K^dagger / sqrt(det K^dagger)
+  su2_pow(G, omega);
+#pragma unroll
+  for (int l = 0; l < 8; ++l) {
+    Real R[4];
+    if ((l & 1) == 0) quat_mul(G, U[l], R);
+    else quat_mul_dag(U[l], G, R);
+    store_params<S>(ptr[l], g.vh, R);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-side launchers
+// ---------------------------------------------------------------------------------------------
+template <typename S, typename Acc, int TPS>
+static cudaError_t launch_su3(void* links, const Geom& g, int parity, double omega, cudaStream_t st) {
+  constexpr int BLOCK = 128;
+  const long long threads = (long long)g.vh * TPS;
+  const unsigned grid = (unsigned)((threads + BLOCK - 1) / BLOCK);
+  or_sweep_su3_kernel<S, Acc, TPS, BLOCK><<<grid, BLOCK, 0, st>>>(
+      (typename S::Vec*)links, g, parity, (Acc)omega);
+  return cudaGetLastError();
+}
+
+template <typename S>
+static cudaError_t launch_su2(void* links, const Geom& g, int parity, double omega, cudaStream_t st) {
+  constexpr int BLOCK = 128;
+  const unsigned grid = (unsigned)((g.vh + BLOCK - 1) / BLOCK);
+  or_sweep_su2_kernel<S, BLOCK><<<grid, BLOCK, 0, st>>>(
+      (typename S::Vec*)links, g, parity, (typename S::Real)omega);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
+                            int variant, cudaStream_t st) {
+  const Geom& g = d.geom;
+  if (d.group == 2) {
+    if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, g, parity, omega, st);
+    return launch_su2<Storage<double, 2, 4> >(links, g, parity, omega, st);
+  }
+  if (d.precision == 32) {
+    // fp32 storage: K and the subgroup solve in fp64 (reading C-15); variants 10+ are
+    // all-fp32 arithmetic, kept for the precision/throughput comparison in profiles/.
+    if (d.params == 12) {
+      switch (variant) {
+        case 0: case 1: return launch_su3<Storage<float, 3, 12>, double, 1>(links, g, parity, omega, st);
+        case 2: return launch_su3<Storage<float, 3, 12>, double, 2>(links, g, parity, omega, st);
+        case 4: return launch_su3<Storage<float, 3, 12>, double, 4>(links, g, parity, omega, st);
+        case 11: return launch_su3<Storage<float, 3, 12>, float, 1>(links, g, parity, omega, st);
+        case 14: return launch_su3<Storage<float, 3, 12>, float, 4>(links, g, parity, omega, st);
+        default: return cudaErrorInvalidValue;
+      }
+    }
+    switch (variant) {
+      case 0: case 2: return launch_su3<Storage<float, 3, 18>, double, 2>(links, g, parity, omega, st);
+      case 4: return launch_su3<Storage<float, 3, 18>, double, 4>(links, g, parity, omega, st);
+      default: return cudaErrorInvalidValue;
+    }
+  }
+  if (d.params == 12) {
+    switch (variant) {
+      case 0: case 4: return launch_su3<Storage<double, 3, 12>, double, 4>(links, g, parity, omega, st);
+      case 2: return launch_su3<Storage<double, 3, 12>, double, 2>(links, g, parity, omega, st);
+      case 8: return launch_su3<Storage<double, 3, 12>, double, 8>(links, g, parity, omega, st);
+      default: return cudaErrorInvalidValue;
+    }
+  }
+  switch (variant) {
+    case 0: case 4: return launch_su3<Storage<double, 3, 18>, double, 4>(links, g, parity, omega, st);
+    case 8: return launch_su3<Storage<double, 3, 18>, double, 8>(links, g, parity, omega, st);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace culgt

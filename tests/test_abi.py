@@ -1,0 +1,101 @@
+"""CPU-side checks of the C-ABI boundary: the library loads, exports every symbol that
+include/culgt_b200.h declares, sizes follow the formulas, and every argument error is reported
+by return code BEFORE any CUDA call (so these run without a GPU)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_1412_3655_b200 as culgt
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "culgt_b200.h")
+
+
+def declared_symbols():
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(culgt_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    lib = culgt.lib()
+    names = declared_symbols()
+    assert len(names) >= 19
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in culgt_b200.h but not exported"
+    # and the Python binding offers the same names
+    for n in names:
+        if n in ("culgt_last_cuda_error",):
+            continue
+        assert hasattr(culgt, n), f"binding lacks {n}"
+
+
+def test_sizes():
+    L = culgt.Lattice((32, 32, 32, 32), 3, 32, 12)
+    V = 32 ** 4
+    assert culgt.culgt_links_bytes(L) == 4 * V * 48 == 201326592
+    assert culgt.culgt_canonical_bytes(L) == 4 * V * 72
+    assert culgt.culgt_gfield_bytes(L) == V * 72
+    assert culgt.culgt_links_bytes(culgt.Lattice((32,) * 4, 3, 64, 18)) == 603979776
+    assert culgt.culgt_links_bytes(culgt.Lattice((48, 48, 48, 96), 3, 32, 12)) == 2038431744
+    assert culgt.culgt_links_bytes(culgt.Lattice((64,) * 4, 3, 64, 18)) == 9663676416
+    assert culgt.culgt_links_bytes(culgt.Lattice((8,) * 4, 2, 64, 4)) == 524288
+    assert culgt.culgt_workspace_bytes(L) >= 8 * 1024
+
+
+@pytest.mark.parametrize("lat,code", [
+    (culgt.Lattice((3, 4, 4, 4)), "CULGT_ERR_DIMS"),
+    (culgt.Lattice((4, 4, 0, 4)), "CULGT_ERR_DIMS"),
+    (culgt.Lattice((4, 4, 4, -2)), "CULGT_ERR_DIMS"),
+    (culgt.Lattice((1024, 1024, 1024, 4)), "CULGT_ERR_DIMS"),
+    (culgt.Lattice((4, 4, 4, 4), 4, 32, 12), "CULGT_ERR_DESC"),
+    (culgt.Lattice((4, 4, 4, 4), 3, 16, 12), "CULGT_ERR_DESC"),
+    (culgt.Lattice((4, 4, 4, 4), 3, 32, 8), "CULGT_ERR_DESC"),
+    (culgt.Lattice((4, 4, 4, 4), 2, 32, 12), "CULGT_ERR_DESC"),
+])
+def test_descriptor_errors(lat, code):
+    assert culgt.culgt_validate(lat) == culgt.ERRORS[code]
+    assert culgt.culgt_links_bytes(lat) == 0
+    assert culgt.culgt_canonical_bytes(lat) == 0
+
+
+def test_argument_errors_by_return_code():
+    lib = culgt.lib()
+    L = culgt.Lattice((4, 4, 4, 4), 3, 64, 18).c()
+    ref = ctypes.byref(L)
+    E = culgt.ERRORS
+    ok_ptr = 4096       # aligned, never dereferenced: validation fails first
+    assert lib.culgt_or_sweep(None, ok_ptr, 0, 1.7, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_or_sweep(ref, None, 0, 1.7, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_or_sweep(ref, ok_ptr + 8, 0, 1.7, None) == E["CULGT_ERR_ALIGN"]
+    assert lib.culgt_or_sweep(ref, ok_ptr, 2, 1.7, None) == E["CULGT_ERR_PARITY"]
+    assert lib.culgt_or_sweep(ref, ok_ptr, -1, 1.7, None) == E["CULGT_ERR_PARITY"]
+    for bad in (0.99, 2.0, float("nan"), float("inf"), -1.5):
+        assert lib.culgt_or_sweep(ref, ok_ptr, 0, bad, None) == E["CULGT_ERR_OMEGA"]
+        assert lib.culgt_or_sweeps(ref, ok_ptr, 1, bad, None) == E["CULGT_ERR_OMEGA"]
+    assert lib.culgt_or_sweeps(ref, ok_ptr, -1, 1.7, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_pack(ref, None, ok_ptr, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_unpack(ref, ok_ptr, None, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_gauge_precision(ref, ok_ptr, None, ok_ptr, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_functional(ref, ok_ptr, ok_ptr, None, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_gauge_transform(ref, ok_ptr, None, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_landau_fix(ref, ok_ptr, ok_ptr, 1.7, 1e-10, 10, 0, None, None, None, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_fix_host(ref, None, ok_ptr, ok_ptr, ok_ptr, 1, 1.7, None, None, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_set_sweep_variant(-3) == E["CULGT_ERR_ARG"]
+    for code in E.values():
+        assert culgt.culgt_strerror(code) != "unknown status"
+    assert culgt.culgt_strerror(-99) == "unknown status"
+
+
+def test_no_cpu_fallback():
+    """Without a CUDA device the binding refuses to compute (it never routes to the oracle)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA device present")
+    L = culgt.Lattice((4, 4, 4, 4), 3, 64, 18)
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        culgt.culgt_or_sweep(L, 4096, 0, 1.7)
+    src = open(os.path.join(ROOT, "paper_1412_3655_b200", "__init__.py")).read()
+    assert "import oracle" not in src and "from oracle" not in src
