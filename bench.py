@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py -- SU(3) Landau overrelaxation throughput on B200 (BASELINE.json metric, configs[3]).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A STEP is one full overrelaxation sweep (black half-sweep + white half-sweep = V site updates,
+PAPER.md L54) of the resident field; every --check-every steps the timed region also computes
+theta and F, as the paper's driver loop does.  Default workload: cfg3_fp32 = 32^4 SU(3), fp32
+12-parameter storage, omega = 1.7, near-identity (eps 0.8) gauge-scrambled seeded input -- the
+configuration the paper's Fig. 1 and BASELINE.json's metric are quoted on.
+
+value       site-updates/s over all ranks, inputs resident in HBM, CUDA events, max over ranks.
+e2e         the same through culgt_fix_host: pinned HOST canonical field -> H2D -> pack -> K
+            sweeps -> theta, F -> unpack -> D2H, all inside the timed region (one job of K steps;
+            the byte counts are per step = job bytes / K).
+roofline    dominant kernel = the half-sweep; algorithmic bytes per launch = 2 * field bytes
+            (every link read once and written once) / the average
+            launch duration measured live with CUDA events on the launching stream.
+cpu_baseline the oracle (oracle/, as it stands) timed on this host's cores on a bounded sample.
+--impl reference  times the oracle itself (rank 0 only), same metric / config / unit.
+
+Multi-GPU: the path has no exchange step ("replicas only"): each rank fixes its own
+independent configuration; value = total site-updates / max-over-ranks time; scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import lattice_inputs as li  # noqa: E402
+
+METRIC = "su3_landau_or_site_updates_per_s"
+UNIT = "site-updates/s"
+FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=500)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3_fp32", choices=sorted(li.CONFIGS))
+    ap.add_argument("--check-every", type=int, default=50)
+    ap.add_argument("--variant", type=int, default=0, help="sweep kernel variant (0 = default)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def committed_traffic(workload: str):
+    """dram bytes per half-sweep launch from the committed ncu --set full capture, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
+            return json.load(f).get(workload)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.004)
+
+    def start(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+
+    def stop(self):
+        if self._thread is not None:
+            self._stop.set()
+            self._thread.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def time_oracle(dims, group, ur, omega, max_sweeps, budget_s, threads):
+    """Full oracle sweeps until budget_s or max_sweeps; returns (site-updates/s, sweeps)."""
+    import oracle
+    oracle.set_threads(threads)
+    V = li.volume(dims)
+    t0 = time.perf_counter()
+    n = 0
+    while n < max_sweeps:
+        oracle.full_sweep(dims, ur, omega)
+        n += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    return V * n / dt, n
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on the host cores, rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    cfg = li.CONFIGS[args.workload]
+    total = args.steps + args.warmup
+    dims = cfg["dims"]
+    sample = "whole lattice, one full sweep per step"
+    if li.volume(dims) * total > 32 ** 4 * 600:
+        dims = (16, 16, 16, 16)
+        sample = "16^4 sub-volume with the same recipe (periodic), one full sweep per step"
+    threads = min(oracle.max_threads(), os.cpu_count() or 1)
+    oracle.set_threads(threads)
+    u = li.make_config(dims, cfg["group"], cfg["kind"], cfg["seed"], eps=cfg["eps"], scramble=cfg["scramble"])
+    if cfg["precision"] == 32:
+        u = li.round_to_fp32(u)
+    ur = li.to_real(u)
+    for _ in range(args.warmup):
+        oracle.full_sweep(dims, ur, cfg["omega"])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.full_sweep(dims, ur, cfg["omega"])
+    dt = time.perf_counter() - t0
+    V = li.volume(dims)
+    value = V * args.steps / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": workload_config(args, cfg),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gflops": value * flops_per_site(cfg) / 1e9,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def flops_per_site(cfg):
+    return 2304 if cfg["group"] == 3 else 278
+
+
+def workload_config(args, cfg):
+    return {
+        "workload": f"{args.workload}: {'x'.join(str(d) for d in cfg['dims'])} SU({cfg['group']}) "
+                    f"fp{cfg['precision']} {cfg['params']}-parameter, omega={cfg['omega']}, "
+                    f"{cfg['kind']} eps={cfg['eps']} scramble={cfg['scramble']} seed={cfg['seed']}",
+        "step": "one full sweep (black+white half-sweep) = V site updates; theta and F every "
+                f"{args.check_every} steps inside the timed region",
+        "l2": "no flush: the field is larger than the 126 MB L2 for the 32^4 and larger workloads "
+              "and every half-sweep streams all of it",
+        "parallelism": "replicas only (one independent configuration per GPU)",
+    }
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1412_3655_b200 as culgt
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    cfg = li.CONFIGS[args.workload]
+    dims, omega = cfg["dims"], cfg["omega"]
+    V = li.volume(dims)
+    lat = culgt.Lattice(tuple(dims), cfg["group"], cfg["precision"], cfg["params"])
+    culgt.culgt_set_sweep_variant(args.variant)
+
+    # seeded synthetic input, one independent configuration per rank
+    u = li.make_config(dims, cfg["group"], cfg["kind"], cfg["seed"] + 7919 * rank, eps=cfg["eps"],
+                       scramble=cfg["scramble"])
+    np_dt = np.float32 if cfg["precision"] == 32 else np.float64
+    host = torch.from_numpy(li.to_real(u, np_dt)).pin_memory()
+    del u
+    can_dev = torch.empty_like(host, device="cuda")
+    links = culgt.alloc_links(lat)
+    ws = culgt.alloc_workspace(lat)
+    scal = torch.zeros(2, dtype=torch.float64, device="cuda")
+    can_dev.copy_(host)
+    culgt.culgt_pack(lat, can_dev, links)
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def check():
+        culgt.culgt_gauge_precision(lat, links, ws, scal[0:1])
+        culgt.culgt_functional(lat, links, ws, scal[1:2])
+
+    # ---- warm-up
+    culgt.culgt_or_sweeps(lat, links, max(args.warmup, 3), omega)
+    check()
+    barrier()
+
+    # ---- timed region: K steps, theta/F every check_every steps
+    sampler = ClockSampler(local_rank)
+    n_checks = 0
+    check_events = []
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    ev0.record(stream)
+    done = 0
+    while done < args.steps:
+        n = min(args.check_every, args.steps - done)
+        culgt.culgt_or_sweeps(lat, links, n, omega)
+        done += n
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        check()
+        b.record(stream)
+        check_events.append((a, b))
+        n_checks += 1
+    ev1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    elapsed_ms = ev0.elapsed_time(ev1)
+    check_ms = sum(a.elapsed_time(b) for a, b in check_events)
+    theta, F = (float(x) for x in scal.cpu())
+
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    elapsed_max_ms = float(t.item())
+    value = world * V * args.steps / (elapsed_max_ms * 1e-3)
+
+    sweep_launches = 2 * args.steps
+    gpu_launches = sweep_launches + n_checks * 4        # theta: 2 kernels, F: 2 kernels
+    launch_ms = (elapsed_ms - check_ms) / sweep_launches
+    field_bytes = culgt.culgt_links_bytes(lat)
+    alg_bytes_per_launch = 2 * field_bytes
+    achieved_gbs = alg_bytes_per_launch / (launch_ms * 1e-3) / 1e9
+    peak, peak_src = measured_peak()
+
+    # ---- end to end through the host-buffer entry point
+    e2e = None
+    if not args.no_e2e:
+        culgt.culgt_fix_host(lat, host, can_dev, links, ws, 2, omega)       # warm the path
+        barrier()
+        t0 = time.perf_counter()
+        th_e, F_e = culgt.culgt_fix_host(lat, host, can_dev, links, ws, args.steps, omega)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        cbytes = culgt.culgt_canonical_bytes(lat)
+        e2e = {"value": world * V * args.steps / float(tt.item()), "unit": UNIT,
+               "h2d_bytes_per_step": cbytes / args.steps, "d2h_bytes_per_step": (cbytes + 16) / args.steps,
+               "job": f"one culgt_fix_host call = H2D {cbytes} B + pack + {args.steps} sweeps + theta,F + unpack + D2H {cbytes} B",
+               "theta": th_e, "F": F_e}
+
+    # ---- CPU baseline: the oracle on this host's cores (rank 0, N=1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        threads = min(oracle.max_threads(), os.cpu_count() or 1)
+        u0 = li.make_config(dims, cfg["group"], cfg["kind"], cfg["seed"], eps=cfg["eps"], scramble=cfg["scramble"])
+        if cfg["precision"] == 32:
+            u0 = li.round_to_fp32(u0)
+        ur = li.to_real(u0)
+        del u0
+        v_all, n_all = time_oracle(dims, cfg["group"], ur, omega, 40, 12.0, threads)
+        v_one, n_one = time_oracle(dims, cfg["group"], ur, omega, 3, 6.0, 1)
+        cpu = {"value": v_all, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"{n_all} full sweeps of the same {'x'.join(map(str, dims))} lattice on {threads} threads "
+                         f"(fp64, canonical layout); one core: {v_one:.4g} site-updates/s over {n_one} sweep(s)",
+               "one_core_value": v_one}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": elapsed_max_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if cfg["precision"] == 32 else "f64", "data": "synthetic",
+            "config": workload_config(args, cfg),
+            "gflops": value * flops_per_site(cfg) / 1e9,
+            "algorithmic_gbs": value * 16 * (cfg["params"] * cfg["precision"] // 8) / 1e9,
+            "gpu_launches": gpu_launches,
+            "e2e": e2e,
+            "roofline": {"bound": "hbm", "achieved": achieved_gbs, "peak": peak, "unit": "GB/s",
+                         "frac": achieved_gbs / peak, "traffic": committed_traffic(args.workload),
+                         "kernel": "or_sweep half-sweep", "bytes_per_launch": alg_bytes_per_launch,
+                         "launch_us": launch_ms * 1e3, "peak_source": peak_src,
+                         "frac_of_8TBs_nominal": achieved_gbs / 8000.0},
+            "cpu_baseline": cpu,
+            "clocks": clocks,
+            "final": {"theta": theta, "F": F},
+            "check_ms_total": check_ms, "variant": args.variant,
+            "context": {"paper": "470 GFlops at 80% of peak bandwidth on a GeForce GTX 580 (PAPER.md L7), context only"},
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
