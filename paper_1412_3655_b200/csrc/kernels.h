@@ -18,6 +18,8 @@ constexpr int kMaxReduceBlocks = 4096;  // block partials kept in the workspace
 
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
                             int variant, cudaStream_t st);
+cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
+                                   int variant, cudaStream_t st);
 cudaError_t launch_pack(const LatticeDesc& d, const void* canonical, void* links, cudaStream_t st);
 cudaError_t launch_unpack(const LatticeDesc& d, const void* links, void* canonical, cudaStream_t st);
 cudaError_t launch_gauge_precision(const LatticeDesc& d, const void* links, double* workspace,

@@ -76,9 +76,12 @@ __device__ __forceinline__ int down_index(const Geom& g, int h, const SiteCoord&
     if (c.odd) return h;
     return c.hx > 0 ? h - 1 : h + g.nh0 - 1;
   }
-  int x = (mu == 1) ? c.x1 : (mu == 2) ? c.x2 : c.x3;
-  int st = g.stride[mu];
-  return x > 0 ? h - st : h + st * (g.n[mu] - 1);
+  // selects instead of g.stride[mu] / g.n[mu]: a run-time index into the kernel-parameter struct
+  // would make the compiler copy it to local memory
+  const int x = (mu == 1) ? c.x1 : (mu == 2) ? c.x2 : c.x3;
+  const int st = (mu == 1) ? g.stride[1] : (mu == 2) ? g.stride[2] : g.stride[3];
+  const int n = (mu == 1) ? g.n[1] : (mu == 2) ? g.n[2] : g.n[3];
+  return x > 0 ? h - st : h + st * (n - 1);
 }
 
 // Half index (other parity) of x + mu_hat, periodic.

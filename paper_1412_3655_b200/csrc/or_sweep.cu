@@ -155,12 +155,15 @@ cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, doubl
     if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, g, parity, omega, st);
     return launch_su2<Storage<double, 2, 4> >(links, g, parity, omega, st);
   }
+  // variant 0 = the production mapping (or_sweep_staged.cu); 20+ select staged mappings
+  if (variant == 0) return launch_or_sweep_staged(d, links, parity, omega, 20, st);
+  if (variant >= 20) return launch_or_sweep_staged(d, links, parity, omega, variant, st);
   if (d.precision == 32) {
     // fp32 storage: K and the subgroup solve in fp64 (reading C-15); variants 10+ are
     // all-fp32 arithmetic, kept for the precision/throughput comparison in profiles/.
     if (d.params == 12) {
       switch (variant) {
-        case 0: case 1: return launch_su3<Storage<float, 3, 12>, double, 1>(links, g, parity, omega, st);
+        case 1: return launch_su3<Storage<float, 3, 12>, double, 1>(links, g, parity, omega, st);
         case 2: return launch_su3<Storage<float, 3, 12>, double, 2>(links, g, parity, omega, st);
         case 4: return launch_su3<Storage<float, 3, 12>, double, 4>(links, g, parity, omega, st);
         case 11: return launch_su3<Storage<float, 3, 12>, float, 1>(links, g, parity, omega, st);
@@ -169,21 +172,21 @@ cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, doubl
       }
     }
     switch (variant) {
-      case 0: case 2: return launch_su3<Storage<float, 3, 18>, double, 2>(links, g, parity, omega, st);
+      case 2: return launch_su3<Storage<float, 3, 18>, double, 2>(links, g, parity, omega, st);
       case 4: return launch_su3<Storage<float, 3, 18>, double, 4>(links, g, parity, omega, st);
       default: return cudaErrorInvalidValue;
     }
   }
   if (d.params == 12) {
     switch (variant) {
-      case 0: case 4: return launch_su3<Storage<double, 3, 12>, double, 4>(links, g, parity, omega, st);
+      case 4: return launch_su3<Storage<double, 3, 12>, double, 4>(links, g, parity, omega, st);
       case 2: return launch_su3<Storage<double, 3, 12>, double, 2>(links, g, parity, omega, st);
       case 8: return launch_su3<Storage<double, 3, 12>, double, 8>(links, g, parity, omega, st);
       default: return cudaErrorInvalidValue;
     }
   }
   switch (variant) {
-    case 0: case 4: return launch_su3<Storage<double, 3, 18>, double, 4>(links, g, parity, omega, st);
+    case 4: return launch_su3<Storage<double, 3, 18>, double, 4>(links, g, parity, omega, st);
     case 8: return launch_su3<Storage<double, 3, 18>, double, 8>(links, g, parity, omega, st);
     default: return cudaErrorInvalidValue;
   }

@@ -1,0 +1,282 @@
+// or_sweep_staged.cu -- the production SU(3) half-sweep kernel.
+//
+// Same mathematics as or_sweep.cu (eq. 3; L19-21), different machine mapping:
+//
+//  * The 8 links of a site are moved global -> shared memory by per-thread cp.async (LDGSTS)
+//    into slots that only the issuing thread reads back (slot layout [stage][vector][thread],
+//    16-byte vectors, so every LDS.128 / cp.async of a warp is 512 contiguous bytes and
+//    conflict-free).  No block barrier is needed: cp.async.wait_group orders a thread against its
+//    own copies.  The paper's obstacle (L72: 8 x 18 link registers do not fit a thread) is solved
+//    on B200 by parking the links in the 228 KB of shared memory per SM instead of splitting the
+//    site over 4 or 8 threads and paying the K(x) exchange.
+//  * Registers then hold only K (fp64), G and one link at a time, so 16 warps per SM are resident
+//    (1 stage) or 8 warps with the NEXT site's links already in flight (2 stages).
+//  * Persistent grid: gridDim = resident CTAs; CTA b processes site blocks b, b + gridDim, ...
+//    Odd-parity launches walk the site blocks in DESCENDING order so that the white half-sweep
+//    starts on the links the black half-sweep touched last, which are still in the 126 MB L2.
+//  * TPS threads cooperate on a site (TPS = 1 for fp32 storage; 2 for fp64 storage, whose 8 x 144
+//    bytes per site would otherwise limit an SM to 6 warps): partial K by xor-shuffle.
+//  * K accumulation and the subgroup chain in fp64 (su3_solve.cuh); link products in the storage
+//    precision.
+#include "lattice.cuh"
+#include "su_math.cuh"
+#include "su3_solve.cuh"
+#include "kernels.h"
+
+namespace culgt {
+
+__device__ __forceinline__ void cp_async_vec(float4* smem, const float4* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_vec(double2* smem, const double2* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_vec(float2* smem, const float2* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// What one thread needs to know about the site it works on: the half index of each of its LPT
+// links (slot = q*LPT + l = 2*mu + down; up links sit at the site's own index h in this parity's
+// sublattice, down links at the index of x - mu in the other parity's).
+template <int LPT>
+struct SiteRef {
+  int idx[LPT];
+  bool active;
+};
+
+template <int BLOCK, int TPS>
+__device__ __forceinline__ SiteRef<8 / TPS> locate(const Geom& g, int parity, int site_block, int q) {
+  constexpr int LPT = 8 / TPS;
+  SiteRef<LPT> r;
+  int h = site_block * (BLOCK / TPS) + (int)threadIdx.x / TPS;
+  r.active = h < g.vh;
+  if (!r.active) h = g.vh - 1;
+  const SiteCoord sc = decode_site(g, h, parity);
+#pragma unroll
+  for (int l = 0; l < LPT; ++l) {
+    const int slot = q * LPT + l;
+    r.idx[l] = (slot & 1) ? down_index(g, h, sc, slot >> 1) : h;
+  }
+  return r;
+}
+
+// Global address of vector 0 of this thread's link l.
+template <typename S, int LPT>
+__device__ __forceinline__ typename S::Vec* slot_ptr(typename S::Vec* links, const Geom& g, int parity,
+                                                     const SiteRef<LPT>& r, int q, int l) {
+  const int slot = q * LPT + l;
+  return link_base<S>(links, g, (slot & 1) ? 1 - parity : parity, slot >> 1, r.idx[l]);
+}
+
+template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB)
+or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
+                           const double omega, const int n_site_blocks, const int reverse) {
+  typedef typename S::Real Real;
+  typedef typename S::Vec Vec;
+  constexpr int LPT = 8 / TPS;          // links per thread
+  constexpr int NV = S::NV;             // vectors per link
+  constexpr int NVT = LPT * NV;         // vectors per thread per stage
+  constexpr int NR = (S::NP == 12) ? 2 : 3;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Vec* const sm = reinterpret_cast<Vec*>(smem_raw) + threadIdx.x;   // (stage, v) at sm[(stage*NVT+v)*BLOCK]
+  const int q = (int)threadIdx.x % TPS;
+
+  auto block_of = [&](int it) {
+    const int b = it * (int)gridDim.x + (int)blockIdx.x;
+    return reverse ? n_site_blocks - 1 - b : b;
+  };
+  auto issue = [&](const SiteRef<LPT>& r, int stage) {
+    if (r.active) {
+#pragma unroll
+      for (int l = 0; l < LPT; ++l) {
+        const Vec* src = slot_ptr<S, LPT>(links, g, parity, r, q, l);
+#pragma unroll
+        for (int j = 0; j < NV; ++j)
+          cp_async_vec(sm + (size_t)((stage * NVT + l * NV + j) * BLOCK), src + (size_t)j * (size_t)g.vh);
+      }
+    }
+    cp_async_commit();
+  };
+  auto load_link = [&](int stage, int l, Real* U) {
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const Vec v = sm[(size_t)((stage * NVT + l * NV + j) * BLOCK)];
+      vec_get(v, U + j * S::VL);
+    }
+  };
+
+  const int n_it = (n_site_blocks - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  if (n_it <= 0) return;
+
+  // prologue: STAGES-1 sites in flight
+  SiteRef<LPT> cur = locate<BLOCK, TPS>(g, parity, block_of(0), q);
+  SiteRef<LPT> nxt = cur;
+  if (STAGES == 1) {
+    // nothing in flight yet
+  } else {
+    issue(cur, 0);
+  }
+
+  for (int it = 0; it < n_it; ++it) {
+    const int stage = (STAGES == 1) ? 0 : (it & 1);
+    if (STAGES == 1) {
+      issue(cur, 0);
+      cp_async_wait<0>();
+    } else {
+      if (it + 1 < n_it) {
+        nxt = locate<BLOCK, TPS>(g, parity, block_of(it + 1), q);
+        issue(nxt, stage ^ 1);
+        cp_async_wait<1>();
+      } else {
+        cp_async_wait<0>();
+      }
+    }
+
+    // ---- K(x) = sum_mu U_mu(x) + U_mu(x-mu)^dagger                     (eq. 3)
+    Acc K[18];
+#pragma unroll
+    for (int i = 0; i < 18; ++i) K[i] = 0;
+#pragma unroll
+    for (int l = 0; l < LPT; ++l) {
+      Real U[18];
+      asm volatile("" ::: "memory");   // keep the shared-memory reads of link l behind link l-1's use
+      load_link(stage, l, U);
+      if (S::NP == 12) reconstruct_row2(U);
+      accumulate(K, U, ((q * LPT + l) & 1) != 0);
+    }
+#pragma unroll
+    for (int m = 1; m < TPS; m <<= 1) {
+#pragma unroll
+      for (int i = 0; i < 18; ++i) K[i] += __shfl_xor_sync(0xffffffffu, K[i], m);
+    }
+
+    // ---- G(x): subgroup loop with g^omega                              (L50-54)
+    Real G[18];
+    if (sizeof(Acc) == 8) {
+      double Kd[18];
+#pragma unroll
+      for (int i = 0; i < 18; ++i) Kd[i] = (double)K[i];
+      su3_solve<Real>(Kd, G, omega);
+    } else {
+      Acc Ga[18];
+      su3_site_G(K, Ga, (Acc)omega);
+#pragma unroll
+      for (int i = 0; i < 18; ++i) G[i] = (Real)Ga[i];
+    }
+
+    // ---- U_mu(x) <- G U_mu(x),  U_mu(x-mu) <- U_mu(x-mu) G^dagger      (L19-21, L48)
+    if (cur.active) {
+#pragma unroll
+      for (int l = 0; l < LPT; ++l) {
+        Real U[18], R[18];
+        asm volatile("" ::: "memory");
+        load_link(stage, l, U);
+        Vec* dst = slot_ptr<S, LPT>(links, g, parity, cur, q, l);
+        if (((q * LPT + l) & 1) == 0) {
+          if (S::NP == 12) reconstruct_row2(U);
+          mul_ab<NR>(G, U, R);
+        } else {
+          mul_abd<NR>(U, G, R);
+        }
+        store_params<S>(dst, g.vh, R);
+      }
+    }
+    if (STAGES == 1) {
+      if (it + 1 < n_it) cur = locate<BLOCK, TPS>(g, parity, block_of(it + 1), q);
+    } else {
+      cur = nxt;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+static int sm_count() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+  }
+  return n;
+}
+
+template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB>
+static cudaError_t launch_staged(void* links, const Geom& g, int parity, double omega, bool reverse_odd,
+                                 cudaStream_t st) {
+  typedef typename S::Vec Vec;
+  auto kern = or_sweep_su3_staged_kernel<S, Acc, TPS, BLOCK, STAGES, MINB>;
+  constexpr size_t smem = (size_t)STAGES * (8 / TPS) * S::NV * BLOCK * sizeof(Vec);
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  constexpr int SITES = BLOCK / TPS;
+  const int n_site_blocks = (g.vh + SITES - 1) / SITES;
+  int grid = sm_count() * MINB;
+  if (grid > n_site_blocks) grid = n_site_blocks;
+  kern<<<grid, BLOCK, smem, st>>>((Vec*)links, g, parity, omega, n_site_blocks,
+                                  (reverse_odd && parity) ? 1 : 0);
+  return cudaGetLastError();
+}
+
+// Variant table (measured in profiles/):
+//   fp32-12: 20 = TPS1 256x2CTA 1 stage (16 warps/SM) [default]; 21 = TPS1 256x1CTA 2 stages;
+//            22 = TPS1 128x2CTA 2 stages; 23 = TPS2 256x2CTA 1 stage; 24 = 20 without the reversed
+//            white traversal; 25 = all-fp32 K/g, 20's mapping
+//   fp32-18: 20 = TPS1 192x2 1 stage; 21 = TPS2 256x2 1 stage
+//   fp64-12: 20 = TPS2 256x2 1 stage; 21 = TPS1 128x2 1 stage; 22 = TPS4 256x2
+//   fp64-18: 20 = TPS2 192x2 1 stage; 21 = TPS4 256x2 1 stage; 22 = TPS2 96x2 2 stages
+cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
+                                   int variant, cudaStream_t st) {
+  const Geom& g = d.geom;
+  if (d.group != 3) return cudaErrorInvalidValue;
+  if (d.precision == 32 && d.params == 12) {
+    typedef Storage<float, 3, 12> S;
+    switch (variant) {
+      case 20: return launch_staged<S, double, 1, 256, 1, 2>(links, g, parity, omega, true, st);
+      case 21: return launch_staged<S, double, 1, 256, 2, 1>(links, g, parity, omega, true, st);
+      case 22: return launch_staged<S, double, 1, 128, 2, 2>(links, g, parity, omega, true, st);
+      case 23: return launch_staged<S, double, 2, 256, 1, 2>(links, g, parity, omega, true, st);
+      case 24: return launch_staged<S, double, 1, 256, 1, 2>(links, g, parity, omega, false, st);
+      case 25: return launch_staged<S, float, 1, 256, 1, 2>(links, g, parity, omega, true, st);
+      default: return cudaErrorInvalidValue;
+    }
+  }
+  if (d.precision == 32) {
+    typedef Storage<float, 3, 18> S;
+    switch (variant) {
+      case 20: return launch_staged<S, double, 1, 192, 1, 2>(links, g, parity, omega, true, st);
+      case 21: return launch_staged<S, double, 2, 256, 1, 2>(links, g, parity, omega, true, st);
+      default: return cudaErrorInvalidValue;
+    }
+  }
+  if (d.params == 12) {
+    typedef Storage<double, 3, 12> S;
+    switch (variant) {
+      case 20: return launch_staged<S, double, 2, 256, 1, 2>(links, g, parity, omega, true, st);
+      case 21: return launch_staged<S, double, 1, 128, 1, 2>(links, g, parity, omega, true, st);
+      case 22: return launch_staged<S, double, 4, 256, 1, 2>(links, g, parity, omega, true, st);
+      default: return cudaErrorInvalidValue;
+    }
+  }
+  typedef Storage<double, 3, 18> S;
+  switch (variant) {
+    case 20: return launch_staged<S, double, 2, 192, 1, 2>(links, g, parity, omega, true, st);
+    case 21: return launch_staged<S, double, 4, 256, 1, 2>(links, g, parity, omega, true, st);
+    case 22: return launch_staged<S, double, 2, 96, 2, 2>(links, g, parity, omega, true, st);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace culgt

@@ -46,13 +46,15 @@ def test_pack_unpack_round_trip_su2(dims, precision):
 
 
 def variants_for(precision, params):
+    """0 = production mapping; 1..8 = direct register kernels with that many threads per site;
+    20+ = shared-memory staged mappings (or_sweep_staged.cu)."""
     if precision == 32 and params == 12:
-        return [0, 2, 4]
+        return [0, 1, 2, 4, 21, 22, 23, 24]
     if precision == 32:
-        return [0, 4]
+        return [0, 2, 4, 21]
     if params == 12:
-        return [0, 2, 8]
-    return [0, 8]
+        return [0, 2, 4, 8, 21, 22]
+    return [0, 4, 8, 21, 22]
 
 
 @pytest.mark.parametrize("dims", DIMS)
