@@ -18,6 +18,7 @@
 //    bytes per site would otherwise limit an SM to 6 warps): partial K by xor-shuffle.
 //  * K accumulation and the subgroup chain in fp64 (su3_solve.cuh); link products in the storage
 //    precision.
+#include <type_traits>
 #include "lattice.cuh"
 #include "su_math.cuh"
 #include "su3_solve.cuh"
@@ -38,6 +39,24 @@ __device__ __forceinline__ void cp_async_vec(float2* smem, const float2* gmem) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// Shared-memory reads as asm.  VOL = true emits ld.volatile: ptxas otherwise recognises the apply
+// pass's reads as repeats of the K pass's reads and keeps all 8 links live in registers across the
+// subgroup solve (spilling them), which is exactly what the staging exists to avoid.
+template <bool VOL>
+__device__ __forceinline__ void lds_vec(unsigned addr, float4& v) {
+  if (VOL) asm volatile("ld.volatile.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  else asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+}
+template <bool VOL>
+__device__ __forceinline__ void lds_vec(unsigned addr, double2& v) {
+  if (VOL) asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+  else asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+}
+template <bool VOL>
+__device__ __forceinline__ void lds_vec(unsigned addr, float2& v) {
+  if (VOL) asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+  else asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+}
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
@@ -66,12 +85,16 @@ __device__ __forceinline__ SiteRef<8 / TPS> locate(const Geom& g, int parity, in
   return r;
 }
 
-// Global address of vector 0 of this thread's link l.
+// Global address of vector j of this thread's link l: a plane base that does not depend on the
+// thread (for TPS = 1 it is uniform over the grid, so it lives in uniform registers) plus the
+// 32-bit half index -- this keeps 64-bit per-thread address arithmetic out of the inner loops.
 template <typename S, int LPT>
-__device__ __forceinline__ typename S::Vec* slot_ptr(typename S::Vec* links, const Geom& g, int parity,
-                                                     const SiteRef<LPT>& r, int q, int l) {
+__device__ __forceinline__ typename S::Vec* vec_ptr(typename S::Vec* links, const Geom& g, int parity,
+                                                    const SiteRef<LPT>& r, int q, int l, int j) {
   const int slot = q * LPT + l;
-  return link_base<S>(links, g, (slot & 1) ? 1 - parity : parity, slot >> 1, r.idx[l]);
+  const int plane = (((slot & 1) ? 1 - parity : parity) * 4 + (slot >> 1)) * S::NV + j;
+  typename S::Vec* base = links + (size_t)plane * (size_t)g.vh;
+  return base + (unsigned)r.idx[l];
 }
 
 template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB>
@@ -86,6 +109,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
   constexpr int NR = (S::NP == 12) ? 2 : 3;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Vec* const sm = reinterpret_cast<Vec*>(smem_raw) + threadIdx.x;   // (stage, v) at sm[(stage*NVT+v)*BLOCK]
+  const unsigned sm_addr = (unsigned)__cvta_generic_to_shared(sm);
   const int q = (int)threadIdx.x % TPS;
 
   auto block_of = [&](int it) {
@@ -96,18 +120,19 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
     if (r.active) {
 #pragma unroll
       for (int l = 0; l < LPT; ++l) {
-        const Vec* src = slot_ptr<S, LPT>(links, g, parity, r, q, l);
 #pragma unroll
         for (int j = 0; j < NV; ++j)
-          cp_async_vec(sm + (size_t)((stage * NVT + l * NV + j) * BLOCK), src + (size_t)j * (size_t)g.vh);
+          cp_async_vec(sm + (size_t)((stage * NVT + l * NV + j) * BLOCK),
+                       vec_ptr<S, LPT>(links, g, parity, r, q, l, j));
       }
     }
     cp_async_commit();
   };
-  auto load_link = [&](int stage, int l, Real* U) {
+  auto load_link = [&](int stage, int l, Real* U, auto vol) {
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
-      const Vec v = sm[(size_t)((stage * NVT + l * NV + j) * BLOCK)];
+      Vec v;
+      lds_vec<decltype(vol)::value>(sm_addr + (unsigned)((stage * NVT + l * NV + j) * BLOCK * (int)sizeof(Vec)), v);
       vec_get(v, U + j * S::VL);
     }
   };
@@ -147,7 +172,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
     for (int l = 0; l < LPT; ++l) {
       Real U[18];
       asm volatile("" ::: "memory");   // keep the shared-memory reads of link l behind link l-1's use
-      load_link(stage, l, U);
+      load_link(stage, l, U, std::false_type());
       if (S::NP == 12) reconstruct_row2(U);
       accumulate(K, U, ((q * LPT + l) & 1) != 0);
     }
@@ -177,15 +202,19 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
       for (int l = 0; l < LPT; ++l) {
         Real U[18], R[18];
         asm volatile("" ::: "memory");
-        load_link(stage, l, U);
-        Vec* dst = slot_ptr<S, LPT>(links, g, parity, cur, q, l);
+        load_link(stage, l, U, std::true_type());
         if (((q * LPT + l) & 1) == 0) {
           if (S::NP == 12) reconstruct_row2(U);
           mul_ab<NR>(G, U, R);
         } else {
           mul_abd<NR>(U, G, R);
         }
-        store_params<S>(dst, g.vh, R);
+#pragma unroll
+        for (int j = 0; j < NV; ++j) {
+          Vec v;
+          vec_set(v, R + j * S::VL);
+          *vec_ptr<S, LPT>(links, g, parity, cur, q, l, j) = v;
+        }
       }
     }
     if (STAGES == 1) {
@@ -235,8 +264,9 @@ static cudaError_t launch_staged(void* links, const Geom& g, int parity, double 
 //            22 = TPS1 128x2CTA 2 stages; 23 = TPS2 256x2CTA 1 stage; 24 = 20 without the reversed
 //            white traversal; 25 = all-fp32 K/g, 20's mapping
 //   fp32-18: 20 = TPS1 192x2 1 stage; 21 = TPS2 256x2 1 stage
-//   fp64-12: 20 = TPS2 256x2 1 stage; 21 = TPS1 128x2 1 stage; 22 = TPS4 256x2
-//   fp64-18: 20 = TPS2 192x2 1 stage; 21 = TPS4 256x2 1 stage; 22 = TPS2 96x2 2 stages
+//   fp64-12: 20 = TPS2 256x2 1 stage; 21 = TPS1 128x2 1 stage; 22 = TPS4 256x2; 23 = TPS1 256x1
+//   fp64-18: 20 = TPS2 192x2 1 stage; 21 = TPS4 256x2 1 stage; 22 = TPS2 96x2 2 stages;
+//            23 = TPS1 192x1 1 stage; 24 = TPS1 96x2 1 stage
 cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
                                    int variant, cudaStream_t st) {
   const Geom& g = d.geom;
@@ -267,6 +297,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
       case 20: return launch_staged<S, double, 2, 256, 1, 2>(links, g, parity, omega, true, st);
       case 21: return launch_staged<S, double, 1, 128, 1, 2>(links, g, parity, omega, true, st);
       case 22: return launch_staged<S, double, 4, 256, 1, 2>(links, g, parity, omega, true, st);
+      case 23: return launch_staged<S, double, 1, 256, 1, 1>(links, g, parity, omega, true, st);
       default: return cudaErrorInvalidValue;
     }
   }
@@ -275,6 +306,8 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
     case 20: return launch_staged<S, double, 2, 192, 1, 2>(links, g, parity, omega, true, st);
     case 21: return launch_staged<S, double, 4, 256, 1, 2>(links, g, parity, omega, true, st);
     case 22: return launch_staged<S, double, 2, 96, 2, 2>(links, g, parity, omega, true, st);
+    case 23: return launch_staged<S, double, 1, 192, 1, 1>(links, g, parity, omega, true, st);
+    case 24: return launch_staged<S, double, 1, 96, 1, 2>(links, g, parity, omega, true, st);
     default: return cudaErrorInvalidValue;
   }
 }

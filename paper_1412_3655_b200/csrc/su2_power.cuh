@@ -8,7 +8,7 @@
 //      g^omega = (cos(omega a), -pv/|pv| sin(omega a)).
 //
 // How a is obtained to fp64 accuracy without an fp64 atan2:
-//   a~ = atan2f(|pv|, p0) in fp32 (error <= ~1e-6), widened exactly to fp64;
+//   a~ = a cheap fp32 polynomial atan2 (error < 3e-6), widened exactly to fp64;
 //   (s~, c~) = sincos(a~) by the fp64 polynomials below;
 //   d = sin(a - a~) = (|pv| c~ - p0 s~)/|p|  exactly;  a = a~ + d + d^3/6   (|d|^5 < 1e-30).
 // The two sincos evaluations (of a~ and of omega*a~) are independent, which gives the FP64 pipe
@@ -20,39 +20,72 @@
 
 namespace culgt {
 
+// Taylor coefficients of sin (odd, from -1/3! up to -1/19!) and cos (even, from -1/2! up to 1/20!).
+// In constant memory so that every DFMA takes its coefficient as a constant-bank operand instead
+// of two MOVs of a 64-bit immediate.
+__constant__ double kSinCoef[9] = {
+    -1.66666666666666666667e-01, 8.33333333333333333333e-03, -1.98412698412698412698e-04,
+    2.75573192239858906526e-06,  -2.50521083854417187751e-08, 1.60590438368216145994e-10,
+    -7.64716373181981647590e-13, 2.81145725434552076320e-15,  -8.22063524662432971696e-18};
+__constant__ double kCosCoef[10] = {
+    -0.5,                        4.16666666666666666667e-02,  -1.38888888888888888889e-03,
+    2.48015873015873015873e-05,  -2.75573192239858906526e-07, 2.08767569878680989792e-09,
+    -1.14707455977297247139e-11, 4.77947733238738529744e-14,  -1.56192069685862264622e-16,
+    4.11031762331216485848e-19};
+
 // sin and cos of x for 0 <= x <= ~7 (omega*a < 2*pi): Cody-Waite reduction by pi/2 (k <= 4, so two
 // constants suffice) and Taylor polynomials on [-pi/4, pi/4] truncated below 1e-17.
 __device__ __forceinline__ void sincos_bounded(double x, double* s, double* c) {
-  const double k = rint(x * 0.63661977236758134308);            // 2/pi
+  // k = rint(x * 2/pi) by the 1.5*2^52 trick: no FRND / F2I on the slow conversion pipe
+  const double magic = 6755399441055744.0;
+  const double kb = fma(x, 0.63661977236758134308, magic);
+  const int q = __double2loint(kb);
+  const double k = kb - magic;
   double y = fma(-k, 1.57079632679489655800e+00, x);            // pi/2 high part
   y = fma(-k, 6.12323399573676603587e-17, y);                   // pi/2 low part
   const double z = y * y;
-  double ps = -8.22063524662432971696e-18;                      // -1/19!
-  ps = fma(ps, z, 2.81145725434552076320e-15);                  // 1/17!
-  ps = fma(ps, z, -7.64716373181981647590e-13);                 // -1/15!
-  ps = fma(ps, z, 1.60590438368216145994e-10);                  // 1/13!
-  ps = fma(ps, z, -2.50521083854417187751e-08);                 // -1/11!
-  ps = fma(ps, z, 2.75573192239858906526e-06);                  // 1/9!
-  ps = fma(ps, z, -1.98412698412698412698e-04);                 // -1/7!
-  ps = fma(ps, z, 8.33333333333333333333e-03);                  // 1/5!
-  ps = fma(ps, z, -1.66666666666666666667e-01);                 // -1/3!
+  double ps = kSinCoef[8];
+#pragma unroll
+  for (int i = 7; i >= 0; --i) ps = fma(ps, z, kSinCoef[i]);
   const double sy = fma(ps * z, y, y);
-  double pc = 4.11031762331216485848e-19;                       // 1/20!
-  pc = fma(pc, z, -1.56192069685862264622e-16);                 // -1/18!
-  pc = fma(pc, z, 4.77947733238738529744e-14);                  // 1/16!
-  pc = fma(pc, z, -1.14707455977297247139e-11);                 // -1/14!
-  pc = fma(pc, z, 2.08767569878680989792e-09);                  // 1/12!
-  pc = fma(pc, z, -2.75573192239858906526e-07);                 // -1/10!
-  pc = fma(pc, z, 2.48015873015873015873e-05);                  // 1/8!
-  pc = fma(pc, z, -1.38888888888888888889e-03);                 // -1/6!
-  pc = fma(pc, z, 4.16666666666666666667e-02);                  // 1/4!
-  pc = fma(pc, z, -0.5);
+  double pc = kCosCoef[9];
+#pragma unroll
+  for (int i = 8; i >= 0; --i) pc = fma(pc, z, kCosCoef[i]);
   const double cy = fma(pc, z, 1.0);
-  const int q = (int)k & 3;
-  const double a = (q & 1) ? cy : sy;                           // |sin x|-carrier
+  const double a = (q & 1) ? cy : sy;
   const double b = (q & 1) ? sy : cy;
   *s = (q & 2) ? -a : a;
   *c = ((q + 1) & 2) ? -b : b;
+}
+
+// 1/sqrt(x) for normal positive x: the 64-bit MUFU seed (~2^-22) and two Newton steps.
+__device__ __forceinline__ double rsqrt_newton(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x * y, y, 1.0);
+  y = fma(0.5 * y, e, y);
+  e = fma(-x * y, y, 1.0);
+  y = fma(0.5 * y, e, y);
+  return y;
+}
+
+// atan2(y, x) for y >= 0 and x^2 + y^2 = 1, in fp32, absolute error < 3e-6 (degree-11 odd
+// polynomial on [0,1] plus octant fix-up).  It only seeds the fp64 correction below.
+__device__ __forceinline__ float atan2_seed(float y, float x) {
+  const float ax = fabsf(x);
+  const float mx = fmaxf(ax, y), mn = fminf(ax, y);      // mx >= 0.707
+  const float t = __fdividef(mn, mx);
+  const float u = t * t;
+  float p = -0.011686083860695362f;
+  p = fmaf(p, u, 0.05254087969660759f);
+  p = fmaf(p, u, -0.11629831045866013f);
+  p = fmaf(p, u, 0.1934700906276703f);
+  p = fmaf(p, u, -0.3326060175895691f);
+  p = fmaf(p, u, 0.9999759197235107f);
+  float a = p * t;
+  if (y > ax) a = 1.57079632679489662f - a;
+  if (x < 0.0f) a = 3.14159265358979324f - a;
+  return a;
 }
 
 // q_out = (conj(p)/|p|)^omega for the un-normalised quaternion p = (p[0]; p[1], p[2], p[3]).
@@ -60,23 +93,26 @@ __device__ __forceinline__ void sincos_bounded(double x, double* s, double* c) {
 __device__ __forceinline__ bool su2_update_power(const double* p, double omega, double* q) {
   const double r2 = p[1] * p[1] + p[2] * p[2] + p[3] * p[3];
   const double n2 = fma(p[0], p[0], r2);
-  if (n2 == 0.0) return false;
-  if (r2 < 1e-300) {                 // g = +1 or -1: axis undefined (C-8: z axis by fiat for g = -1)
+  if (n2 < 1e-280) {                 // |p| = 0 skips the update; denormal-range |p| is treated alike
+    return false;
+  }
+  if (r2 < 1e-280) {                 // g = +1 or -1: axis undefined (C-8: z axis by fiat for g = -1)
     double s = 0.0, c = 1.0;
     if (p[0] < 0.0) sincos_bounded(omega * 3.14159265358979323846, &s, &c);
     q[0] = c; q[1] = 0.0; q[2] = 0.0; q[3] = s;
     return true;
   }
-  const double rinv = rsqrt(r2);     // 1/|pv|
-  const double ninv = rsqrt(n2);     // 1/|p|
-  const double R = r2 * rinv;        // |pv|
-  const double a0 = (double)atan2f((float)R, (float)p[0]);
+  const double rinv = rsqrt_newton(r2);   // 1/|pv|
+  const double ninv = rsqrt_newton(n2);   // 1/|p|
+  const double R = r2 * rinv;             // |pv|
+  const double sn = R * ninv, cs = p[0] * ninv;      // sin a, cos a
+  const double a0 = (double)atan2_seed((float)sn, (float)cs);
   double s0, c0, s1, c1;
   sincos_bounded(a0, &s0, &c0);
   sincos_bounded(omega * a0, &s1, &c1);
-  double d = (R * c0 - p[0] * s0) * ninv;          // sin(a - a0)
+  double d = sn * c0 - cs * s0;                    // sin(a - a0), |d| < 1e-5
   d = fma(d * d * d, 1.0 / 6.0, d);                // a - a0
-  const double e = omega * d;                      // omega a - omega a0, |e| < 1e-5
+  const double e = omega * d;                      // omega a - omega a0
   const double ce = fma(-0.5 * e, e, 1.0);
   const double se = fma(e * e * e, -1.0 / 6.0, e);
   const double C = c1 * ce - s1 * se;

@@ -12,6 +12,26 @@ namespace culgt {
 #define CULGT_RE(r, c) (2 * (3 * (r) + (c)))
 #define CULGT_IM(r, c) (2 * (3 * (r) + (c)) + 1)
 
+__device__ __forceinline__ float fma_t(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_t(double a, double b, double c) { return fma(a, b, c); }
+
+// acc += x * y (complex), written as four fused multiply-adds so that no separate add is issued.
+template <typename T>
+__device__ __forceinline__ void cmac(T& accr, T& acci, T xr, T xi, T yr, T yi) {
+  accr = fma_t(xr, yr, accr);
+  accr = fma_t(-xi, yi, accr);
+  acci = fma_t(xr, yi, acci);
+  acci = fma_t(xi, yr, acci);
+}
+// acc += x * conj(y)
+template <typename T>
+__device__ __forceinline__ void cmac_conj(T& accr, T& acci, T xr, T xi, T yr, T yi) {
+  accr = fma_t(xr, yr, accr);
+  accr = fma_t(xi, yi, accr);
+  acci = fma_t(xi, yr, acci);
+  acci = fma_t(-xr, yi, acci);
+}
+
 // Third row of an SU(3) matrix from its first two: row2 = conj(row0 x row1)
 // ("reconstruct the full matrix in registers", L118).
 template <typename T>
@@ -19,11 +39,15 @@ __device__ __forceinline__ void reconstruct_row2(T* m) {
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
     const int a = (c + 1) % 3, b = (c + 2) % 3;
-    // (row0[a]*row1[b] - row0[b]*row1[a]) conjugated
-    T re = m[CULGT_RE(0, a)] * m[CULGT_RE(1, b)] - m[CULGT_IM(0, a)] * m[CULGT_IM(1, b)]
-         - m[CULGT_RE(0, b)] * m[CULGT_RE(1, a)] + m[CULGT_IM(0, b)] * m[CULGT_IM(1, a)];
-    T im = m[CULGT_RE(0, a)] * m[CULGT_IM(1, b)] + m[CULGT_IM(0, a)] * m[CULGT_RE(1, b)]
-         - m[CULGT_RE(0, b)] * m[CULGT_IM(1, a)] - m[CULGT_IM(0, b)] * m[CULGT_RE(1, a)];
+    // row0[a]*row1[b] - row0[b]*row1[a], then conjugated
+    T re = m[CULGT_RE(0, a)] * m[CULGT_RE(1, b)];
+    T im = m[CULGT_RE(0, a)] * m[CULGT_IM(1, b)];
+    re = fma_t(-m[CULGT_IM(0, a)], m[CULGT_IM(1, b)], re);
+    im = fma_t(m[CULGT_IM(0, a)], m[CULGT_RE(1, b)], im);
+    re = fma_t(-m[CULGT_RE(0, b)], m[CULGT_RE(1, a)], re);
+    im = fma_t(-m[CULGT_RE(0, b)], m[CULGT_IM(1, a)], im);
+    re = fma_t(m[CULGT_IM(0, b)], m[CULGT_IM(1, a)], re);
+    im = fma_t(-m[CULGT_IM(0, b)], m[CULGT_RE(1, a)], im);
     m[CULGT_RE(2, c)] = re;
     m[CULGT_IM(2, c)] = -im;
   }
@@ -36,12 +60,13 @@ __device__ __forceinline__ void mul_ab(const T* A, const T* B, T* C) {
   for (int r = 0; r < NR; ++r)
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      T re = 0, im = 0;
+      T re = A[CULGT_RE(r, 0)] * B[CULGT_RE(0, c)];
+      T im = A[CULGT_RE(r, 0)] * B[CULGT_IM(0, c)];
+      re = fma_t(-A[CULGT_IM(r, 0)], B[CULGT_IM(0, c)], re);
+      im = fma_t(A[CULGT_IM(r, 0)], B[CULGT_RE(0, c)], im);
 #pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        re += A[CULGT_RE(r, k)] * B[CULGT_RE(k, c)] - A[CULGT_IM(r, k)] * B[CULGT_IM(k, c)];
-        im += A[CULGT_RE(r, k)] * B[CULGT_IM(k, c)] + A[CULGT_IM(r, k)] * B[CULGT_RE(k, c)];
-      }
+      for (int k = 1; k < 3; ++k)
+        cmac(re, im, A[CULGT_RE(r, k)], A[CULGT_IM(r, k)], B[CULGT_RE(k, c)], B[CULGT_IM(k, c)]);
       C[CULGT_RE(r, c)] = re;
       C[CULGT_IM(r, c)] = im;
     }
@@ -54,13 +79,14 @@ __device__ __forceinline__ void mul_abd(const T* A, const T* B, T* C) {
   for (int r = 0; r < NR; ++r)
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      T re = 0, im = 0;
+      // sum_k A[r][k] * conj(B[c][k])
+      T re = A[CULGT_RE(r, 0)] * B[CULGT_RE(c, 0)];
+      T im = A[CULGT_IM(r, 0)] * B[CULGT_RE(c, 0)];
+      re = fma_t(A[CULGT_IM(r, 0)], B[CULGT_IM(c, 0)], re);
+      im = fma_t(-A[CULGT_RE(r, 0)], B[CULGT_IM(c, 0)], im);
 #pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        // A[r][k] * conj(B[c][k])
-        re += A[CULGT_RE(r, k)] * B[CULGT_RE(c, k)] + A[CULGT_IM(r, k)] * B[CULGT_IM(c, k)];
-        im += A[CULGT_IM(r, k)] * B[CULGT_RE(c, k)] - A[CULGT_RE(r, k)] * B[CULGT_IM(c, k)];
-      }
+      for (int k = 1; k < 3; ++k)
+        cmac_conj(re, im, A[CULGT_RE(r, k)], A[CULGT_IM(r, k)], B[CULGT_RE(c, k)], B[CULGT_IM(c, k)]);
       C[CULGT_RE(r, c)] = re;
       C[CULGT_IM(r, c)] = im;
     }

@@ -53,8 +53,8 @@ def variants_for(precision, params):
     if precision == 32:
         return [0, 2, 4, 21]
     if params == 12:
-        return [0, 2, 4, 8, 21, 22]
-    return [0, 4, 8, 21, 22]
+        return [0, 2, 4, 8, 21, 22, 23]
+    return [0, 4, 8, 21, 22, 23, 24]
 
 
 @pytest.mark.parametrize("dims", DIMS)
