@@ -247,6 +247,11 @@ CONFIGS = {
                       kind="near_identity", eps=0.8, scramble=True, omega=1.7, seed=1003),
     "cfg3_fp64": dict(dims=(32, 32, 32, 32), group=3, precision=64, params=18,
                       kind="near_identity", eps=0.8, scramble=True, omega=1.7, seed=1003),
+    # same lattice and input as cfg3 in the two remaining storage formats (SURVEY.md 8(f) NEXT-2d)
+    "cfg3_fp32_18": dict(dims=(32, 32, 32, 32), group=3, precision=32, params=18,
+                         kind="near_identity", eps=0.8, scramble=True, omega=1.7, seed=1003),
+    "cfg3_fp64_12": dict(dims=(32, 32, 32, 32), group=3, precision=64, params=12,
+                         kind="near_identity", eps=0.8, scramble=True, omega=1.7, seed=1003),
     "cfg4_fp32": dict(dims=(48, 48, 48, 96), group=3, precision=32, params=12, kind="haar",
                       eps=0.0, scramble=False, omega=1.7, seed=1004),
     "cfg4_fp64": dict(dims=(64, 64, 64, 64), group=3, precision=64, params=18, kind="haar",

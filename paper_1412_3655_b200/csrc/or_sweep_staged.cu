@@ -57,6 +57,9 @@ __device__ __forceinline__ void lds_vec(unsigned addr, float2& v) {
   if (VOL) asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
   else asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
 }
+__device__ __forceinline__ void prefetch_l2(const void* gmem) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(gmem));
+}
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
@@ -97,7 +100,7 @@ __device__ __forceinline__ typename S::Vec* vec_ptr(typename S::Vec* links, cons
   return base + (unsigned)r.idx[l];
 }
 
-template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB>
+template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int PF>
 __global__ void __launch_bounds__(BLOCK, MINB)
 or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
                            const double omega, const int n_site_blocks, const int reverse) {
@@ -153,6 +156,17 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
     const int stage = (STAGES == 1) ? 0 : (it & 1);
     if (STAGES == 1) {
       issue(cur, 0);
+      if (PF && it + 1 < n_it) {
+        // pull the NEXT site block's lines into L2 while this one is computed: the blocking
+        // cp.async of the next iteration then pays L2 latency, not HBM latency
+        nxt = locate<BLOCK, TPS>(g, parity, block_of(it + 1), q);
+        if (nxt.active) {
+#pragma unroll
+          for (int l = 0; l < LPT; ++l)
+#pragma unroll
+            for (int j = 0; j < NV; ++j) prefetch_l2(vec_ptr<S, LPT>(links, g, parity, nxt, q, l, j));
+        }
+      }
       cp_async_wait<0>();
     } else {
       if (it + 1 < n_it) {
@@ -217,7 +231,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
         }
       }
     }
-    if (STAGES == 1) {
+    if (STAGES == 1 && !PF) {
       if (it + 1 < n_it) cur = locate<BLOCK, TPS>(g, parity, block_of(it + 1), q);
     } else {
       cur = nxt;
@@ -238,11 +252,11 @@ static int sm_count() {
   return n;
 }
 
-template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB>
+template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int PF = 0>
 static cudaError_t launch_staged(void* links, const Geom& g, int parity, double omega, bool reverse_odd,
                                  cudaStream_t st) {
   typedef typename S::Vec Vec;
-  auto kern = or_sweep_su3_staged_kernel<S, Acc, TPS, BLOCK, STAGES, MINB>;
+  auto kern = or_sweep_su3_staged_kernel<S, Acc, TPS, BLOCK, STAGES, MINB, PF>;
   constexpr size_t smem = (size_t)STAGES * (8 / TPS) * S::NV * BLOCK * sizeof(Vec);
   static bool configured = false;
   if (!configured) {
@@ -280,6 +294,8 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
       case 23: return launch_staged<S, double, 2, 256, 1, 2>(links, g, parity, omega, true, st);
       case 24: return launch_staged<S, double, 1, 256, 1, 2>(links, g, parity, omega, false, st);
       case 25: return launch_staged<S, float, 1, 256, 1, 2>(links, g, parity, omega, true, st);
+      case 26: return launch_staged<S, double, 1, 256, 1, 2, 1>(links, g, parity, omega, true, st);
+      case 27: return launch_staged<S, float, 1, 256, 1, 2, 1>(links, g, parity, omega, true, st);
       default: return cudaErrorInvalidValue;
     }
   }
@@ -308,6 +324,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
     case 22: return launch_staged<S, double, 2, 96, 2, 2>(links, g, parity, omega, true, st);
     case 23: return launch_staged<S, double, 1, 192, 1, 1>(links, g, parity, omega, true, st);
     case 24: return launch_staged<S, double, 1, 96, 1, 2>(links, g, parity, omega, true, st);
+    case 25: return launch_staged<S, double, 1, 192, 1, 1, 1>(links, g, parity, omega, true, st);
     default: return cudaErrorInvalidValue;
   }
 }
