@@ -67,13 +67,18 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def committed_traffic(workload: str):
-    """dram bytes per half-sweep launch from the committed ncu --set full capture, or None."""
+def committed_traffic(workload: str, capture: str = "ncu_set_full_cold_cache"):
+    """dram bytes (read + write) per half-sweep launch from the committed ncu captures
+    (profiles/roofline_traffic.csv), or None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
-            return json.load(f).get(workload)
+        with open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) as f:
+            for line in f:
+                p = line.strip().split(",")
+                if len(p) >= 4 and p[0] == workload and p[1] == capture:
+                    return int(p[2]) + int(p[3])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
@@ -335,6 +340,7 @@ def main():
             "e2e": e2e,
             "roofline": {"bound": "hbm", "achieved": achieved_gbs, "peak": peak, "unit": "GB/s",
                          "frac": achieved_gbs / peak, "traffic": committed_traffic(args.workload),
+                         "traffic_steady_state": committed_traffic(args.workload, "steady_state"),
                          "kernel": "or_sweep half-sweep", "bytes_per_launch": alg_bytes_per_launch,
                          "launch_us": launch_ms * 1e3, "peak_source": peak_src,
                          "frac_of_8TBs_nominal": achieved_gbs / 8000.0},

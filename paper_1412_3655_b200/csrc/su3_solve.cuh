@@ -8,8 +8,8 @@
 //   after (0,1): row 0 (all columns) and row 1 columns 1,2     (40 DFMA instead of 48)
 //   after (0,2): row 2 columns 1,2                             (16 instead of 48)
 //   after (1,2): nothing                                       ( 0 instead of 48)
-// The accumulated G = g_3 g_2 g_1 carries no such amplification and is formed in the storage
-// precision GT (float for fp32 storage, double for fp64 storage).
+// The accumulated G = g_3 g_2 g_1 is formed in the type GT the caller asks for (the sweep kernels
+// use double and round once to the storage precision).
 #pragma once
 #include "su_math.cuh"
 #include "su2_power.cuh"
