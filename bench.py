@@ -181,6 +181,28 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def max_over_ranks(value: float, world: int, device="cpu") -> float:
+    """MAX over the ranks of a per-rank scalar (the only cross-rank data dependency of the
+    bench: the path itself has no exchange step).  Works on any backend."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, volume: int, steps: int, elapsed_max_s: float) -> float:
+    """Replicas only: every rank sweeps its own lattice; units of all ranks / slowest rank's time."""
+    return world * volume * steps / elapsed_max_s
+
+
+def rank_seed(base_seed: int, rank: int) -> int:
+    """One independent seeded configuration per rank."""
+    return base_seed + 7919 * rank
+
+
 def flops_per_site(cfg):
     return 2304 if cfg["group"] == 3 else 278
 
@@ -224,7 +246,7 @@ def main():
     culgt.culgt_set_sweep_variant(args.variant)
 
     # seeded synthetic input, one independent configuration per rank
-    u = li.make_config(dims, cfg["group"], cfg["kind"], cfg["seed"] + 7919 * rank, eps=cfg["eps"],
+    u = li.make_config(dims, cfg["group"], cfg["kind"], rank_seed(cfg["seed"], rank), eps=cfg["eps"],
                        scramble=cfg["scramble"])
     np_dt = np.float32 if cfg["precision"] == 32 else np.float64
     host = torch.from_numpy(li.to_real(u, np_dt)).pin_memory()
@@ -278,11 +300,8 @@ def main():
     check_ms = sum(a.elapsed_time(b) for a, b in check_events)
     theta, F = (float(x) for x in scal.cpu())
 
-    t = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    elapsed_max_ms = float(t.item())
-    value = world * V * args.steps / (elapsed_max_ms * 1e-3)
+    elapsed_max_ms = max_over_ranks(elapsed_ms, world, "cuda")
+    value = whole_job_value(world, V, args.steps, elapsed_max_ms * 1e-3)
 
     sweep_launches = 2 * args.steps
     gpu_launches = sweep_launches + n_checks * 4        # theta: 2 kernels, F: 2 kernels
@@ -301,11 +320,9 @@ def main():
         th_e, F_e = culgt.culgt_fix_host(lat, host, can_dev, links, ws, args.steps, omega)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        dt_max = max_over_ranks(dt, world, "cuda")
         cbytes = culgt.culgt_canonical_bytes(lat)
-        e2e = {"value": world * V * args.steps / float(tt.item()), "unit": UNIT,
+        e2e = {"value": whole_job_value(world, V, args.steps, dt_max), "unit": UNIT,
                "h2d_bytes_per_step": cbytes / args.steps, "d2h_bytes_per_step": (cbytes + 16) / args.steps,
                "job": f"one culgt_fix_host call = H2D {cbytes} B + pack + {args.steps} sweeps + theta,F + unpack + D2H {cbytes} B",
                "theta": th_e, "F": F_e}
