@@ -115,8 +115,10 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
   const unsigned sm_addr = (unsigned)__cvta_generic_to_shared(sm);
   const int q = (int)threadIdx.x % TPS;
 
+  // site blocks of this CTA: strided (b, b + grid, ...) or, with OPT bit 2, one contiguous chunk
+  const int per_cta = (n_site_blocks + (int)gridDim.x - 1) / (int)gridDim.x;
   auto block_of = [&](int it) {
-    const int b = it * (int)gridDim.x + (int)blockIdx.x;
+    const int b = (PF & 4) ? (int)blockIdx.x * per_cta + it : it * (int)gridDim.x + (int)blockIdx.x;
     return reverse ? n_site_blocks - 1 - b : b;
   };
   auto issue = [&](const SiteRef<LPT>& r, int stage) {
@@ -140,7 +142,8 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
     }
   };
 
-  const int n_it = (n_site_blocks - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  const int n_it = (PF & 4) ? min(per_cta, n_site_blocks - (int)blockIdx.x * per_cta)
+                            : (n_site_blocks - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   if (n_it <= 0) return;
 
   // prologue: STAGES-1 sites in flight
@@ -205,7 +208,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
       // G = g_3 g_2 g_1 is accumulated in fp64 and rounded once: accumulating it in fp32 costs
       // 0.7 % less time but doubles the worst link error at 32^4 (1.08e-5 vs 5.8e-6)
       double Gd[18];
-      su3_solve<double>(Kd, Gd, omega);
+      su3_solve<(sizeof(Real) == 8), double>(Kd, Gd, omega);
 #pragma unroll
       for (int i = 0; i < 18; ++i) G[i] = (Real)Gd[i];
     } else {
@@ -301,6 +304,8 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
       case 25: return launch_staged<S, float, 1, 256, 1, 2>(links, g, parity, omega, true, st);
       case 26: return launch_staged<S, double, 1, 256, 1, 2, 1>(links, g, parity, omega, true, st);
       case 27: return launch_staged<S, float, 1, 256, 1, 2, 1>(links, g, parity, omega, true, st);
+      case 28: return launch_staged<S, double, 1, 256, 1, 2, 4>(links, g, parity, omega, true, st);
+      case 29: return launch_staged<S, double, 1, 512, 1, 1>(links, g, parity, omega, true, st);
       default: return cudaErrorInvalidValue;
     }
   }
@@ -330,6 +335,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
     case 23: return launch_staged<S, double, 1, 192, 1, 1>(links, g, parity, omega, true, st);
     case 24: return launch_staged<S, double, 1, 96, 1, 2>(links, g, parity, omega, true, st);
     case 25: return launch_staged<S, double, 1, 192, 1, 1, 1>(links, g, parity, omega, true, st);
+    case 26: return launch_staged<S, double, 1, 192, 1, 1, 4>(links, g, parity, omega, true, st);
     default: return cudaErrorInvalidValue;
   }
 }

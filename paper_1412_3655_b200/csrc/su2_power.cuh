@@ -35,7 +35,11 @@ __constant__ double kCosCoef[10] = {
 
 // sin and cos of x for 0 <= x <= ~7 (omega*a < 2*pi): Cody-Waite reduction by pi/2 (k <= 4, so two
 // constants suffice) and Taylor polynomials on [-pi/4, pi/4] truncated below 1e-17.
+// FULL = false stops the series at y^11/11! and y^12/12! (truncation < 7e-12): enough for fp32
+// link storage, where the chain's errors are compared at 2e-5 after an amplification of <~ 1e3.
+template <bool FULL>
 __device__ __forceinline__ void sincos_bounded(double x, double* s, double* c) {
+  constexpr int NS = FULL ? 9 : 5, NC = FULL ? 10 : 6;
   // k = rint(x * 2/pi) by the 1.5*2^52 trick: no FRND / F2I on the slow conversion pipe
   const double magic = 6755399441055744.0;
   const double kb = fma(x, 0.63661977236758134308, magic);
@@ -44,13 +48,13 @@ __device__ __forceinline__ void sincos_bounded(double x, double* s, double* c) {
   double y = fma(-k, 1.57079632679489655800e+00, x);            // pi/2 high part
   y = fma(-k, 6.12323399573676603587e-17, y);                   // pi/2 low part
   const double z = y * y;
-  double ps = kSinCoef[8];
+  double ps = kSinCoef[NS - 1];
 #pragma unroll
-  for (int i = 7; i >= 0; --i) ps = fma(ps, z, kSinCoef[i]);
+  for (int i = NS - 2; i >= 0; --i) ps = fma(ps, z, kSinCoef[i]);
   const double sy = fma(ps * z, y, y);
-  double pc = kCosCoef[9];
+  double pc = kCosCoef[NC - 1];
 #pragma unroll
-  for (int i = 8; i >= 0; --i) pc = fma(pc, z, kCosCoef[i]);
+  for (int i = NC - 2; i >= 0; --i) pc = fma(pc, z, kCosCoef[i]);
   const double cy = fma(pc, z, 1.0);
   const double a = (q & 1) ? cy : sy;
   const double b = (q & 1) ? sy : cy;
@@ -58,14 +62,18 @@ __device__ __forceinline__ void sincos_bounded(double x, double* s, double* c) {
   *c = ((q + 1) & 2) ? -b : b;
 }
 
-// 1/sqrt(x) for normal positive x: the 64-bit MUFU seed (~2^-22) and two Newton steps.
+// 1/sqrt(x) for normal positive x: the 64-bit MUFU seed (~2^-22) and two Newton steps (one when
+// FULL = false: ~1e-13).
+template <bool FULL>
 __device__ __forceinline__ double rsqrt_newton(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   double e = fma(-x * y, y, 1.0);
   y = fma(0.5 * y, e, y);
-  e = fma(-x * y, y, 1.0);
-  y = fma(0.5 * y, e, y);
+  if (FULL) {
+    e = fma(-x * y, y, 1.0);
+    y = fma(0.5 * y, e, y);
+  }
   return y;
 }
 
@@ -90,6 +98,7 @@ __device__ __forceinline__ float atan2_seed(float y, float x) {
 
 // q_out = (conj(p)/|p|)^omega for the un-normalised quaternion p = (p[0]; p[1], p[2], p[3]).
 // Returns false (q_out untouched) when p == 0, where the update is skipped (reading C-9).
+template <bool FULL>
 __device__ __forceinline__ bool su2_update_power(const double* p, double omega, double* q) {
   const double r2 = p[1] * p[1] + p[2] * p[2] + p[3] * p[3];
   const double n2 = fma(p[0], p[0], r2);
@@ -98,18 +107,18 @@ __device__ __forceinline__ bool su2_update_power(const double* p, double omega, 
   }
   if (r2 < 1e-280) {                 // g = +1 or -1: axis undefined (C-8: z axis by fiat for g = -1)
     double s = 0.0, c = 1.0;
-    if (p[0] < 0.0) sincos_bounded(omega * 3.14159265358979323846, &s, &c);
+    if (p[0] < 0.0) sincos_bounded<FULL>(omega * 3.14159265358979323846, &s, &c);
     q[0] = c; q[1] = 0.0; q[2] = 0.0; q[3] = s;
     return true;
   }
-  const double rinv = rsqrt_newton(r2);   // 1/|pv|
-  const double ninv = rsqrt_newton(n2);   // 1/|p|
+  const double rinv = rsqrt_newton<FULL>(r2);   // 1/|pv|
+  const double ninv = rsqrt_newton<FULL>(n2);   // 1/|p|
   const double R = r2 * rinv;             // |pv|
   const double sn = R * ninv, cs = p[0] * ninv;      // sin a, cos a
   const double a0 = (double)atan2_seed((float)sn, (float)cs);
   double s0, c0, s1, c1;
-  sincos_bounded(a0, &s0, &c0);
-  sincos_bounded(omega * a0, &s1, &c1);
+  sincos_bounded<FULL>(a0, &s0, &c0);
+  sincos_bounded<FULL>(omega * a0, &s1, &c1);
   double d = sn * c0 - cs * s0;                    // sin(a - a0), |d| < 1e-5
   d = fma(d * d * d, 1.0 / 6.0, d);                // a - a0
   const double e = omega * d;                      // omega a - omega a0

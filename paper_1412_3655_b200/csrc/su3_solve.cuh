@@ -17,14 +17,14 @@
 namespace culgt {
 
 // p = real-quaternion part (x2) of the (I,J) block of K; q = (conj(p)/|p|)^omega.
-template <int I, int J>
+template <int I, int J, bool FULL>
 __device__ __forceinline__ bool subgroup_quaternion(const double* K, double omega, double* q) {
   double p[4];
   p[0] = K[CULGT_RE(I, I)] + K[CULGT_RE(J, J)];
   p[1] = K[CULGT_IM(I, J)] + K[CULGT_IM(J, I)];
   p[2] = K[CULGT_RE(I, J)] - K[CULGT_RE(J, I)];
   p[3] = K[CULGT_IM(I, I)] - K[CULGT_IM(J, J)];
-  return su2_update_power(p, omega, q);
+  return su2_update_power<FULL>(p, omega, q);
 }
 
 // (x, y) <- (a x + b y, -conj(b) x + conj(a) y) for complex x = M[I][c], y = M[J][c];
@@ -50,11 +50,12 @@ __device__ __forceinline__ void rotate_col(T* M, int c, T ar, T ai, T br, T bi) 
 
 // K (fp64, destroyed) -> G (type GT).  g_s embeds q = (c, v1, v2, v3) as
 // [I][I] = a = c + i v3, [I][J] = b = v2 + i v1, [J][I] = -conj(b), [J][J] = conj(a)  (C-7).
-template <typename GT>
+// FULL selects full-length (fp64 storage) or shortened (fp32 storage) series in su2_power.cuh.
+template <bool FULL, typename GT>
 __device__ __forceinline__ void su3_solve(double* K, GT* G, double omega) {
   double q[4];
   // ---- subgroup (0,1)
-  bool ok = subgroup_quaternion<0, 1>(K, omega, q);
+  bool ok = subgroup_quaternion<0, 1, FULL>(K, omega, q);
   if (!ok) { q[0] = 1.0; q[1] = 0.0; q[2] = 0.0; q[3] = 0.0; }
   {
     const double ar = q[0], ai = q[3], br = q[2], bi = q[1];
@@ -65,7 +66,7 @@ __device__ __forceinline__ void su3_solve(double* K, GT* G, double omega) {
   // G = g_1
   const GT a1r = (GT)q[0], a1i = (GT)q[3], b1r = (GT)q[2], b1i = (GT)q[1];
   // ---- subgroup (0,2)
-  ok = subgroup_quaternion<0, 2>(K, omega, q);
+  ok = subgroup_quaternion<0, 2, FULL>(K, omega, q);
   if (!ok) { q[0] = 1.0; q[1] = 0.0; q[2] = 0.0; q[3] = 0.0; }
   {
     const double ar = q[0], ai = q[3], br = q[2], bi = q[1];
@@ -88,7 +89,7 @@ __device__ __forceinline__ void su3_solve(double* K, GT* G, double omega) {
     G[CULGT_RE(2, 2)] = a2r;                    G[CULGT_IM(2, 2)] = -a2i;
   }
   // ---- subgroup (1,2)
-  ok = subgroup_quaternion<1, 2>(K, omega, q);
+  ok = subgroup_quaternion<1, 2, FULL>(K, omega, q);
   if (ok) {
     const GT ar = (GT)q[0], ai = (GT)q[3], br = (GT)q[2], bi = (GT)q[1];
 #pragma unroll
