@@ -157,11 +157,7 @@ cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, doubl
   }
   // variant 0 = the production mapping (or_sweep_staged.cu); 20+ select staged mappings
   if (variant == 0) {
-    // measured best mapping per storage format (profiles/)
-    int best = 20;                                            // fp32-12: 1 thread/site, 16 warps/SM
-    if (d.precision == 64 && d.params == 18) best = 23;       // fp64-18: 1 thread/site, 192 x 1 CTA
-    else if (d.precision == 64) best = 21;                    // fp64-12: 1 thread/site, 128 x 2 CTAs
-    else if (d.params == 18) best = 21;                       // fp32-18: 2 threads/site, 256 x 2 CTAs
+    const int best = 20;   // the production mapping of each storage format (or_sweep_staged.cu)
     return launch_or_sweep_staged(d, links, parity, omega, best, st);
   }
   if (variant >= 20) return launch_or_sweep_staged(d, links, parity, omega, variant, st);

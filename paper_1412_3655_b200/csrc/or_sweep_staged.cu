@@ -9,15 +9,19 @@
 //    own copies.  The paper's obstacle (L72: 8 x 18 link registers do not fit a thread) is solved
 //    on B200 by parking the links in the 228 KB of shared memory per SM instead of splitting the
 //    site over 4 or 8 threads and paying the K(x) exchange.
-//  * Registers then hold only K (fp64), G and one link at a time, so 16 warps per SM are resident
-//    (1 stage) or 8 warps with the NEXT site's links already in flight (2 stages).
-//  * Persistent grid: gridDim = resident CTAs; CTA b processes site blocks b, b + gridDim, ...
-//    Odd-parity launches walk the site blocks in DESCENDING order so that the white half-sweep
-//    starts on the links the black half-sweep touched last, which are still in the 126 MB L2.
-//  * TPS threads cooperate on a site (TPS = 1 for fp32 storage; 2 for fp64 storage, whose 8 x 144
-//    bytes per site would otherwise limit an SM to 6 warps): partial K by xor-shuffle.
-//  * K accumulation and the subgroup chain in fp64 (su3_solve.cuh); link products in the storage
-//    precision.
+//  * Registers then hold only K (fp64), G and one link at a time: 126 registers for fp32
+//    storage, no spills in any format.
+//  * Grid: ONE small CTA per site block (128 threads x 4 CTAs/SM for fp32-12, 64 x 3 for fp64-18),
+//    handed out in order by the hardware block scheduler.  A persistent grid-stride loop (kept as
+//    a variant) keeps every CTA of an SM in the same load-then-compute phase and measures 8-23 %
+//    slower; small CTAs that retire and are replaced one at a time keep loads, arithmetic and
+//    stores of different CTAs overlapped.  Odd-parity launches map blockIdx to site blocks in
+//    DESCENDING order so that the white half-sweep starts on the links the black half-sweep
+//    touched last, which are still in the 126 MB L2.
+//  * One thread per site for every storage format (TPS = 1); TPS = 2, 4 (partial K by
+//    xor-shuffle, the subgroup solve repeated per thread) are kept as measured alternatives.
+//  * K accumulation, the subgroup chain and G in fp64 (su3_solve.cuh); reconstruction and link
+//    products in the storage precision.
 #include <type_traits>
 #include "lattice.cuh"
 #include "su_math.cuh"
@@ -25,6 +29,13 @@
 #include "kernels.h"
 
 namespace culgt {
+
+// Option bits of the OPT template parameter.
+constexpr int OPT_PREFETCH = 1;    // persistent only: prefetch.global.L2 of the next site block
+constexpr int OPT_CHUNKED = 4;     // persistent only: contiguous chunk of site blocks per CTA
+constexpr int OPT_NOMATH = 8;      // measurement only: G = 1 (memory pattern + products, no K / solve)
+constexpr int OPT_FLAT = 16;       // one CTA per site block (hardware block scheduler), not persistent
+constexpr int OPT_STREAM_ST = 32;  // st.global.cs stores
 
 __device__ __forceinline__ void cp_async_vec(float4* smem, const float4* gmem) {
   const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -56,6 +67,15 @@ template <bool VOL>
 __device__ __forceinline__ void lds_vec(unsigned addr, float2& v) {
   if (VOL) asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
   else asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+}
+__device__ __forceinline__ void st_cs(float4* p, const float4& v) {
+  asm volatile("st.global.cs.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void st_cs(double2* p, const double2& v) {
+  asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void st_cs(float2* p, const float2& v) {
+  asm volatile("st.global.cs.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.x), "f"(v.y) : "memory");
 }
 __device__ __forceinline__ void prefetch_l2(const void* gmem) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(gmem));
@@ -100,7 +120,7 @@ __device__ __forceinline__ typename S::Vec* vec_ptr(typename S::Vec* links, cons
   return base + (unsigned)r.idx[l];
 }
 
-template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int PF>
+template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int OPT>
 __global__ void __launch_bounds__(BLOCK, MINB)
 or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
                            const double omega, const int n_site_blocks, const int reverse) {
@@ -118,7 +138,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
   // site blocks of this CTA: strided (b, b + grid, ...) or, with OPT bit 2, one contiguous chunk
   const int per_cta = (n_site_blocks + (int)gridDim.x - 1) / (int)gridDim.x;
   auto block_of = [&](int it) {
-    const int b = (PF & 4) ? (int)blockIdx.x * per_cta + it : it * (int)gridDim.x + (int)blockIdx.x;
+    const int b = (OPT & OPT_CHUNKED) ? (int)blockIdx.x * per_cta + it : it * (int)gridDim.x + (int)blockIdx.x;
     return reverse ? n_site_blocks - 1 - b : b;
   };
   auto issue = [&](const SiteRef<LPT>& r, int stage) {
@@ -142,7 +162,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
     }
   };
 
-  const int n_it = (PF & 4) ? min(per_cta, n_site_blocks - (int)blockIdx.x * per_cta)
+  const int n_it = (OPT & OPT_CHUNKED) ? min(per_cta, n_site_blocks - (int)blockIdx.x * per_cta)
                             : (n_site_blocks - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   if (n_it <= 0) return;
 
@@ -159,7 +179,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
     const int stage = (STAGES == 1) ? 0 : (it & 1);
     if (STAGES == 1) {
       issue(cur, 0);
-      if ((PF & 1) && it + 1 < n_it) {
+      if ((OPT & OPT_PREFETCH) && it + 1 < n_it) {
         // pull the NEXT site block's lines into L2 while this one is computed: the blocking
         // cp.async of the next iteration then pays L2 latency, not HBM latency
         nxt = locate<BLOCK, TPS>(g, parity, block_of(it + 1), q);
@@ -181,6 +201,11 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
       }
     }
 
+    Real G[18];
+    if (OPT & OPT_NOMATH) {   // measurement only: memory pattern + apply, no K / solve (G = 1)
+#pragma unroll
+      for (int i = 0; i < 18; ++i) G[i] = (i == 0 || i == 8 || i == 16) ? (Real)1 : (Real)0;
+    } else {
     // ---- K(x) = sum_mu U_mu(x) + U_mu(x-mu)^dagger                     (eq. 3)
     Acc K[18];
 #pragma unroll
@@ -200,7 +225,6 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
     }
 
     // ---- G(x): subgroup loop with g^omega                              (L50-54)
-    Real G[18];
     if (sizeof(Acc) == 8) {
       double Kd[18];
 #pragma unroll
@@ -218,6 +242,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
       for (int i = 0; i < 18; ++i) G[i] = (Real)Ga[i];
     }
 
+    }
     // ---- U_mu(x) <- G U_mu(x),  U_mu(x-mu) <- U_mu(x-mu) G^dagger      (L19-21, L48)
     if (cur.active) {
 #pragma unroll
@@ -235,11 +260,12 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
         for (int j = 0; j < NV; ++j) {
           Vec v;
           vec_set(v, R + j * S::VL);
-          *vec_ptr<S, LPT>(links, g, parity, cur, q, l, j) = v;
+          if (OPT & OPT_STREAM_ST) st_cs(vec_ptr<S, LPT>(links, g, parity, cur, q, l, j), v);
+          else *vec_ptr<S, LPT>(links, g, parity, cur, q, l, j) = v;
         }
       }
     }
-    if (STAGES == 1 && !(PF & 1)) {
+    if (STAGES == 1 && !(OPT & OPT_PREFETCH)) {
       if (it + 1 < n_it) cur = locate<BLOCK, TPS>(g, parity, block_of(it + 1), q);
     } else {
       cur = nxt;
@@ -260,11 +286,11 @@ static int sm_count() {
   return n;
 }
 
-template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int PF = 0>
+template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int OPT>
 static cudaError_t launch_staged(void* links, const Geom& g, int parity, double omega, bool reverse_odd,
                                  cudaStream_t st) {
   typedef typename S::Vec Vec;
-  auto kern = or_sweep_su3_staged_kernel<S, Acc, TPS, BLOCK, STAGES, MINB, PF>;
+  auto kern = or_sweep_su3_staged_kernel<S, Acc, TPS, BLOCK, STAGES, MINB, OPT>;
   constexpr size_t smem = (size_t)STAGES * (8 / TPS) * S::NV * BLOCK * sizeof(Vec);
   static bool configured = false;
   if (!configured) {
@@ -274,21 +300,19 @@ static cudaError_t launch_staged(void* links, const Geom& g, int parity, double 
   }
   constexpr int SITES = BLOCK / TPS;
   const int n_site_blocks = (g.vh + SITES - 1) / SITES;
-  int grid = sm_count() * MINB;
+  // OPT bit 16: one CTA per site block (the hardware block scheduler hands out blocks in order)
+  // instead of a persistent grid-stride loop
+  int grid = (OPT & OPT_FLAT) ? n_site_blocks : sm_count() * MINB;
   if (grid > n_site_blocks) grid = n_site_blocks;
   kern<<<grid, BLOCK, smem, st>>>((Vec*)links, g, parity, omega, n_site_blocks,
                                   (reverse_odd && parity) ? 1 : 0);
   return cudaGetLastError();
 }
 
-// Variant table (measured in profiles/):
-//   fp32-12: 20 = TPS1 256x2CTA 1 stage (16 warps/SM) [default]; 21 = TPS1 256x1CTA 2 stages;
-//            22 = TPS1 128x2CTA 2 stages; 23 = TPS2 256x2CTA 1 stage; 24 = 20 without the reversed
-//            white traversal; 25 = all-fp32 K/g, 20's mapping
-//   fp32-18: 20 = TPS1 192x2 1 stage; 21 = TPS2 256x2 1 stage
-//   fp64-12: 20 = TPS2 256x2 1 stage; 21 = TPS1 128x2 1 stage; 22 = TPS4 256x2; 23 = TPS1 256x1
-//   fp64-18: 20 = TPS2 192x2 1 stage; 21 = TPS4 256x2 1 stage; 22 = TPS2 96x2 2 stages;
-//            23 = TPS1 192x1 1 stage; 24 = TPS1 96x2 1 stage
+// Variant table (measured in profiles/r1_variant_sweep.md).  20 is the production
+// mapping of each storage format; the others are the measured alternatives and stay callable
+// (culgt_set_sweep_variant) and parity-tested.  "AxB" = A threads per CTA, B CTAs per SM;
+// "flat" = one CTA per site block, "pers" = persistent grid-stride loop; tps = threads per site.
 cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
                                    int variant, cudaStream_t st) {
   const Geom& g = d.geom;
@@ -296,46 +320,55 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
   if (d.precision == 32 && d.params == 12) {
     typedef Storage<float, 3, 12> S;
     switch (variant) {
-      case 20: return launch_staged<S, double, 1, 256, 1, 2>(links, g, parity, omega, true, st);
-      case 21: return launch_staged<S, double, 1, 256, 2, 1>(links, g, parity, omega, true, st);
-      case 22: return launch_staged<S, double, 1, 128, 2, 2>(links, g, parity, omega, true, st);
-      case 23: return launch_staged<S, double, 2, 256, 1, 2>(links, g, parity, omega, true, st);
-      case 24: return launch_staged<S, double, 1, 256, 1, 2>(links, g, parity, omega, false, st);
-      case 25: return launch_staged<S, float, 1, 256, 1, 2>(links, g, parity, omega, true, st);
-      case 26: return launch_staged<S, double, 1, 256, 1, 2, 1>(links, g, parity, omega, true, st);
-      case 27: return launch_staged<S, float, 1, 256, 1, 2, 1>(links, g, parity, omega, true, st);
-      case 28: return launch_staged<S, double, 1, 256, 1, 2, 4>(links, g, parity, omega, true, st);
-      case 29: return launch_staged<S, double, 1, 512, 1, 1>(links, g, parity, omega, true, st);
+      case 20: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 21: return launch_staged<S, double, 1, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
+      case 22: return launch_staged<S, double, 1, 128, 2, 2, 0>(links, g, parity, omega, true, st);          // pers, 2 stages
+      case 23: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
+      case 24: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT>(links, g, parity, omega, false, st);  // no reversal
+      case 25: return launch_staged<S, float, 1, 128, 1, 4, OPT_FLAT>(links, g, parity, omega, true, st);    // all-fp32
+      case 26: return launch_staged<S, double, 1, 256, 1, 2, OPT_PREFETCH>(links, g, parity, omega, true, st);
+      case 27: return launch_staged<S, double, 1, 256, 1, 2, OPT_CHUNKED>(links, g, parity, omega, true, st);
+      case 28: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT | OPT_NOMATH>(links, g, parity, omega, true, st);
+      case 29: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT | OPT_STREAM_ST>(links, g, parity, omega, true, st);
+      case 30: return launch_staged<S, double, 1, 256, 1, 2, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 31: return launch_staged<S, double, 1, 32, 1, 16, OPT_FLAT>(links, g, parity, omega, true, st);
       default: return cudaErrorInvalidValue;
     }
   }
   if (d.precision == 32) {
     typedef Storage<float, 3, 18> S;
     switch (variant) {
-      case 20: return launch_staged<S, double, 1, 192, 1, 2>(links, g, parity, omega, true, st);
-      case 21: return launch_staged<S, double, 2, 256, 1, 2>(links, g, parity, omega, true, st);
+      case 20: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
+      case 21: return launch_staged<S, double, 1, 192, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
+      case 22: return launch_staged<S, double, 1, 128, 1, 3, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 23: return launch_staged<S, double, 2, 256, 1, 2, OPT_FLAT>(links, g, parity, omega, true, st);
       default: return cudaErrorInvalidValue;
     }
   }
   if (d.params == 12) {
     typedef Storage<double, 3, 12> S;
     switch (variant) {
-      case 20: return launch_staged<S, double, 2, 256, 1, 2>(links, g, parity, omega, true, st);
-      case 21: return launch_staged<S, double, 1, 128, 1, 2>(links, g, parity, omega, true, st);
-      case 22: return launch_staged<S, double, 4, 256, 1, 2>(links, g, parity, omega, true, st);
-      case 23: return launch_staged<S, double, 1, 256, 1, 1>(links, g, parity, omega, true, st);
+      case 20: return launch_staged<S, double, 1, 64, 1, 4, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 21: return launch_staged<S, double, 1, 128, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
+      case 22: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
+      case 23: return launch_staged<S, double, 4, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 4 tps, pers
+      case 24: return launch_staged<S, double, 1, 128, 1, 2, OPT_FLAT>(links, g, parity, omega, true, st);
       default: return cudaErrorInvalidValue;
     }
   }
   typedef Storage<double, 3, 18> S;
   switch (variant) {
-    case 20: return launch_staged<S, double, 2, 192, 1, 2>(links, g, parity, omega, true, st);
-    case 21: return launch_staged<S, double, 4, 256, 1, 2>(links, g, parity, omega, true, st);
-    case 22: return launch_staged<S, double, 2, 96, 2, 2>(links, g, parity, omega, true, st);
-    case 23: return launch_staged<S, double, 1, 192, 1, 1>(links, g, parity, omega, true, st);
-    case 24: return launch_staged<S, double, 1, 96, 1, 2>(links, g, parity, omega, true, st);
-    case 25: return launch_staged<S, double, 1, 192, 1, 1, 1>(links, g, parity, omega, true, st);
-    case 26: return launch_staged<S, double, 1, 192, 1, 1, 4>(links, g, parity, omega, true, st);
+    case 20: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT>(links, g, parity, omega, true, st);
+    case 21: return launch_staged<S, double, 1, 192, 1, 1, 0>(links, g, parity, omega, true, st);            // pers
+    case 22: return launch_staged<S, double, 2, 192, 1, 2, 0>(links, g, parity, omega, true, st);            // 2 tps, pers
+    case 23: return launch_staged<S, double, 4, 256, 1, 2, 0>(links, g, parity, omega, true, st);            // 4 tps, pers
+    case 24: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT>(links, g, parity, omega, false, st);     // no reversal
+    case 26: return launch_staged<S, double, 1, 192, 1, 1, OPT_PREFETCH>(links, g, parity, omega, true, st);
+    case 27: return launch_staged<S, double, 1, 192, 1, 1, OPT_CHUNKED>(links, g, parity, omega, true, st);
+    case 28: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT | OPT_NOMATH>(links, g, parity, omega, true, st);
+    case 30: return launch_staged<S, double, 1, 192, 1, 1, OPT_FLAT>(links, g, parity, omega, true, st);
+    case 31: return launch_staged<S, double, 1, 32, 1, 6, OPT_FLAT>(links, g, parity, omega, true, st);
+    case 32: return launch_staged<S, double, 1, 96, 2, 1, 0>(links, g, parity, omega, true, st);             // pers, 2 stages
     default: return cudaErrorInvalidValue;
   }
 }
