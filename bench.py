@@ -267,8 +267,7 @@ def main():
         torch.cuda.synchronize()
 
     def check():
-        culgt.culgt_gauge_precision(lat, links, ws, scal[0:1])
-        culgt.culgt_functional(lat, links, ws, scal[1:2])
+        culgt.culgt_gauge_precision_functional(lat, links, ws, scal[0:1], scal[1:2])
 
     # ---- warm-up
     culgt.culgt_or_sweeps(lat, links, max(args.warmup, 3), omega)
@@ -304,7 +303,7 @@ def main():
     value = whole_job_value(world, V, args.steps, elapsed_max_ms * 1e-3)
 
     sweep_launches = 2 * args.steps
-    gpu_launches = sweep_launches + n_checks * 4        # theta: 2 kernels, F: 2 kernels
+    gpu_launches = sweep_launches + n_checks * 2        # fused theta+F: partial + final kernel
     launch_ms = (elapsed_ms - check_ms) / sweep_launches
     field_bytes = culgt.culgt_links_bytes(lat)
     alg_bytes_per_launch = 2 * field_bytes

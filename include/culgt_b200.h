@@ -64,7 +64,8 @@ typedef struct {
 size_t culgt_links_bytes(const culgt_lattice* lat);      /* internal field: 4*V*params*sizeof(real) */
 size_t culgt_canonical_bytes(const culgt_lattice* lat);  /* V*4*Nc*Nc*2*sizeof(real)                */
 size_t culgt_gfield_bytes(const culgt_lattice* lat);     /* V*Nc*Nc*2*sizeof(real)                  */
-size_t culgt_workspace_bytes(const culgt_lattice* lat);  /* reductions: block partials + 2 scalars   */
+size_t culgt_workspace_bytes(const culgt_lattice* lat);  /* reductions: block partials + 2 scalars;
+                                                            grows with the volume (V/128 doubles)    */
 
 /* Validate a descriptor: CULGT_OK, CULGT_ERR_NULL, CULGT_ERR_DIMS or CULGT_ERR_DESC. */
 int culgt_validate(const culgt_lattice* lat);
@@ -98,6 +99,11 @@ int culgt_gauge_precision(const culgt_lattice* lat, const void* links, void* wor
                           double* theta_dev, void* stream);
 int culgt_functional(const culgt_lattice* lat, const void* links, void* workspace,
                      double* F_dev, void* stream);
+
+/* a7 + a8 in ONE pass over the field (what the driver loop needs at every check): both
+ * scalars as above, written to the DEVICE addresses theta_dev and F_dev.  Same workspace. */
+int culgt_gauge_precision_functional(const culgt_lattice* lat, const void* links, void* workspace,
+                                     double* theta_dev, double* F_dev, void* stream);
 
 /* a9: U_mu(x) <- g(x) U_mu(x) g(x+mu)^dagger for all x, mu (the paper's worked code
  * example P:L105-118).  g: device pointer to a canonical g field (read-only); links in place. */

@@ -65,6 +65,7 @@ def lib() -> ctypes.CDLL:
     L.culgt_or_sweeps.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_gauge_precision.argtypes = [latp, vp, vp, vp, vp]
     L.culgt_functional.argtypes = [latp, vp, vp, vp, vp]
+    L.culgt_gauge_precision_functional.argtypes = [latp, vp, vp, vp, vp, vp]
     L.culgt_gauge_transform.argtypes = [latp, vp, vp, vp]
     L.culgt_landau_fix.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                    ctypes.c_int, ctypes.POINTER(ctypes.c_int), dp, dp, vp]
@@ -206,6 +207,13 @@ def culgt_functional(lat: Lattice, links, workspace, F_dev, stream=None) -> None
     _require_cuda()
     _check(lib().culgt_functional(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace),
                                   _ptr(F_dev), _stream(stream)), "culgt_functional")
+
+
+def culgt_gauge_precision_functional(lat: Lattice, links, workspace, theta_dev, F_dev, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_gauge_precision_functional(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace),
+                                                  _ptr(theta_dev), _ptr(F_dev), _stream(stream)),
+           "culgt_gauge_precision_functional")
 
 
 def culgt_gauge_transform(lat: Lattice, links, g, stream=None) -> None:

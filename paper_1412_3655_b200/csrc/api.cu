@@ -68,8 +68,9 @@ size_t culgt_gfield_bytes(const culgt_lattice* lat) {
 }
 
 size_t culgt_workspace_bytes(const culgt_lattice* lat) {
-  if (describe(lat, nullptr) != CULGT_OK) return 0;
-  return (size_t)(kMaxReduceBlocks + 2) * sizeof(double);   // block partials + {theta, F} scalars
+  LatticeDesc d;
+  if (describe(lat, &d) != CULGT_OK) return 0;
+  return reduce_workspace_doubles(d.geom.vh) * sizeof(double);   // block partials + {theta, F} scalars
 }
 
 int culgt_pack(const culgt_lattice* lat, const void* canonical, void* links, void* stream) {
@@ -157,19 +158,26 @@ int culgt_gauge_transform(const culgt_lattice* lat, void* links, const void* g, 
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
-// theta and F into the two doubles that follow the block partials in the workspace, read back.
+int culgt_gauge_precision_functional(const culgt_lattice* lat, const void* links, void* workspace,
+                                     double* theta_dev, double* F_dev, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !workspace || !theta_dev || !F_dev) return CULGT_ERR_NULL;
+  if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_theta_functional(d, links, (double*)workspace, theta_dev, F_dev, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+// theta and F (one fused pass) into the two doubles at the end of the workspace, read back.
 static int read_theta_F(const LatticeDesc& d, const void* links, void* workspace, cudaStream_t st,
                         double* theta, double* F) {
   double* ws = (double*)workspace;
-  double* scal = ws + kMaxReduceBlocks;
-  cudaError_t e = launch_gauge_precision(d, links, ws, scal, st);
+  double* scal = ws + reduce_workspace_doubles(d.geom.vh) - 2;
+  cudaError_t e = launch_theta_functional(d, links, ws, scal, scal + 1, st);
   if (e != cudaSuccess) return cuda_fail(e);
-  if (F) {
-    e = launch_functional(d, links, ws, scal + 1, st);
-    if (e != cudaSuccess) return cuda_fail(e);
-  }
   double host[2] = {0, 0};
-  e = cudaMemcpyAsync(host, scal, (F ? 2 : 1) * sizeof(double), cudaMemcpyDeviceToHost, st);
+  e = cudaMemcpyAsync(host, scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st);
   if (e != cudaSuccess) return cuda_fail(e);
   e = cudaStreamSynchronize(st);
   if (e != cudaSuccess) return cuda_fail(e);

@@ -28,6 +28,27 @@ __device__ __forceinline__ double block_sum(double v) {
   return t;   // valid in thread 0
 }
 
+// sum_ab |Delta_ab|^2 with Delta = [(K - K^dagger)/(2i)]_traceless (reading C-11):
+// D_ab = (K_ab - conj(K_ba))/(2i);  re(D_ab) = (im K_ab + im K_ba)/2, im(D_ab) = -(re K_ab - re K_ba)/2.
+__device__ __forceinline__ double theta_from_K(const double* K) {
+  double dre[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) dre[a] = K[CULGT_IM(a, a)];
+  const double tr = (dre[0] + dre[1] + dre[2]) * (1.0 / 3.0);
+  double sum = 0;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) sum += (dre[a] - tr) * (dre[a] - tr);
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = a + 1; b < 3; ++b) {
+      const double re = 0.5 * (K[CULGT_IM(a, b)] + K[CULGT_IM(b, a)]);
+      const double im = -0.5 * (K[CULGT_RE(a, b)] - K[CULGT_RE(b, a)]);
+      sum += 2.0 * (re * re + im * im);     // |D_ab|^2 + |D_ba|^2, D Hermitian
+    }
+  return sum;
+}
+
 // Per-site theta term for SU(3): sum_ab |Delta_ab|^2.
 template <typename S>
 __device__ __forceinline__ double theta_term_su3(const typename S::Vec* links, const Geom& g, int h, int parity) {
@@ -46,24 +67,7 @@ __device__ __forceinline__ double theta_term_su3(const typename S::Vec* links, c
     if (S::NP == 12) reconstruct_row2(U);
     accumulate(K, U, true);
   }
-  // D = (K - K^dagger)/(2i):  D_ab = (K_ab - conj(K_ba))/(2i);  re(D_ab) = (im K_ab + im K_ba)/2,
-  // im(D_ab) = -(re K_ab - re K_ba)/2.  Then remove the trace.
-  double dre[3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a) dre[a] = K[CULGT_IM(a, a)];
-  const double tr = (dre[0] + dre[1] + dre[2]) * (1.0 / 3.0);
-  double sum = 0;
-#pragma unroll
-  for (int a = 0; a < 3; ++a) sum += (dre[a] - tr) * (dre[a] - tr);
-#pragma unroll
-  for (int a = 0; a < 3; ++a)
-#pragma unroll
-    for (int b = a + 1; b < 3; ++b) {
-      const double re = 0.5 * (K[CULGT_IM(a, b)] + K[CULGT_IM(b, a)]);
-      const double im = -0.5 * (K[CULGT_RE(a, b)] - K[CULGT_RE(b, a)]);
-      sum += 2.0 * (re * re + im * im);     // |D_ab|^2 + |D_ba|^2, D Hermitian
-    }
-  return sum;
+  return theta_from_K(K);
 }
 
 // SU(2): Delta = d.sigma, tr[Delta Delta^dagger] = 2|d|^2, d = sum_mu a_mu(x) - a_mu(x-mu).
@@ -138,6 +142,78 @@ functional_partial_kernel(const typename S::Vec* __restrict__ links, const Geom 
   if (threadIdx.x == 0) partial[blockIdx.x] = s;
 }
 
+// Fused theta + F in one pass over the field (what the driver loop needs at every check).
+// CTA b handles the BLOCK/2 sites h in [b*BLOCK/2, (b+1)*BLOCK/2) of BOTH parities (threads
+// 0..BLOCK/2-1 black, the rest white): a link is read once as U_mu(x) by its own site and once
+// as U_mu(x'-mu) by the neighbour x' = x+mu of the other parity, and with both parities in one
+// CTA the second read comes from L1/L2 instead of HBM (mu = 0: same CTA; mu = 1,2: a few CTAs
+// away; mu = 3: one time-slice of CTAs away, far below the L2 size).  F = sum of Re tr over the
+// 4 up links of every site of both parities = every link exactly once.
+template <typename S, int BLOCK>
+__global__ void __launch_bounds__(BLOCK)
+theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
+                        double* __restrict__ partial_theta, double* __restrict__ partial_F) {
+  typedef typename S::Real Real;
+  constexpr int HALF = BLOCK / 2;
+  const int parity = threadIdx.x >= HALF;
+  const int h = blockIdx.x * HALF + (int)threadIdx.x - parity * HALF;
+  double th = 0, f = 0;
+  if (h < g.vh) {
+    const SiteCoord sc = decode_site(g, h, parity);
+    if (S::NC == 3) {
+      double K[18];
+#pragma unroll
+      for (int i = 0; i < 18; ++i) K[i] = 0;
+#pragma unroll
+      for (int mu = 0; mu < 4; ++mu) {
+        Real U[18];
+        load_params<S>(link_base<S>(links, g, parity, mu, h), g.vh, U);
+        if (S::NP == 12) reconstruct_row2(U);
+        f += (double)U[CULGT_RE(0, 0)] + (double)U[CULGT_RE(1, 1)] + (double)U[CULGT_RE(2, 2)];
+        accumulate(K, U, false);
+        load_params<S>(link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu)), g.vh, U);
+        if (S::NP == 12) reconstruct_row2(U);
+        accumulate(K, U, true);
+      }
+      th = theta_from_K(K);
+    } else {
+      double d[3] = {0, 0, 0};
+#pragma unroll
+      for (int mu = 0; mu < 4; ++mu) {
+        Real u[4], w[4];
+        load_params<S>(link_base<S>(links, g, parity, mu, h), g.vh, u);
+        load_params<S>(link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu)), g.vh, w);
+        f += 2.0 * (double)u[0];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) d[i] += (double)u[i + 1] - (double)w[i + 1];
+      }
+      th = 2.0 * (d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    }
+  }
+  const double st = block_sum<BLOCK>(th);
+  __syncthreads();                       // block_sum's shared slots are reused
+  const double sf = block_sum<BLOCK>(f);
+  if (threadIdx.x == 0) {
+    partial_theta[blockIdx.x] = st;
+    partial_F[blockIdx.x] = sf;
+  }
+}
+
+// Sums of two partial arrays by two blocks (blockIdx 0: theta, 1: F), fixed order, scaled.
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK)
+final_sum2_kernel(const double* __restrict__ partial, int n, double scale0, double scale1,
+                  double* __restrict__ out0, double* __restrict__ out1) {
+  const double* p = partial + (size_t)blockIdx.x * n;
+  double acc = 0;
+  for (int i = threadIdx.x; i < n; i += BLOCK) acc += p[i];
+  const double s = block_sum<BLOCK>(acc);
+  if (threadIdx.x == 0) {
+    if (blockIdx.x == 0) *out0 = s * scale0;
+    else *out1 = s * scale1;
+  }
+}
+
 // Second pass: one block sums `n` partials in a fixed order and scales.
 template <int BLOCK>
 __global__ void __launch_bounds__(BLOCK)
@@ -178,6 +254,19 @@ static cudaError_t run_functional(const LatticeDesc& d, const void* links, doubl
   return cudaGetLastError();
 }
 
+template <typename S>
+static cudaError_t run_theta_functional(const LatticeDesc& d, const void* links, double* ws, double* out_theta,
+                                        double* out_F, cudaStream_t st) {
+  constexpr int BLOCK = 256;
+  const int nblk = reduce_blocks_fused(d.geom.vh);
+  theta_functional_kernel<S, BLOCK><<<nblk, BLOCK, 0, st>>>((const typename S::Vec*)links, d.geom, ws, ws + nblk);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  final_sum2_kernel<kReduceBlock><<<2, kReduceBlock, 0, st>>>(ws, nblk, 1.0 / ((double)S::NC * (double)d.V),
+                                                             1.0 / (4.0 * S::NC * (double)d.V), out_theta, out_F);
+  return cudaGetLastError();
+}
+
 #define CULGT_DISPATCH(FN, ...)                                                                   \
   if (d.group == 2) {                                                                             \
     if (d.precision == 32) return FN<Storage<float, 2, 4> >(__VA_ARGS__);                         \
@@ -193,6 +282,10 @@ static cudaError_t run_functional(const LatticeDesc& d, const void* links, doubl
 cudaError_t launch_gauge_precision(const LatticeDesc& d, const void* links, double* workspace,
                                    double* out, cudaStream_t st) {
   CULGT_DISPATCH(run_theta, d, links, workspace, out, st)
+}
+cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
+                                    double* out_theta, double* out_F, cudaStream_t st) {
+  CULGT_DISPATCH(run_theta_functional, d, links, workspace, out_theta, out_F, st)
 }
 cudaError_t launch_functional(const LatticeDesc& d, const void* links, double* workspace,
                               double* out, cudaStream_t st) {

@@ -67,6 +67,12 @@ class GpuField:
         culgt.culgt_functional(self.lat, self.links, self.ws, self.scal[1:2])
         return float(self.scal[1].item())
 
+    def theta_functional(self):
+        """both scalars from the fused one-pass entry point"""
+        culgt.culgt_gauge_precision_functional(self.lat, self.links, self.ws, self.scal[0:1], self.scal[1:2])
+        th, F = self.scal.cpu().tolist()
+        return th, F
+
     def transform(self, g):
         gt = torch.from_numpy(li.to_real(np.ascontiguousarray(g), np_dtype(self.lat.precision))).cuda()
         culgt.culgt_gauge_transform(self.lat, self.links, gt)

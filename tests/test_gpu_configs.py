@@ -141,3 +141,41 @@ def test_cfg3_32x4_links_and_first_sweeps(name):
         else:
             assert abs(f.theta() - th_o) <= 1e-3 * th_o, s
             assert abs(f.functional() - F_o) <= 2e-6, s
+
+
+@pytest.mark.parametrize("name", ["cfg4_fp32", "cfg4_fp64"])
+def test_cfg4_large_volume_links_theta_F(name):
+    """configs[4] (48^3 x 96 fp32-12 = 2.04 GB, 64^4 fp64-18 = 9.66 GB; hot Haar links; 64-bit byte
+    offsets, asymmetric extents, plane sizes that are not powers of two) in the launch
+    configuration bench.py times: theta and F of the input, ALL 4V links after the first sweep,
+    theta and F after it -- the oracle needs ~2 s per sweep at this size, so one sweep."""
+    import psutil
+    c = li.CONFIGS[name]
+    need = 6 * li.volume(c["dims"]) * 4 * 18 * 8           # ~6 fp64 canonical copies on the host
+    if psutil.virtual_memory().available < need:
+        pytest.skip(f"host has less than {need >> 30} GiB free for the full-size oracle field")
+    _INPUTS.clear()
+    c, f, ref = field_and_ref(name)
+    _INPUTS.clear()
+    dims, om, prec = c["dims"], c["omega"], c["precision"]
+    th, F = f.theta_functional()
+    th_o, F_o = oracle.gauge_precision(dims, ref), oracle.functional(dims, ref)
+    if prec == 64:
+        assert theta_close(th, th_o) and abs(F - F_o) <= 1e-10 * abs(F_o) + 1e-15
+    else:
+        assert abs(th - th_o) <= 1e-5 * th_o and abs(F - F_o) <= 1e-6
+    oracle.full_sweep(dims, ref, om)
+    f.sweep(om)
+    got = f.download()
+    err = 0.0
+    step = 1 << 20                                          # compare in slabs: no third full copy
+    for lo in range(0, got.shape[0], step):
+        err = max(err, float(np.abs(got[lo:lo + step] - li.from_real(ref[lo:lo + step])).max()))
+    del got
+    assert err < TOL_LINK[prec], err
+    th, F = f.theta_functional()
+    th_o, F_o = oracle.gauge_precision(dims, ref), oracle.functional(dims, ref)
+    if prec == 64:
+        assert theta_close(th, th_o) and abs(F - F_o) <= 1e-10 * abs(F_o) + 1e-15
+    else:
+        assert abs(th - th_o) <= 1e-3 * th_o and abs(F - F_o) <= 2e-6

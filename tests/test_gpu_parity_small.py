@@ -94,7 +94,7 @@ def test_su2_links_after_one_sweep(dims, precision):
     assert np.abs(f.download() - li.from_real(ref)).max() < TOL_LINK[precision]
 
 
-@pytest.mark.parametrize("dims", DIMS[:4])
+@pytest.mark.parametrize("dims", DIMS)
 @pytest.mark.parametrize("group,precision,params", [(3, 64, 18), (3, 64, 12), (3, 32, 12), (3, 32, 18),
                                                     (2, 64, 4), (2, 32, 4)])
 def test_theta_and_F_match_oracle(dims, group, precision, params):
@@ -111,6 +111,12 @@ def test_theta_and_F_match_oracle(dims, group, precision, params):
         assert abs(F - F_o) <= 1e-6
     # deterministic: same bits when repeated
     assert f.theta() == th and f.functional() == F
+    # the fused one-pass entry point gives the same two scalars (different summation order only)
+    th2, F2 = f.theta_functional()
+    assert abs(th2 - th) <= 1e-13 * th and abs(F2 - F) <= 1e-13
+    assert f.theta_functional() == (th2, F2)
+    if precision == 64:
+        assert theta_close(th2, th_o) and abs(F2 - F_o) <= 1e-10 * abs(F_o) + 1e-15
 
 
 @pytest.mark.parametrize("dims", DIMS[:4])
