@@ -133,7 +133,9 @@ int culgt_gauge_precision(const culgt_lattice* lat, const void* links, void* wor
   if (rc != CULGT_OK) return rc;
   if (!links || !workspace || !theta_dev) return CULGT_ERR_NULL;
   if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
-  cudaError_t e = launch_gauge_precision(d, links, (double*)workspace, theta_dev, (cudaStream_t)stream);
+  // one fused pass computes both scalars; F goes to the spare slot at the end of the workspace
+  double* spare = (double*)workspace + reduce_workspace_doubles(d.geom.vh) - 1;
+  cudaError_t e = launch_theta_functional(d, links, (double*)workspace, theta_dev, spare, (cudaStream_t)stream);
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
@@ -144,7 +146,8 @@ int culgt_functional(const culgt_lattice* lat, const void* links, void* workspac
   if (rc != CULGT_OK) return rc;
   if (!links || !workspace || !F_dev) return CULGT_ERR_NULL;
   if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
-  cudaError_t e = launch_functional(d, links, (double*)workspace, F_dev, (cudaStream_t)stream);
+  double* spare = (double*)workspace + reduce_workspace_doubles(d.geom.vh) - 2;
+  cudaError_t e = launch_theta_functional(d, links, (double*)workspace, spare, F_dev, (cudaStream_t)stream);
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 

@@ -215,8 +215,20 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
       Real U[18];
       asm volatile("" ::: "memory");   // keep the shared-memory reads of link l behind link l-1's use
       load_link(stage, l, U, std::false_type());
-      if (S::NP == 12) reconstruct_row2(U);
-      accumulate(K, U, ((q * LPT + l) & 1) != 0);
+      if (S::NP == 12 && sizeof(Real) < sizeof(Acc)) {
+        // fp32 12-parameter storage: widen the two stored rows and rebuild the third row in
+        // fp64 for K.  A third row rebuilt in fp32 puts ~1e-7 into K, which the small-|p| sites
+        // of a hot 10^7-site lattice amplify past the 2e-5 link tolerance; it also
+        // needs 12 instead of 18 fp32->fp64 conversions per link.
+        Acc Ua[18];
+#pragma unroll
+        for (int i = 0; i < 12; ++i) Ua[i] = (Acc)U[i];
+        reconstruct_row2(Ua);
+        accumulate(K, Ua, ((q * LPT + l) & 1) != 0);
+      } else {
+        if (S::NP == 12) reconstruct_row2(U);
+        accumulate(K, U, ((q * LPT + l) & 1) != 0);
+      }
     }
 #pragma unroll
     for (int m = 1; m < TPS; m <<= 1) {

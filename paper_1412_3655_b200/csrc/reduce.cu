@@ -1,11 +1,12 @@
-// reduce.cu -- a7 functional F and a8 gauge precision theta.
+// reduce.cu -- a7 functional F and a8 gauge precision theta, one fused pass.
 //
 //   F     = 1/(4 Nc V) sum_x sum_mu Re tr U_mu(x)                      PAPER.md eq. (2) at g = 1
 //   theta = 1/(Nc V) sum_x tr[Delta(x) Delta(x)^dagger],  Delta(x) = [(K(x) - K(x)^dagger)/(2i)]_traceless
 //           which equals sum_mu A_mu(x) - A_mu(x-mu) of eq. (1) (reading C-11).
 // Reduction: per-thread fp64 partial -> warp xor-shuffles -> one shared-memory slot per warp ->
-// one partial per block in the workspace -> a single block sums the partials in a fixed order.
-// Deterministic: no atomics, the same launch always produces the same bits.
+// one partial per block in the workspace -> a single block per quantity sums the partials in a
+// fixed order.  Deterministic: no atomics, the same launch always produces the same bits.
+// All arithmetic is fp64 on the stored values (12-parameter storage: third row rebuilt in fp64).
 #include "lattice.cuh"
 #include "su_math.cuh"
 #include "kernels.h"
@@ -49,99 +50,6 @@ __device__ __forceinline__ double theta_from_K(const double* K) {
   return sum;
 }
 
-// Per-site theta term for SU(3): sum_ab |Delta_ab|^2.
-template <typename S>
-__device__ __forceinline__ double theta_term_su3(const typename S::Vec* links, const Geom& g, int h, int parity) {
-  typedef typename S::Real Real;
-  const SiteCoord sc = decode_site(g, h, parity);
-  double K[18];
-#pragma unroll
-  for (int i = 0; i < 18; ++i) K[i] = 0;
-#pragma unroll
-  for (int mu = 0; mu < 4; ++mu) {
-    Real U[18];
-    load_params<S>(link_base<S>(links, g, parity, mu, h), g.vh, U);
-    if (S::NP == 12) reconstruct_row2(U);
-    accumulate(K, U, false);
-    load_params<S>(link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu)), g.vh, U);
-    if (S::NP == 12) reconstruct_row2(U);
-    accumulate(K, U, true);
-  }
-  return theta_from_K(K);
-}
-
-// SU(2): Delta = d.sigma, tr[Delta Delta^dagger] = 2|d|^2, d = sum_mu a_mu(x) - a_mu(x-mu).
-template <typename S>
-__device__ __forceinline__ double theta_term_su2(const typename S::Vec* links, const Geom& g, int h, int parity) {
-  typedef typename S::Real Real;
-  const SiteCoord sc = decode_site(g, h, parity);
-  double d[3] = {0, 0, 0};
-#pragma unroll
-  for (int mu = 0; mu < 4; ++mu) {
-    Real u[4], w[4];
-    load_params<S>(link_base<S>(links, g, parity, mu, h), g.vh, u);
-    load_params<S>(link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu)), g.vh, w);
-#pragma unroll
-    for (int i = 0; i < 3; ++i) d[i] += (double)u[i + 1] - (double)w[i + 1];
-  }
-  return 2.0 * (d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-}
-
-template <typename S, int BLOCK>
-__global__ void __launch_bounds__(BLOCK)
-theta_partial_kernel(const typename S::Vec* __restrict__ links, const Geom g, double* __restrict__ partial) {
-  double acc = 0;
-  const long long total = 2ll * g.vh;
-  for (long long t = (long long)blockIdx.x * BLOCK + threadIdx.x; t < total; t += (long long)gridDim.x * BLOCK) {
-    const int parity = t >= g.vh;
-    const int h = (int)(t - (long long)parity * g.vh);
-    acc += (S::NC == 3) ? theta_term_su3<S>(links, g, h, parity) : theta_term_su2<S>(links, g, h, parity);
-  }
-  const double s = block_sum<BLOCK>(acc);
-  if (threadIdx.x == 0) partial[blockIdx.x] = s;
-}
-
-// F: sum over all stored links of Re tr U.  One thread per (parity, mu, h) link, grid-strided;
-// consecutive threads walk consecutive h of one plane set.
-template <typename S, int BLOCK>
-__global__ void __launch_bounds__(BLOCK)
-functional_partial_kernel(const typename S::Vec* __restrict__ links, const Geom g, double* __restrict__ partial) {
-  typedef typename S::Real Real;
-  double acc = 0;
-  const long long total = 8ll * g.vh;
-  for (long long t = (long long)blockIdx.x * BLOCK + threadIdx.x; t < total; t += (long long)gridDim.x * BLOCK) {
-    const int pm = (int)(t / g.vh);               // parity*4 + mu
-    const int h = (int)(t - (long long)pm * g.vh);
-    const typename S::Vec* p = links + ((size_t)pm * S::NV) * (size_t)g.vh + (size_t)h;
-    if (S::NC == 2) {
-      Real a[4];
-      load_params<S>(p, g.vh, a);
-      acc += 2.0 * (double)a[0];
-    } else if (S::NP == 18) {
-      // diagonal entries are reals 0, 8, 16 of the 18
-      Real m[18];
-      if (S::VL == 2) {
-        Real v[2];
-        vec_get(p[0], v); acc += (double)v[0];
-        vec_get(p[(size_t)4 * g.vh], v); acc += (double)v[0];
-        vec_get(p[(size_t)8 * g.vh], v); acc += (double)v[0];
-      } else {
-        load_params<S>(p, g.vh, m);
-        acc += (double)m[0] + (double)m[8] + (double)m[16];
-      }
-    } else {
-      Real m[18];
-      load_params<S>(p, g.vh, m);
-      // Re u22 = Re conj(u00 u11 - u01 u10)
-      const Real u22 = m[CULGT_RE(0, 0)] * m[CULGT_RE(1, 1)] - m[CULGT_IM(0, 0)] * m[CULGT_IM(1, 1)]
-                     - m[CULGT_RE(0, 1)] * m[CULGT_RE(1, 0)] + m[CULGT_IM(0, 1)] * m[CULGT_IM(1, 0)];
-      acc += (double)m[CULGT_RE(0, 0)] + (double)m[CULGT_RE(1, 1)] + (double)u22;
-    }
-  }
-  const double s = block_sum<BLOCK>(acc);
-  if (threadIdx.x == 0) partial[blockIdx.x] = s;
-}
-
 // Fused theta + F in one pass over the field (what the driver loop needs at every check).
 // CTA b handles the BLOCK/2 sites h in [b*BLOCK/2, (b+1)*BLOCK/2) of BOTH parities (threads
 // 0..BLOCK/2-1 black, the rest white): a link is read once as U_mu(x) by its own site and once
@@ -167,13 +75,18 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
 #pragma unroll
       for (int mu = 0; mu < 4; ++mu) {
         Real U[18];
+        double Ud[18];                       // widened first: the third row is rebuilt in fp64
         load_params<S>(link_base<S>(links, g, parity, mu, h), g.vh, U);
-        if (S::NP == 12) reconstruct_row2(U);
-        f += (double)U[CULGT_RE(0, 0)] + (double)U[CULGT_RE(1, 1)] + (double)U[CULGT_RE(2, 2)];
-        accumulate(K, U, false);
+#pragma unroll
+        for (int i = 0; i < S::NP; ++i) Ud[i] = (double)U[i];
+        if (S::NP == 12) reconstruct_row2(Ud);
+        f += Ud[CULGT_RE(0, 0)] + Ud[CULGT_RE(1, 1)] + Ud[CULGT_RE(2, 2)];
+        accumulate(K, Ud, false);
         load_params<S>(link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu)), g.vh, U);
-        if (S::NP == 12) reconstruct_row2(U);
-        accumulate(K, U, true);
+#pragma unroll
+        for (int i = 0; i < S::NP; ++i) Ud[i] = (double)U[i];
+        if (S::NP == 12) reconstruct_row2(Ud);
+        accumulate(K, Ud, true);
       }
       th = theta_from_K(K);
     } else {
@@ -214,46 +127,6 @@ final_sum2_kernel(const double* __restrict__ partial, int n, double scale0, doub
   }
 }
 
-// Second pass: one block sums `n` partials in a fixed order and scales.
-template <int BLOCK>
-__global__ void __launch_bounds__(BLOCK)
-final_sum_kernel(const double* __restrict__ partial, int n, double scale, double* __restrict__ out) {
-  double acc = 0;
-  for (int i = threadIdx.x; i < n; i += BLOCK) acc += partial[i];
-  const double s = block_sum<BLOCK>(acc);
-  if (threadIdx.x == 0) *out = s * scale;
-}
-
-static int reduce_grid(long long items) {
-  long long blocks = (items + kReduceBlock - 1) / kReduceBlock;
-  // persistent-style grid: a multiple of the 148 SMs, capped by the workspace
-  const long long cap = 148 * 8;
-  if (blocks > cap) blocks = cap;
-  if (blocks > kMaxReduceBlocks) blocks = kMaxReduceBlocks;
-  if (blocks < 1) blocks = 1;
-  return (int)blocks;
-}
-
-template <typename S>
-static cudaError_t run_theta(const LatticeDesc& d, const void* links, double* ws, double* out, cudaStream_t st) {
-  const int grid = reduce_grid(d.V);
-  theta_partial_kernel<S, kReduceBlock><<<grid, kReduceBlock, 0, st>>>((const typename S::Vec*)links, d.geom, ws);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  final_sum_kernel<kReduceBlock><<<1, kReduceBlock, 0, st>>>(ws, grid, 1.0 / ((double)S::NC * (double)d.V), out);
-  return cudaGetLastError();
-}
-
-template <typename S>
-static cudaError_t run_functional(const LatticeDesc& d, const void* links, double* ws, double* out, cudaStream_t st) {
-  const int grid = reduce_grid(4 * d.V);
-  functional_partial_kernel<S, kReduceBlock><<<grid, kReduceBlock, 0, st>>>((const typename S::Vec*)links, d.geom, ws);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  final_sum_kernel<kReduceBlock><<<1, kReduceBlock, 0, st>>>(ws, grid, 1.0 / (4.0 * S::NC * (double)d.V), out);
-  return cudaGetLastError();
-}
-
 template <typename S>
 static cudaError_t run_theta_functional(const LatticeDesc& d, const void* links, double* ws, double* out_theta,
                                         double* out_F, cudaStream_t st) {
@@ -279,17 +152,9 @@ static cudaError_t run_theta_functional(const LatticeDesc& d, const void* links,
   if (d.params == 12) return FN<Storage<double, 3, 12> >(__VA_ARGS__);                            \
   return FN<Storage<double, 3, 18> >(__VA_ARGS__);
 
-cudaError_t launch_gauge_precision(const LatticeDesc& d, const void* links, double* workspace,
-                                   double* out, cudaStream_t st) {
-  CULGT_DISPATCH(run_theta, d, links, workspace, out, st)
-}
 cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
                                     double* out_theta, double* out_F, cudaStream_t st) {
   CULGT_DISPATCH(run_theta_functional, d, links, workspace, out_theta, out_F, st)
-}
-cudaError_t launch_functional(const LatticeDesc& d, const void* links, double* workspace,
-                              double* out, cudaStream_t st) {
-  CULGT_DISPATCH(run_functional, d, links, workspace, out, st)
 }
 
 }  // namespace culgt

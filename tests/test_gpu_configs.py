@@ -162,8 +162,8 @@ def test_cfg4_large_volume_links_theta_F(name):
     th_o, F_o = oracle.gauge_precision(dims, ref), oracle.functional(dims, ref)
     if prec == 64:
         assert theta_close(th, th_o) and abs(F - F_o) <= 1e-10 * abs(F_o) + 1e-15
-    else:
-        assert abs(th - th_o) <= 1e-5 * th_o and abs(F - F_o) <= 1e-6
+    else:   # fp32 storage, fp64 reduction arithmetic on identical inputs
+        assert abs(th - th_o) <= 1e-9 * th_o and abs(F - F_o) <= 1e-10
     oracle.full_sweep(dims, ref, om)
     f.sweep(om)
     got = f.download()
