@@ -252,6 +252,11 @@ CONFIGS = {
                          kind="near_identity", eps=0.8, scramble=True, omega=1.7, seed=1003),
     "cfg3_fp64_12": dict(dims=(32, 32, 32, 32), group=3, precision=64, params=12,
                          kind="near_identity", eps=0.8, scramble=True, omega=1.7, seed=1003),
+    # the SU(2) path of cfg1 at the headline volume (not a BASELINE.json config; measurement only)
+    "su2_32_fp64": dict(dims=(32, 32, 32, 32), group=2, precision=64, params=4, kind="haar",
+                        eps=0.0, scramble=False, omega=1.5, seed=1001),
+    "su2_32_fp32": dict(dims=(32, 32, 32, 32), group=2, precision=32, params=4, kind="haar",
+                        eps=0.0, scramble=False, omega=1.5, seed=1001),
     "cfg4_fp32": dict(dims=(48, 48, 48, 96), group=3, precision=32, params=12, kind="haar",
                       eps=0.0, scramble=False, omega=1.7, seed=1004),
     "cfg4_fp64": dict(dims=(64, 64, 64, 64), group=3, precision=64, params=18, kind="haar",

@@ -13,6 +13,7 @@
 // measurement (profiles/).
 #include "lattice.cuh"
 #include "su_math.cuh"
+#include "su2_power.cuh"
 #include "kernels.h"
 
 namespace culgt {
@@ -85,14 +86,19 @@ or_sweep_su3_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
 }
 
 // ---------------------------------------------------------------------------------------------
-// SU(2), 4-parameter storage, one thread per site, all arithmetic in Real.
+// SU(2), 4-parameter storage, one thread per site.  8 links = 32 (fp32) / 64 (fp64) registers, so
+// they stay in registers.  K(x) and the closed-form update g = K^dagger/sqrt(det K^dagger)
+// (PAPER.md L52), g^omega, in fp64 for both storage precisions (the same conditioning argument as
+// for SU(3), reading C-15); the 8 quaternion products in the storage precision.  Odd-parity
+// launches walk the site blocks in descending order (L2 carry-over, as the SU(3) kernel).
 // ---------------------------------------------------------------------------------------------
 template <typename S, int BLOCK>
 __global__ void __launch_bounds__(BLOCK)
 or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
-                    const typename S::Real omega) {
+                    const double omega, const int reverse) {
   typedef typename S::Real Real;
-  const int h = blockIdx.x * BLOCK + threadIdx.x;
+  const int blk = reverse ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x;
+  const int h = blk * BLOCK + threadIdx.x;
   if (h >= g.vh) return;
   const SiteCoord sc = decode_site(g, h, parity);
   Real U[8][4];
@@ -105,18 +111,16 @@ or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
 #pragma unroll
   for (int l = 0; l < 8; ++l) load_params<S>(ptr[l], g.vh, U[l]);
   // K = k0 + i k.sigma = sum_mu u_up + conj(u_dn)
-  Real k[4] = {0, 0, 0, 0};
+  double k[4] = {0, 0, 0, 0};
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) {
-    k[0] += U[2 * mu][0] + U[2 * mu + 1][0];
+    k[0] += (double)U[2 * mu][0] + (double)U[2 * mu + 1][0];
 #pragma unroll
-    for (int i = 1; i < 4; ++i) k[i] += U[2 * mu][i] - U[2 * mu + 1][i];
+    for (int i = 1; i < 4; ++i) k[i] += (double)U[2 * mu][i] - (double)U[2 * mu + 1][i];
   }
-  const Real n2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3];
-  if (n2 == 0) return;                               // K = 0: skip the update (C-9)
-  const Real ninv = rsqrt_t(n2);
-  Real G[4] = {k[0] * ninv, -k[1] * ninv, -k[2] * ninv, -k[3] * ninv};   // K^dagger / sqrt(det K^dagger)
-  su2_pow(G, omega);
+  double Gd[4];
+  if (!su2_update_power<(sizeof(Real) == 8)>(k, omega, Gd)) return;   // K = 0: skip the update (C-9)
+  const Real G[4] = {(Real)Gd[0], (Real)Gd[1], (Real)Gd[2], (Real)Gd[3]};
 #pragma unroll
   for (int l = 0; l < 8; ++l) {
     Real R[4];
@@ -143,8 +147,7 @@ template <typename S>
 static cudaError_t launch_su2(void* links, const Geom& g, int parity, double omega, cudaStream_t st) {
   constexpr int BLOCK = 128;
   const unsigned grid = (unsigned)((g.vh + BLOCK - 1) / BLOCK);
-  or_sweep_su2_kernel<S, BLOCK><<<grid, BLOCK, 0, st>>>(
-      (typename S::Vec*)links, g, parity, (typename S::Real)omega);
+  or_sweep_su2_kernel<S, BLOCK><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g, parity, omega, parity);
   return cudaGetLastError();
 }
 
