@@ -59,6 +59,10 @@ def _load():
     lib.oracle_plaquette.argtypes = [i32p, ctypes.c_int, dp]
     lib.oracle_plaquette.restype = ctypes.c_double
     lib.oracle_reconstruct12.argtypes = [ctypes.c_int64, dp]
+    lib.oracle_K_coulomb.argtypes = [i32p, ctypes.c_int, dp, dp]
+    lib.oracle_delta_coulomb.argtypes = [i32p, ctypes.c_int, dp, dp]
+    lib.oracle_or_sweep_coulomb.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double]
+    lib.oracle_coulomb_theta_F.argtypes = [i32p, ctypes.c_int, dp, dp, dp]
     _lib = lib
     return lib
 
@@ -166,3 +170,39 @@ def reconstruct12(m: np.ndarray) -> None:
     if m.shape[-3:] != (3, 3, 2):
         raise ValueError("need [...,3,3,2]")
     _load().oracle_reconstruct12(int(m.size // 18), _dp(m))
+
+
+# ---- Coulomb gauge (reading C-22): spatial directions only, per time-slice ----------
+
+def K_coulomb_field(dims, u: np.ndarray) -> np.ndarray:
+    nc = _check_links(dims, u)
+    out = np.empty((u.shape[0], nc, nc, 2))
+    _load().oracle_K_coulomb(_dims(dims), nc, _dp(u), _dp(out))
+    return out
+
+
+def delta_coulomb_field(dims, u: np.ndarray) -> np.ndarray:
+    nc = _check_links(dims, u)
+    out = np.empty((u.shape[0], nc, nc, 2))
+    _load().oracle_delta_coulomb(_dims(dims), nc, _dp(u), _dp(out))
+    return out
+
+
+def or_sweep_coulomb(dims, u: np.ndarray, parity: int, omega: float) -> None:
+    """One Coulomb-gauge half-sweep, in place."""
+    nc = _check_links(dims, u)
+    _load().oracle_or_sweep_coulomb(_dims(dims), nc, _dp(u), int(parity), float(omega))
+
+
+def full_sweep_coulomb(dims, u: np.ndarray, omega: float) -> None:
+    or_sweep_coulomb(dims, u, 0, omega)
+    or_sweep_coulomb(dims, u, 1, omega)
+
+
+def coulomb_theta_F(dims, u: np.ndarray):
+    """(theta_t, F_t): float64 arrays of length N3, one value per time-slice."""
+    nc = _check_links(dims, u)
+    n3 = int(dims[3])
+    th, f = np.empty(n3), np.empty(n3)
+    _load().oracle_coulomb_theta_F(_dims(dims), nc, _dp(u), _dp(th), _dp(f))
+    return th, f

@@ -406,3 +406,89 @@ void oracle_reconstruct12(int64_t n, double* M) {
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// Coulomb gauge (named by the paper beside Landau gauge, P:L7; its details are in the
+// paper's ref. [2], which is not available -- DESIGN.md reading C-22):
+// the Landau formulas with mu restricted to the 3 spatial directions, time-slice by time-slice.
+//   F_t   = 1/(3 N_c V_s) sum_{x in slice t} sum_{i<3} Re tr U_i(x)                (eq. (2), i < 3)
+//   K_C(x) = sum_{i<3} [ U_i(x) + U_i(x-i)^dagger ]                                (eq. (3), i < 3)
+//   Delta_C(x) = sum_{i<3} ( A_i(x) - A_i(x-i) ),  theta_t = 1/(N_c V_s) sum_{x in t} tr[Delta_C Delta_C^dagger]
+// The site update is the same G = site_G(K_C, omega); being a gauge transformation g(x) it acts
+// on ALL 8 links touching x, time links included, although they do not enter K_C.
+// ---------------------------------------------------------------------------------------------
+namespace {
+Mat gather_K_spatial(const double* U, const Lat& L, int64_t s) {
+  Mat K = zero_mat();
+  for (int mu = 0; mu < 3; ++mu) {
+    K = add(K, load_mat(link_ptr(U, L, s, mu), L.nc), L.nc);
+    int64_t sd = neighbour(L, s, mu, -1);
+    K = add(K, dagger(load_mat(link_ptr(U, L, sd, mu), L.nc), L.nc), L.nc);
+  }
+  return K;
+}
+Mat delta_spatial_at(const double* U, const Lat& L, int64_t s) {
+  Mat D = zero_mat();
+  for (int mu = 0; mu < 3; ++mu) {
+    Mat Ax = gauge_field_A(load_mat(link_ptr(U, L, s, mu), L.nc), L.nc);
+    Mat Ad = gauge_field_A(load_mat(link_ptr(U, L, neighbour(L, s, mu, -1), mu), L.nc), L.nc);
+    for (int a = 0; a < L.nc; ++a)
+      for (int b = 0; b < L.nc; ++b) D.e[a][b] += Ax.e[a][b] - Ad.e[a][b];
+  }
+  return D;
+}
+}  // namespace
+
+extern "C" {
+
+// K_C(x) for every site: out is double[V][nc][nc][2].
+void oracle_K_coulomb(const int32_t* dims, int nc, const double* U, double* out) {
+  Lat L = make_lat(dims, nc);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) store_mat(out + s * nc * nc * 2, nc, gather_K_spatial(U, L, s));
+}
+
+// Delta_C(x) for every site: out is double[V][nc][nc][2].
+void oracle_delta_coulomb(const int32_t* dims, int nc, const double* U, double* out) {
+  Lat L = make_lat(dims, nc);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) store_mat(out + s * nc * nc * 2, nc, delta_spatial_at(U, L, s));
+}
+
+// One HALF sweep of Coulomb-gauge overrelaxation over the sites of `parity`, in place.
+void oracle_or_sweep_coulomb(const int32_t* dims, int nc, double* U, int parity, double omega) {
+  Lat L = make_lat(dims, nc);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    if (parity_of(L, s) != parity) continue;
+    Mat G = site_G(gather_K_spatial(U, L, s), omega, nc);
+    Mat Gd = dagger(G, nc);
+    for (int mu = 0; mu < 4; ++mu) {
+      double* up = link_ptr(U, L, s, mu);
+      store_mat(up, nc, mul(G, load_mat(up, nc), nc));
+      double* dn = link_ptr(U, L, neighbour(L, s, mu, -1), mu);
+      store_mat(dn, nc, mul(load_mat(dn, nc), Gd, nc));
+    }
+  }
+}
+
+// theta_t and F_t for every time-slice t = x3: both are double[N3].
+void oracle_coulomb_theta_F(const int32_t* dims, int nc, const double* U, double* theta_t, double* F_t) {
+  Lat L = make_lat(dims, nc);
+  const int64_t Vs = (int64_t)L.N[0] * L.N[1] * L.N[2];
+  std::vector<double> th(L.V), f(L.V);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    Mat D = delta_spatial_at(U, L, s);
+    th[s] = trace(mul(D, dagger(D, nc), nc), nc).real();
+    double t = 0.0;
+    for (int mu = 0; mu < 3; ++mu) t += trace(load_mat(link_ptr(U, L, s, mu), nc), nc).real();
+    f[s] = t;
+  }
+  for (int t = 0; t < L.N[3]; ++t) {          // sites of slice t are contiguous in canonical order
+    theta_t[t] = neumaier_sum(th.data() + t * Vs, Vs) / ((double)nc * (double)Vs);
+    F_t[t] = neumaier_sum(f.data() + t * Vs, Vs) / (3.0 * nc * (double)Vs);
+  }
+}
+
+}  // extern "C"
