@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--workload", default="cfg3_fp32", choices=sorted(li.CONFIGS))
     ap.add_argument("--check-every", type=int, default=50)
     ap.add_argument("--variant", type=int, default=0, help="sweep kernel variant (0 = default)")
+    ap.add_argument("--gauge", default="landau", choices=["landau", "coulomb"],
+                    help="coulomb: K(x) from the spatial links, per-slice theta_t/F_t (DESIGN.md C-22)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -126,15 +128,16 @@ class ClockSampler:
                 "samples": len(self.samples)}
 
 
-def time_oracle(dims, group, ur, omega, max_sweeps, budget_s, threads):
+def time_oracle(dims, group, ur, omega, max_sweeps, budget_s, threads, gauge="landau"):
     """Full oracle sweeps until budget_s or max_sweeps; returns (site-updates/s, sweeps)."""
     import oracle
     oracle.set_threads(threads)
+    sweep = oracle.full_sweep_coulomb if gauge == "coulomb" else oracle.full_sweep
     V = li.volume(dims)
     t0 = time.perf_counter()
     n = 0
     while n < max_sweeps:
-        oracle.full_sweep(dims, ur, omega)
+        sweep(dims, ur, omega)
         n += 1
         if time.perf_counter() - t0 > budget_s:
             break
@@ -161,11 +164,12 @@ def run_reference(args):
     if cfg["precision"] == 32:
         u = li.round_to_fp32(u)
     ur = li.to_real(u)
+    sweep = oracle.full_sweep_coulomb if args.gauge == "coulomb" else oracle.full_sweep
     for _ in range(args.warmup):
-        oracle.full_sweep(dims, ur, cfg["omega"])
+        sweep(dims, ur, cfg["omega"])
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle.full_sweep(dims, ur, cfg["omega"])
+        sweep(dims, ur, cfg["omega"])
     dt = time.perf_counter() - t0
     V = li.volume(dims)
     value = V * args.steps / dt
@@ -176,7 +180,7 @@ def run_reference(args):
         "data": "synthetic", "config": workload_config(args, cfg),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-        "gflops": value * flops_per_site(cfg) / 1e9,
+        "gflops": value * flops_per_site(cfg, args.gauge) / 1e9,
     }
     print(json.dumps(line), flush=True)
 
@@ -203,12 +207,16 @@ def rank_seed(base_seed: int, rank: int) -> int:
     return base_seed + 7919 * rank
 
 
-def flops_per_site(cfg):
+def flops_per_site(cfg, gauge="landau"):
+    """Fixed algorithmic counts: Coulomb gauge gathers 6 links instead of 8 into K."""
+    if gauge == "coulomb":
+        return 2304 - 36 if cfg["group"] == 3 else 278 - 8
     return 2304 if cfg["group"] == 3 else 278
 
 
 def workload_config(args, cfg):
     return {
+        "gauge": args.gauge,
         "workload": f"{args.workload}: {'x'.join(str(d) for d in cfg['dims'])} SU({cfg['group']}) "
                     f"fp{cfg['precision']} {cfg['params']}-parameter, omega={cfg['omega']}, "
                     f"{cfg['kind']} eps={cfg['eps']} scramble={cfg['scramble']} seed={cfg['seed']}",
@@ -266,11 +274,20 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    coulomb = args.gauge == "coulomb"
+    n3 = int(dims[3])
+    if coulomb:
+        scal = torch.zeros(2 * n3, dtype=torch.float64, device="cuda")     # theta_t, F_t per slice
+    sweeps = culgt.culgt_or_sweeps_coulomb if coulomb else culgt.culgt_or_sweeps
+
     def check():
-        culgt.culgt_gauge_precision_functional(lat, links, ws, scal[0:1], scal[1:2])
+        if coulomb:
+            culgt.culgt_coulomb_precision_functional(lat, links, ws, scal[:n3], scal[n3:])
+        else:
+            culgt.culgt_gauge_precision_functional(lat, links, ws, scal[0:1], scal[1:2])
 
     # ---- warm-up
-    culgt.culgt_or_sweeps(lat, links, max(args.warmup, 3), omega)
+    sweeps(lat, links, max(args.warmup, 3), omega)
     check()
     barrier()
 
@@ -284,7 +301,7 @@ def main():
     done = 0
     while done < args.steps:
         n = min(args.check_every, args.steps - done)
-        culgt.culgt_or_sweeps(lat, links, n, omega)
+        sweeps(lat, links, n, omega)
         done += n
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(stream)
@@ -297,7 +314,8 @@ def main():
     clocks = sampler.stop()
     elapsed_ms = ev0.elapsed_time(ev1)
     check_ms = sum(a.elapsed_time(b) for a, b in check_events)
-    theta, F = (float(x) for x in scal.cpu())
+    res = scal.cpu()
+    theta, F = (float(res[:n3].max()), float(res[n3:].mean())) if coulomb else (float(res[0]), float(res[1]))
 
     elapsed_max_ms = max_over_ranks(elapsed_ms, world, "cuda")
     value = whole_job_value(world, V, args.steps, elapsed_max_ms * 1e-3)
@@ -313,17 +331,31 @@ def main():
     # ---- end to end through the host-buffer entry point
     e2e = None
     if not args.no_e2e:
-        culgt.culgt_fix_host(lat, host, can_dev, links, ws, 2, omega)       # warm the path
+        def host_job(n):
+            if not coulomb:
+                return culgt.culgt_fix_host(lat, host, can_dev, links, ws, n, omega)
+            # Coulomb: the same job assembled from the C-ABI calls (H2D, pack, sweeps, theta_t/F_t,
+            # unpack, D2H of the field and of the 2*N3 scalars)
+            can_dev.copy_(host, non_blocking=True)
+            culgt.culgt_pack(lat, can_dev, links)
+            sweeps(lat, links, n, omega)
+            check()
+            culgt.culgt_unpack(lat, links, can_dev)
+            host.copy_(can_dev, non_blocking=True)
+            r = scal.cpu()
+            return float(r[:n3].max()), float(r[n3:].mean())
+
+        host_job(2)                                                         # warm the path
         barrier()
         t0 = time.perf_counter()
-        th_e, F_e = culgt.culgt_fix_host(lat, host, can_dev, links, ws, args.steps, omega)
+        th_e, F_e = host_job(args.steps)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         dt_max = max_over_ranks(dt, world, "cuda")
         cbytes = culgt.culgt_canonical_bytes(lat)
         e2e = {"value": whole_job_value(world, V, args.steps, dt_max), "unit": UNIT,
                "h2d_bytes_per_step": cbytes / args.steps, "d2h_bytes_per_step": (cbytes + 16) / args.steps,
-               "job": f"one culgt_fix_host call = H2D {cbytes} B + pack + {args.steps} sweeps + theta,F + unpack + D2H {cbytes} B",
+               "job": f"one {'culgt_fix_host call' if not coulomb else 'host job (pack, sweeps, theta_t/F_t, unpack)'} = H2D {cbytes} B + pack + {args.steps} sweeps + theta,F + unpack + D2H {cbytes} B",
                "theta": th_e, "F": F_e}
 
     # ---- CPU baseline: the oracle on this host's cores (rank 0, N=1 only)
@@ -336,8 +368,8 @@ def main():
             u0 = li.round_to_fp32(u0)
         ur = li.to_real(u0)
         del u0
-        v_all, n_all = time_oracle(dims, cfg["group"], ur, omega, 40, 12.0, threads)
-        v_one, n_one = time_oracle(dims, cfg["group"], ur, omega, 3, 6.0, 1)
+        v_all, n_all = time_oracle(dims, cfg["group"], ur, omega, 40, 12.0, threads, args.gauge)
+        v_one, n_one = time_oracle(dims, cfg["group"], ur, omega, 3, 6.0, 1, args.gauge)
         cpu = {"value": v_all, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": f"{n_all} full sweeps of the same {'x'.join(map(str, dims))} lattice on {threads} threads "
                          f"(fp64, canonical layout); one core: {v_one:.4g} site-updates/s over {n_one} sweep(s)",
@@ -350,7 +382,7 @@ def main():
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if cfg["precision"] == 32 else "f64", "data": "synthetic",
             "config": workload_config(args, cfg),
-            "gflops": value * flops_per_site(cfg) / 1e9,
+            "gflops": value * flops_per_site(cfg, args.gauge) / 1e9,
             "algorithmic_gbs": value * 16 * (cfg["params"] * cfg["precision"] // 8) / 1e9,
             "gpu_launches": gpu_launches,
             "e2e": e2e,

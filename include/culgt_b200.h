@@ -126,6 +126,26 @@ int culgt_fix_host(const culgt_lattice* lat, void* canonical_host, void* canonic
                    void* links_dev, void* workspace, int n_sweeps, double omega,
                    double* theta_out, double* F_out, void* stream);
 
+/* ---- Coulomb gauge (named by the paper, P:L7; reading C-22): the same update
+ * with mu restricted to the 3 spatial directions, time-slice by time-slice:
+ *   K_C(x) = sum_{i<3} [ U_i(x) + U_i(x-i)^dagger ],  G from K_C as above,
+ *   U_mu(x) <- G U_mu(x),  U_mu(x-mu) <- U_mu(x-mu) G^dagger  for ALL 4 mu (a gauge transformation
+ *   acts on every link touching x, time links included).
+ *   F_t = 1/(3 Nc Vs) sum_{x in slice t} sum_{i<3} Re tr U_i(x),
+ *   theta_t = 1/(Nc Vs) sum_{x in slice t} tr[Delta_C Delta_C^dagger],  Delta_C = sum_{i<3} A_i(x) - A_i(x-i),
+ *   t = x3 = 0..N3-1, Vs = N0*N1*N2.
+ * culgt_or_sweep_coulomb / culgt_or_sweeps_coulomb: as the Landau calls.
+ * culgt_coulomb_precision_functional: theta_t_dev, F_t_dev are DEVICE arrays of dims[3] doubles.
+ * culgt_coulomb_fix: full sweeps until max_t theta_t < theta_target or max_sweeps; SYNCHRONISES at
+ *   each check; theta_t_out / F_t_out: HOST arrays of dims[3] doubles (may be NULL). */
+int culgt_or_sweep_coulomb(const culgt_lattice* lat, void* links, int parity, double omega, void* stream);
+int culgt_or_sweeps_coulomb(const culgt_lattice* lat, void* links, int n_sweeps, double omega, void* stream);
+int culgt_coulomb_precision_functional(const culgt_lattice* lat, const void* links, void* workspace,
+                                       double* theta_t_dev, double* F_t_dev, void* stream);
+int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, double omega,
+                      double theta_target, int max_sweeps, int check_every, int* sweeps_done,
+                      double* theta_t_out, double* F_t_out, void* stream);
+
 /* Kernel-variant selection for measurement: variant 0 = the default chosen
  * by measurement; other values select alternative thread-to-site mappings where provided.
  * Returns CULGT_OK or CULGT_ERR_ARG.  Process-global; not thread-safe. */

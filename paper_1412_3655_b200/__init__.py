@@ -70,6 +70,11 @@ def lib() -> ctypes.CDLL:
     L.culgt_landau_fix.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                    ctypes.c_int, ctypes.POINTER(ctypes.c_int), dp, dp, vp]
     L.culgt_fix_host.argtypes = [latp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_double, dp, dp, vp]
+    L.culgt_or_sweep_coulomb.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
+    L.culgt_or_sweeps_coulomb.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
+    L.culgt_coulomb_precision_functional.argtypes = [latp, vp, vp, vp, vp, vp]
+    L.culgt_coulomb_fix.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
+                                    ctypes.POINTER(ctypes.c_int), dp, dp, vp]
     L.culgt_set_sweep_variant.argtypes = [ctypes.c_int]
     L.culgt_strerror.argtypes = [ctypes.c_int]
     L.culgt_strerror.restype = ctypes.c_char_p
@@ -246,6 +251,42 @@ def culgt_fix_host(lat: Lattice, canonical_host, canonical_dev, links_dev, works
                                 _ptr(links_dev), _ptr(workspace), int(n_sweeps), float(omega),
                                 ctypes.byref(theta), ctypes.byref(F), _stream(stream)), "culgt_fix_host")
     return theta.value, F.value
+
+
+# ---- Coulomb gauge (reading C-22) ----------------------------------------------------
+
+def culgt_or_sweep_coulomb(lat: Lattice, links, parity: int, omega: float, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_or_sweep_coulomb(ctypes.byref(lat.c()), _ptr(links), int(parity), float(omega),
+                                        _stream(stream)), "culgt_or_sweep_coulomb")
+
+
+def culgt_or_sweeps_coulomb(lat: Lattice, links, n_sweeps: int, omega: float, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_or_sweeps_coulomb(ctypes.byref(lat.c()), _ptr(links), int(n_sweeps), float(omega),
+                                         _stream(stream)), "culgt_or_sweeps_coulomb")
+
+
+def culgt_coulomb_precision_functional(lat: Lattice, links, workspace, theta_t_dev, F_t_dev, stream=None) -> None:
+    """theta_t_dev, F_t_dev: device float64 arrays of dims[3] elements."""
+    _require_cuda()
+    _check(lib().culgt_coulomb_precision_functional(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace),
+                                                    _ptr(theta_t_dev), _ptr(F_t_dev), _stream(stream)),
+           "culgt_coulomb_precision_functional")
+
+
+def culgt_coulomb_fix(lat: Lattice, links, workspace, omega: float, theta_target: float,
+                      max_sweeps: int, check_every: int = 1, stream=None):
+    """Returns (sweeps_done, theta_t, F_t) with theta_t, F_t lists of dims[3] floats."""
+    _require_cuda()
+    n3 = int(lat.dims[3])
+    done = ctypes.c_int(0)
+    th = (ctypes.c_double * n3)()
+    F = (ctypes.c_double * n3)()
+    _check(lib().culgt_coulomb_fix(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace), float(omega),
+                                   float(theta_target), int(max_sweeps), int(check_every),
+                                   ctypes.byref(done), th, F, _stream(stream)), "culgt_coulomb_fix")
+    return done.value, list(th), list(F)
 
 
 def culgt_set_sweep_variant(variant: int) -> None:

@@ -2,6 +2,7 @@
 // codes and dispatch to the kernel launchers.  No compute happens here.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 #include "../../include/culgt_b200.h"
 #include "kernels.h"
@@ -70,7 +71,7 @@ size_t culgt_gfield_bytes(const culgt_lattice* lat) {
 size_t culgt_workspace_bytes(const culgt_lattice* lat) {
   LatticeDesc d;
   if (describe(lat, &d) != CULGT_OK) return 0;
-  return reduce_workspace_doubles(d.geom.vh) * sizeof(double);   // block partials + {theta, F} scalars
+  return reduce_workspace_doubles(d.geom) * sizeof(double);   // block partials + 2 * N3 result slots
 }
 
 int culgt_pack(const culgt_lattice* lat, const void* canonical, void* links, void* stream) {
@@ -134,7 +135,7 @@ int culgt_gauge_precision(const culgt_lattice* lat, const void* links, void* wor
   if (!links || !workspace || !theta_dev) return CULGT_ERR_NULL;
   if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
   // one fused pass computes both scalars; F goes to the spare slot at the end of the workspace
-  double* spare = (double*)workspace + reduce_workspace_doubles(d.geom.vh) - 1;
+  double* spare = (double*)workspace + reduce_partial_doubles(d.geom) + 1;
   cudaError_t e = launch_theta_functional(d, links, (double*)workspace, theta_dev, spare, (cudaStream_t)stream);
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
@@ -146,7 +147,7 @@ int culgt_functional(const culgt_lattice* lat, const void* links, void* workspac
   if (rc != CULGT_OK) return rc;
   if (!links || !workspace || !F_dev) return CULGT_ERR_NULL;
   if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
-  double* spare = (double*)workspace + reduce_workspace_doubles(d.geom.vh) - 2;
+  double* spare = (double*)workspace + reduce_partial_doubles(d.geom);
   cudaError_t e = launch_theta_functional(d, links, (double*)workspace, spare, F_dev, (cudaStream_t)stream);
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
@@ -172,11 +173,11 @@ int culgt_gauge_precision_functional(const culgt_lattice* lat, const void* links
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
-// theta and F (one fused pass) into the two doubles at the end of the workspace, read back.
+// theta and F (one fused pass) into the first two result slots of the workspace, read back.
 static int read_theta_F(const LatticeDesc& d, const void* links, void* workspace, cudaStream_t st,
                         double* theta, double* F) {
   double* ws = (double*)workspace;
-  double* scal = ws + reduce_workspace_doubles(d.geom.vh) - 2;
+  double* scal = ws + reduce_partial_doubles(d.geom);
   cudaError_t e = launch_theta_functional(d, links, ws, scal, scal + 1, st);
   if (e != cudaSuccess) return cuda_fail(e);
   double host[2] = {0, 0};
@@ -246,6 +247,108 @@ int culgt_fix_host(const culgt_lattice* lat, void* canonical_host, void* canonic
   if ((rc = read_theta_F(d, links_dev, workspace, st, &theta, &F)) != CULGT_OK) return rc;
   if (theta_out) *theta_out = theta;
   if (F_out) *F_out = F;
+  return CULGT_OK;
+}
+
+// ---- Coulomb gauge (reading C-22) -----------------------------------------------------
+
+int culgt_or_sweep_coulomb(const culgt_lattice* lat, void* links, int parity, double omega, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (parity != 0 && parity != 1) return CULGT_ERR_PARITY;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  cudaError_t e = launch_or_sweep(d, links, parity, omega, 0, (cudaStream_t)stream, true);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_or_sweeps_coulomb(const culgt_lattice* lat, void* links, int n_sweeps, double omega, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (n_sweeps < 0) return CULGT_ERR_ARG;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  for (int i = 0; i < n_sweeps; ++i)
+    for (int parity = 0; parity < 2; ++parity) {
+      cudaError_t e = launch_or_sweep(d, links, parity, omega, 0, (cudaStream_t)stream, true);
+      if (e != cudaSuccess) return cuda_fail(e);
+    }
+  return CULGT_OK;
+}
+
+int culgt_coulomb_precision_functional(const culgt_lattice* lat, const void* links, void* workspace,
+                                       double* theta_t_dev, double* F_t_dev, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !workspace || !theta_t_dev || !F_t_dev) return CULGT_ERR_NULL;
+  if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_coulomb_theta_functional(d, links, (double*)workspace, theta_t_dev, F_t_dev,
+                                                  (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+// max_t theta_t and mean_t F_t through the result slots of the workspace (synchronises).
+static int read_coulomb(const LatticeDesc& d, const void* links, void* workspace, cudaStream_t st,
+                        double* theta_max, double* F_mean, double* theta_t_host, double* F_t_host) {
+  const int n3 = d.geom.n[3];
+  double* ws = (double*)workspace;
+  double* res = ws + reduce_partial_doubles(d.geom);
+  cudaError_t e = launch_coulomb_theta_functional(d, links, ws, res, res + n3, st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  double stack_buf[512];
+  double* host = (2 * n3 <= 512) ? stack_buf : (double*)malloc(2 * (size_t)n3 * sizeof(double));
+  if (!host) return CULGT_ERR_ARG;
+  e = cudaMemcpyAsync(host, res, 2 * (size_t)n3 * sizeof(double), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  int rc = CULGT_OK;
+  if (e != cudaSuccess) {
+    rc = cuda_fail(e);
+  } else {
+    double tmax = 0, fsum = 0;
+    for (int t = 0; t < n3; ++t) {
+      if (host[t] > tmax || host[t] != host[t]) tmax = host[t];
+      fsum += host[n3 + t];
+      if (theta_t_host) theta_t_host[t] = host[t];
+      if (F_t_host) F_t_host[t] = host[n3 + t];
+    }
+    *theta_max = tmax;
+    *F_mean = fsum / n3;
+  }
+  if (host != stack_buf) free(host);
+  return rc;
+}
+
+int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, double omega,
+                      double theta_target, int max_sweeps, int check_every, int* sweeps_done,
+                      double* theta_t_out, double* F_t_out, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !workspace) return CULGT_ERR_NULL;
+  if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
+  if (max_sweeps < 0 || check_every < 1) return CULGT_ERR_ARG;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  double tmax = 0, fmean = 0;
+  int done = 0;
+  if ((rc = read_coulomb(d, links, workspace, st, &tmax, &fmean, theta_t_out, F_t_out)) != CULGT_OK) return rc;
+  while (tmax >= theta_target && done < max_sweeps) {
+    int n = check_every;
+    if (done + n > max_sweeps) n = max_sweeps - done;
+    for (int i = 0; i < n; ++i)
+      for (int parity = 0; parity < 2; ++parity) {
+        cudaError_t e = launch_or_sweep(d, links, parity, omega, 0, st, true);
+        if (e != cudaSuccess) return cuda_fail(e);
+      }
+    done += n;
+    if ((rc = read_coulomb(d, links, workspace, st, &tmax, &fmean, theta_t_out, F_t_out)) != CULGT_OK) return rc;
+  }
+  if (sweeps_done) *sweeps_done = done;
   return CULGT_OK;
 }
 

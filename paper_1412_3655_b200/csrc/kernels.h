@@ -16,21 +16,30 @@ struct LatticeDesc {
 constexpr int kReduceBlock = 256;       // threads per block of the reduction kernels
 // CTAs (= partials per quantity) of the fused theta+F kernel: 128 sites of each parity per CTA
 inline int reduce_blocks_fused(int vh) { return (vh + 127) / 128; }
-// doubles in the reduction workspace: partials + the two scalars the *_host paths read back
-inline size_t reduce_workspace_doubles(int vh) {
-  const size_t fused = 2 * (size_t)reduce_blocks_fused(vh);
-  return (fused > 4096 ? fused : 4096) + 2;   // never below 32 KiB
+// doubles in the reduction workspace: block partials (Landau: 2 * vh/128; Coulomb: 2 * N3 *
+// slice/128; never below 4096) followed by 2 * N3 result slots that the *_host / *_fix paths
+// read back (Landau uses the first two).
+inline size_t reduce_partial_doubles(const Geom& g) {
+  size_t n = 2 * (size_t)reduce_blocks_fused(g.vh);
+  const size_t c = 2 * (size_t)g.n[3] * (size_t)reduce_blocks_fused(g.stride[3]);
+  if (c > n) n = c;
+  return n > 4096 ? n : 4096;
 }
+inline size_t reduce_workspace_doubles(const Geom& g) { return reduce_partial_doubles(g) + 2 * (size_t)g.n[3]; }
 
+// coulomb = true: Coulomb-gauge half-sweep (K from the spatial links; production mapping only)
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
-                            int variant, cudaStream_t st);
+                            int variant, cudaStream_t st, bool coulomb = false);
 cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
-                                   int variant, cudaStream_t st);
+                                   int variant, bool coulomb, cudaStream_t st);
 cudaError_t launch_pack(const LatticeDesc& d, const void* canonical, void* links, cudaStream_t st);
 cudaError_t launch_unpack(const LatticeDesc& d, const void* links, void* canonical, cudaStream_t st);
 // fused theta + F; workspace holds 2 * reduce_blocks_fused(vh) partials
 cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
                                     double* out_theta, double* out_F, cudaStream_t st);
+// Coulomb gauge: per-slice theta_t, F_t (N3 doubles each)
+cudaError_t launch_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
+                                            double* out_theta_t, double* out_F_t, cudaStream_t st);
 cudaError_t launch_gauge_transform(const LatticeDesc& d, void* links, const void* g, cudaStream_t st);
 
 }  // namespace culgt

@@ -92,7 +92,7 @@ or_sweep_su3_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
 // for SU(3), reading C-15); the 8 quaternion products in the storage precision.  Odd-parity
 // launches walk the site blocks in descending order (L2 carry-over, as the SU(3) kernel).
 // ---------------------------------------------------------------------------------------------
-template <typename S, int BLOCK>
+template <typename S, int BLOCK, bool COULOMB>
 __global__ void __launch_bounds__(BLOCK)
 or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
                     const double omega, const int reverse) {
@@ -113,7 +113,7 @@ or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
   // K = k0 + i k.sigma = sum_mu u_up + conj(u_dn)
   double k[4] = {0, 0, 0, 0};
 #pragma unroll
-  for (int mu = 0; mu < 4; ++mu) {
+  for (int mu = 0; mu < (COULOMB ? 3 : 4); ++mu) {     // Coulomb gauge: spatial links only (C-22)
     k[0] += (double)U[2 * mu][0] + (double)U[2 * mu + 1][0];
 #pragma unroll
     for (int i = 1; i < 4; ++i) k[i] += (double)U[2 * mu][i] - (double)U[2 * mu + 1][i];
@@ -144,26 +144,28 @@ static cudaError_t launch_su3(void* links, const Geom& g, int parity, double ome
 }
 
 template <typename S>
-static cudaError_t launch_su2(void* links, const Geom& g, int parity, double omega, cudaStream_t st) {
+static cudaError_t launch_su2(void* links, const Geom& g, int parity, double omega, bool coulomb, cudaStream_t st) {
   constexpr int BLOCK = 128;
   const unsigned grid = (unsigned)((g.vh + BLOCK - 1) / BLOCK);
-  or_sweep_su2_kernel<S, BLOCK><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g, parity, omega, parity);
+  if (coulomb) or_sweep_su2_kernel<S, BLOCK, true><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g, parity, omega, parity);
+  else or_sweep_su2_kernel<S, BLOCK, false><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g, parity, omega, parity);
   return cudaGetLastError();
 }
 
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
-                            int variant, cudaStream_t st) {
+                            int variant, cudaStream_t st, bool coulomb) {
   const Geom& g = d.geom;
   if (d.group == 2) {
-    if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, g, parity, omega, st);
-    return launch_su2<Storage<double, 2, 4> >(links, g, parity, omega, st);
+    if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, g, parity, omega, coulomb, st);
+    return launch_su2<Storage<double, 2, 4> >(links, g, parity, omega, coulomb, st);
   }
   // variant 0 = the production mapping (or_sweep_staged.cu); 20+ select staged mappings
   if (variant == 0) {
     const int best = 20;   // the production mapping of each storage format (or_sweep_staged.cu)
-    return launch_or_sweep_staged(d, links, parity, omega, best, st);
+    return launch_or_sweep_staged(d, links, parity, omega, best, coulomb, st);
   }
-  if (variant >= 20) return launch_or_sweep_staged(d, links, parity, omega, variant, st);
+  if (coulomb) return cudaErrorInvalidValue;   // Coulomb gauge: production mapping (variant 0) only
+  if (variant >= 20) return launch_or_sweep_staged(d, links, parity, omega, variant, false, st);
   if (d.precision == 32) {
     // fp32 storage: K and the subgroup solve in fp64 (reading C-15); variants 10+ are
     // all-fp32 arithmetic, kept for the precision/throughput comparison in profiles/.

@@ -36,6 +36,7 @@ constexpr int OPT_CHUNKED = 4;     // persistent only: contiguous chunk of site 
 constexpr int OPT_NOMATH = 8;      // measurement only: G = 1 (memory pattern + products, no K / solve)
 constexpr int OPT_FLAT = 16;       // one CTA per site block (hardware block scheduler), not persistent
 constexpr int OPT_STREAM_ST = 32;  // st.global.cs stores
+constexpr int OPT_COULOMB = 64;    // Coulomb gauge (reading C-22): K(x) from the 6 spatial links only
 
 __device__ __forceinline__ void cp_async_vec(float4* smem, const float4* gmem) {
   const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -212,6 +213,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
     for (int i = 0; i < 18; ++i) K[i] = 0;
 #pragma unroll
     for (int l = 0; l < LPT; ++l) {
+      if ((OPT & OPT_COULOMB) && ((q * LPT + l) >> 1) == 3) continue;   // time links do not enter K_C
       Real U[18];
       asm volatile("" ::: "memory");   // keep the shared-memory reads of link l behind link l-1's use
       load_link(stage, l, U, std::false_type());
@@ -326,9 +328,19 @@ static cudaError_t launch_staged(void* links, const Geom& g, int parity, double 
 // (culgt_set_sweep_variant) and parity-tested.  "AxB" = A threads per CTA, B CTAs per SM;
 // "flat" = one CTA per site block, "pers" = persistent grid-stride loop; tps = threads per site.
 cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
-                                   int variant, cudaStream_t st) {
+                                   int variant, bool coulomb, cudaStream_t st) {
   const Geom& g = d.geom;
   if (d.group != 3) return cudaErrorInvalidValue;
+  if (coulomb) {   // Coulomb gauge: the production mapping of each format with K from spatial links
+    if (variant != 20) return cudaErrorInvalidValue;
+    if (d.precision == 32 && d.params == 12)
+      return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
+    if (d.precision == 32)
+      return launch_staged<Storage<float, 3, 18>, double, 2, 256, 1, 2, OPT_COULOMB>(links, g, parity, omega, true, st);
+    if (d.params == 12)
+      return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
+    return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
+  }
   if (d.precision == 32 && d.params == 12) {
     typedef Storage<float, 3, 12> S;
     switch (variant) {

@@ -57,23 +57,31 @@ __device__ __forceinline__ double theta_from_K(const double* K) {
 // CTA the second read comes from L1/L2 instead of HBM (mu = 0: same CTA; mu = 1,2: a few CTAs
 // away; mu = 3: one time-slice of CTAs away, far below the L2 size).  F = sum of Re tr over the
 // 4 up links of every site of both parities = every link exactly once.
-template <typename S, int BLOCK>
+//
+// COULOMB = true (reading C-22): mu runs over the 3 spatial directions only and the sums are kept
+// per time-slice: blockIdx.y = t, the CTA's sites are the BLOCK/2 sites [bx*BLOCK/2, ...) of each
+// parity INSIDE slice t (a slice is the contiguous index range [t*stride3, (t+1)*stride3) of each
+// parity's sublattice), partials are laid out [t][bx].
+template <typename S, int BLOCK, bool COULOMB>
 __global__ void __launch_bounds__(BLOCK)
 theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
                         double* __restrict__ partial_theta, double* __restrict__ partial_F) {
   typedef typename S::Real Real;
   constexpr int HALF = BLOCK / 2;
+  constexpr int ND = COULOMB ? 3 : 4;
   const int parity = threadIdx.x >= HALF;
-  const int h = blockIdx.x * HALF + (int)threadIdx.x - parity * HALF;
+  const int in_group = blockIdx.x * HALF + (int)threadIdx.x - parity * HALF;   // index inside the slice / lattice
+  const int group_size = COULOMB ? g.stride[3] : g.vh;
+  const int h = COULOMB ? (int)blockIdx.y * g.stride[3] + in_group : in_group;
   double th = 0, f = 0;
-  if (h < g.vh) {
+  if (in_group < group_size) {
     const SiteCoord sc = decode_site(g, h, parity);
     if (S::NC == 3) {
       double K[18];
 #pragma unroll
       for (int i = 0; i < 18; ++i) K[i] = 0;
 #pragma unroll
-      for (int mu = 0; mu < 4; ++mu) {
+      for (int mu = 0; mu < ND; ++mu) {
         Real U[18];
         double Ud[18];                       // widened first: the third row is rebuilt in fp64
         load_params<S>(link_base<S>(links, g, parity, mu, h), g.vh, U);
@@ -92,7 +100,7 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
     } else {
       double d[3] = {0, 0, 0};
 #pragma unroll
-      for (int mu = 0; mu < 4; ++mu) {
+      for (int mu = 0; mu < ND; ++mu) {
         Real u[4], w[4];
         load_params<S>(link_base<S>(links, g, parity, mu, h), g.vh, u);
         load_params<S>(link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu)), g.vh, w);
@@ -107,23 +115,26 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
   __syncthreads();                       // block_sum's shared slots are reused
   const double sf = block_sum<BLOCK>(f);
   if (threadIdx.x == 0) {
-    partial_theta[blockIdx.x] = st;
-    partial_F[blockIdx.x] = sf;
+    const size_t slot = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
+    partial_theta[slot] = st;
+    partial_F[slot] = sf;
   }
 }
 
-// Sums of two partial arrays by two blocks (blockIdx 0: theta, 1: F), fixed order, scaled.
+// Final pass: block (group, quantity) sums the n partials of that group in a fixed order and
+// scales.  partial = [quantity][group][n]; quantity 0 = theta, 1 = F; group = time-slice for the
+// Coulomb sums, a single group for the Landau sums.
 template <int BLOCK>
 __global__ void __launch_bounds__(BLOCK)
-final_sum2_kernel(const double* __restrict__ partial, int n, double scale0, double scale1,
-                  double* __restrict__ out0, double* __restrict__ out1) {
-  const double* p = partial + (size_t)blockIdx.x * n;
+final_sum_kernel(const double* __restrict__ partial, int n, double scale0, double scale1,
+                 double* __restrict__ out0, double* __restrict__ out1) {
+  const double* p = partial + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * (size_t)n;
   double acc = 0;
   for (int i = threadIdx.x; i < n; i += BLOCK) acc += p[i];
   const double s = block_sum<BLOCK>(acc);
   if (threadIdx.x == 0) {
-    if (blockIdx.x == 0) *out0 = s * scale0;
-    else *out1 = s * scale1;
+    if (blockIdx.y == 0) out0[blockIdx.x] = s * scale0;
+    else out1[blockIdx.x] = s * scale1;
   }
 }
 
@@ -132,11 +143,29 @@ static cudaError_t run_theta_functional(const LatticeDesc& d, const void* links,
                                         double* out_F, cudaStream_t st) {
   constexpr int BLOCK = 256;
   const int nblk = reduce_blocks_fused(d.geom.vh);
-  theta_functional_kernel<S, BLOCK><<<nblk, BLOCK, 0, st>>>((const typename S::Vec*)links, d.geom, ws, ws + nblk);
+  theta_functional_kernel<S, BLOCK, false><<<nblk, BLOCK, 0, st>>>((const typename S::Vec*)links, d.geom, ws, ws + nblk);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  final_sum2_kernel<kReduceBlock><<<2, kReduceBlock, 0, st>>>(ws, nblk, 1.0 / ((double)S::NC * (double)d.V),
-                                                             1.0 / (4.0 * S::NC * (double)d.V), out_theta, out_F);
+  final_sum_kernel<kReduceBlock><<<dim3(1, 2), kReduceBlock, 0, st>>>(
+      ws, nblk, 1.0 / ((double)S::NC * (double)d.V), 1.0 / (4.0 * S::NC * (double)d.V), out_theta, out_F);
+  return cudaGetLastError();
+}
+
+// Coulomb gauge: theta_t and F_t for every time-slice t (arrays of N3 doubles).
+template <typename S>
+static cudaError_t run_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* ws,
+                                                double* out_theta_t, double* out_F_t, cudaStream_t st) {
+  constexpr int BLOCK = 256;
+  const int n3 = d.geom.n[3];
+  const int nbx = reduce_blocks_fused(d.geom.stride[3]);
+  const size_t per_quantity = (size_t)n3 * nbx;
+  theta_functional_kernel<S, BLOCK, true><<<dim3(nbx, n3), BLOCK, 0, st>>>((const typename S::Vec*)links, d.geom,
+                                                                           ws, ws + per_quantity);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const double vs = (double)d.V / (double)n3;
+  final_sum_kernel<kReduceBlock><<<dim3(n3, 2), kReduceBlock, 0, st>>>(
+      ws, nbx, 1.0 / ((double)S::NC * vs), 1.0 / (3.0 * S::NC * vs), out_theta_t, out_F_t);
   return cudaGetLastError();
 }
 
@@ -155,6 +184,11 @@ static cudaError_t run_theta_functional(const LatticeDesc& d, const void* links,
 cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
                                     double* out_theta, double* out_F, cudaStream_t st) {
   CULGT_DISPATCH(run_theta_functional, d, links, workspace, out_theta, out_F, st)
+}
+
+cudaError_t launch_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
+                                            double* out_theta_t, double* out_F_t, cudaStream_t st) {
+  CULGT_DISPATCH(run_coulomb_theta_functional, d, links, workspace, out_theta_t, out_F_t, st)
 }
 
 }  // namespace culgt
