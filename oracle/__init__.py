@@ -59,6 +59,7 @@ def _load():
     lib.oracle_plaquette.argtypes = [i32p, ctypes.c_int, dp]
     lib.oracle_plaquette.restype = ctypes.c_double
     lib.oracle_reconstruct12.argtypes = [ctypes.c_int64, dp]
+    lib.oracle_reunitarize.argtypes = [ctypes.c_int64, ctypes.c_int, dp]
     lib.oracle_K_coulomb.argtypes = [i32p, ctypes.c_int, dp, dp]
     lib.oracle_delta_coulomb.argtypes = [i32p, ctypes.c_int, dp, dp]
     lib.oracle_or_sweep_coulomb.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double]
@@ -206,3 +207,12 @@ def coulomb_theta_F(dims, u: np.ndarray):
     th, f = np.empty(n3), np.empty(n3)
     _load().oracle_coulomb_theta_F(_dims(dims), nc, _dp(u), _dp(th), _dp(f))
     return th, f
+
+
+def reunitarize(m: np.ndarray) -> None:
+    """In place: project every nc x nc matrix of real [...,nc,nc,2] back onto SU(nc) by Gram-Schmidt
+    on the first rows (reading C-23)."""
+    nc = m.shape[-2]
+    if m.shape[-3:] != (nc, nc, 2) or nc not in (2, 3):
+        raise ValueError("need [...,nc,nc,2] with nc = 2 or 3")
+    _load().oracle_reunitarize(int(m.size // (2 * nc * nc)), nc, _dp(m))

@@ -492,3 +492,45 @@ void oracle_coulomb_theta_F(const int32_t* dims, int nc, const double* U, double
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// Re-unitarisation (reading C-13/C-23; SURVEY.md 8(f) NEXT-2c).  Not part of the paper's
+// text: long fp32 runs let the stored rows drift off the group (C-13), and the projection back is
+// the Gram-Schmidt step the 12-parameter representation already implies (the third
+// row IS conj(row0 x row1)):  r0 <- r0/|r0|;  r1 <- r1 - <r0,r1> r0;  r1 <- r1/|r1|;
+// r2 <- conj(r0 x r1),  <a,b> = sum_k conj(a_k) b_k.   SU(2): (a0..a3) <- (a0..a3)/|a|, applied
+// to the first row of the 2x2 matrix and the second row rebuilt as (-conj(b), conj(a)).
+// ---------------------------------------------------------------------------------------------
+extern "C" {
+
+// n matrices, M = double[n][nc][nc][2], in place.
+void oracle_reunitarize(int64_t n, int nc, double* M) {
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t k = 0; k < n; ++k) {
+    Mat m = load_mat(M + k * nc * nc * 2, nc);
+    if (nc == 2) {
+      double nrm = std::sqrt(std::norm(m.e[0][0]) + std::norm(m.e[0][1]));
+      cd a = m.e[0][0] / nrm, b = m.e[0][1] / nrm;
+      m.e[0][0] = a;  m.e[0][1] = b;
+      m.e[1][0] = -std::conj(b);  m.e[1][1] = std::conj(a);
+    } else {
+      double n0 = 0.0;
+      for (int c = 0; c < 3; ++c) n0 += std::norm(m.e[0][c]);
+      n0 = std::sqrt(n0);
+      for (int c = 0; c < 3; ++c) m.e[0][c] /= n0;
+      cd ip(0.0, 0.0);
+      for (int c = 0; c < 3; ++c) ip += std::conj(m.e[0][c]) * m.e[1][c];
+      for (int c = 0; c < 3; ++c) m.e[1][c] -= ip * m.e[0][c];
+      double n1 = 0.0;
+      for (int c = 0; c < 3; ++c) n1 += std::norm(m.e[1][c]);
+      n1 = std::sqrt(n1);
+      for (int c = 0; c < 3; ++c) m.e[1][c] /= n1;
+      m.e[2][0] = std::conj(m.e[0][1] * m.e[1][2] - m.e[0][2] * m.e[1][1]);
+      m.e[2][1] = std::conj(m.e[0][2] * m.e[1][0] - m.e[0][0] * m.e[1][2]);
+      m.e[2][2] = std::conj(m.e[0][0] * m.e[1][1] - m.e[0][1] * m.e[1][0]);
+    }
+    store_mat(M + k * nc * nc * 2, nc, m);
+  }
+}
+
+}  // extern "C"
