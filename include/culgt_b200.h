@@ -76,6 +76,12 @@ int culgt_validate(const culgt_lattice* lat);
 int culgt_pack(const culgt_lattice* lat, const void* canonical, void* links, void* stream);
 int culgt_unpack(const culgt_lattice* lat, const void* links, void* canonical, void* stream);
 
+/* Re-unitarisation (reading C-23; not in the paper's text): projects every stored link
+ * back onto the group by Gram-Schmidt on its stored rows (r0 <- r0/|r0|, r1 <- r1 - <r0,r1> r0,
+ * r1 <- r1/|r1|; 18-parameter: r2 <- conj(r0 x r1); SU(2): quaternion normalisation), in fp64,
+ * in place.  For long fp32 runs, whose stored rows drift slowly off SU(3) (C-13).  Asynchronous. */
+int culgt_reunitarize(const culgt_lattice* lat, void* links, void* stream);
+
 /* a1-a6: ONE HALF sweep of overrelaxation over all sites x of `parity`, in place:
  *   K(x) = sum_mu [ U_mu(x) + U_mu(x-mu)^dagger ]                         eq. (3)
  *   SU(2): g = K^dagger/sqrt(det K^dagger), G = g^omega

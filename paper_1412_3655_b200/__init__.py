@@ -61,6 +61,7 @@ def lib() -> ctypes.CDLL:
     L.culgt_validate.argtypes = [latp]
     L.culgt_pack.argtypes = [latp, vp, vp, vp]
     L.culgt_unpack.argtypes = [latp, vp, vp, vp]
+    L.culgt_reunitarize.argtypes = [latp, vp, vp]
     L.culgt_or_sweep.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_or_sweeps.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_gauge_precision.argtypes = [latp, vp, vp, vp, vp]
@@ -188,6 +189,11 @@ def culgt_pack(lat: Lattice, canonical, links, stream=None) -> None:
 def culgt_unpack(lat: Lattice, links, canonical, stream=None) -> None:
     _require_cuda()
     _check(lib().culgt_unpack(ctypes.byref(lat.c()), _ptr(links), _ptr(canonical), _stream(stream)), "culgt_unpack")
+
+
+def culgt_reunitarize(lat: Lattice, links, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_reunitarize(ctypes.byref(lat.c()), _ptr(links), _stream(stream)), "culgt_reunitarize")
 
 
 def culgt_or_sweep(lat: Lattice, links, parity: int, omega: float, stream=None) -> None:

@@ -94,6 +94,16 @@ int culgt_unpack(const culgt_lattice* lat, const void* links, void* canonical, v
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
+int culgt_reunitarize(const culgt_lattice* lat, void* links, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_reunitarize(d, links, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
 static int check_omega(double omega) {
   if (!(omega >= 1.0 && omega < 2.0)) return CULGT_ERR_OMEGA;   // NaN fails the comparison
   return CULGT_OK;

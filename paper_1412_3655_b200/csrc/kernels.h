@@ -33,6 +33,7 @@ cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, doubl
 cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
                                    int variant, bool coulomb, cudaStream_t st);
 cudaError_t launch_pack(const LatticeDesc& d, const void* canonical, void* links, cudaStream_t st);
+cudaError_t launch_reunitarize(const LatticeDesc& d, void* links, cudaStream_t st);
 cudaError_t launch_unpack(const LatticeDesc& d, const void* links, void* canonical, cudaStream_t st);
 // fused theta + F; workspace holds 2 * reduce_blocks_fused(vh) partials
 cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, double* workspace,

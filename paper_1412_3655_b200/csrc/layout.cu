@@ -74,6 +74,84 @@ static cudaError_t dispatch_layout(const LatticeDesc& d, void* canonical, void* 
   return launch_layout<Storage<double, 3, 18>, PACK>(canonical, links, g, st);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Re-unitarisation (reading C-23): Gram-Schmidt on the stored rows of every link, in
+// fp64, rounded once to the storage precision.  One thread per (parity, mu, h) link.
+//   r0 <- r0/|r0|;  r1 <- r1 - <r0,r1> r0;  r1 <- r1/|r1|;  (18-parameter: r2 <- conj(r0 x r1));
+//   SU(2): (a0..a3) <- (a0..a3)/|a|.
+// ---------------------------------------------------------------------------------------------
+template <typename S, int BLOCK>
+__global__ void __launch_bounds__(BLOCK)
+reunitarize_kernel(typename S::Vec* __restrict__ links, const Geom g) {
+  typedef typename S::Real Real;
+  const long long t = (long long)blockIdx.x * BLOCK + threadIdx.x;     // (parity*4 + mu)*vh + h
+  if (t >= 8ll * g.vh) return;
+  const int pm = (int)(t / g.vh);
+  const int h = (int)(t - (long long)pm * g.vh);
+  typename S::Vec* p = links + ((size_t)pm * S::NV) * (size_t)g.vh + (size_t)h;
+  Real r[S::NP];
+  load_params<S>(p, g.vh, r);
+  if (S::NC == 2) {
+    double a[4] = {(double)r[0], (double)r[1], (double)r[2], (double)r[3]};
+    const double inv = 1.0 / sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2] + a[3] * a[3]);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) r[i] = (Real)(a[i] * inv);
+  } else {
+    double m[18];
+#pragma unroll
+    for (int i = 0; i < 12; ++i) m[i] = (double)r[i];
+    double n0 = 0;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) n0 += m[i] * m[i];
+    const double i0 = 1.0 / sqrt(n0);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) m[i] *= i0;
+    double ipr = 0, ipi = 0;                       // <r0, r1> = sum conj(r0_k) r1_k
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      ipr += m[CULGT_RE(0, c)] * m[CULGT_RE(1, c)] + m[CULGT_IM(0, c)] * m[CULGT_IM(1, c)];
+      ipi += m[CULGT_RE(0, c)] * m[CULGT_IM(1, c)] - m[CULGT_IM(0, c)] * m[CULGT_RE(1, c)];
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      m[CULGT_RE(1, c)] -= ipr * m[CULGT_RE(0, c)] - ipi * m[CULGT_IM(0, c)];
+      m[CULGT_IM(1, c)] -= ipr * m[CULGT_IM(0, c)] + ipi * m[CULGT_RE(0, c)];
+    }
+    double n1 = 0;
+#pragma unroll
+    for (int i = 6; i < 12; ++i) n1 += m[i] * m[i];
+    const double i1 = 1.0 / sqrt(n1);
+#pragma unroll
+    for (int i = 6; i < 12; ++i) m[i] *= i1;
+    if (S::NP == 18) reconstruct_row2(m);
+#pragma unroll
+    for (int i = 0; i < S::NP; ++i) r[i] = (Real)m[i];
+  }
+  store_params<S>(p, g.vh, r);
+}
+
+template <typename S>
+static cudaError_t run_reunitarize(void* links, const Geom& g, cudaStream_t st) {
+  constexpr int BLOCK = 256;
+  const unsigned grid = (unsigned)((8ll * g.vh + BLOCK - 1) / BLOCK);
+  reunitarize_kernel<S, BLOCK><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_reunitarize(const LatticeDesc& d, void* links, cudaStream_t st) {
+  const Geom& g = d.geom;
+  if (d.group == 2) {
+    if (d.precision == 32) return run_reunitarize<Storage<float, 2, 4> >(links, g, st);
+    return run_reunitarize<Storage<double, 2, 4> >(links, g, st);
+  }
+  if (d.precision == 32) {
+    if (d.params == 12) return run_reunitarize<Storage<float, 3, 12> >(links, g, st);
+    return run_reunitarize<Storage<float, 3, 18> >(links, g, st);
+  }
+  if (d.params == 12) return run_reunitarize<Storage<double, 3, 12> >(links, g, st);
+  return run_reunitarize<Storage<double, 3, 18> >(links, g, st);
+}
+
 cudaError_t launch_pack(const LatticeDesc& d, const void* canonical, void* links, cudaStream_t st) {
   return dispatch_layout<true>(d, const_cast<void*>(canonical), links, st);
 }
