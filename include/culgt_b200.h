@@ -156,6 +156,14 @@ int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, do
  * by measurement; other values select alternative thread-to-site mappings where provided.
  * Returns CULGT_OK or CULGT_ERR_ARG.  Process-global; not thread-safe. */
 int culgt_set_sweep_variant(int variant);
+
+/* Run-time autotuner (the paper's per-GPU selection of the fastest set-up, P:L89 (d)):
+ * times every result-equivalent sweep mapping built for this storage format with
+ * `sweeps_per_trial` REAL full sweeps each on `links` (the field is gauge-fixed further by them),
+ * makes the fastest the process-wide variant and reports it.  SYNCHRONISES.  best_variant,
+ * best_us_per_half_sweep: host pointers, may be NULL. */
+int culgt_autotune_sweep(const culgt_lattice* lat, void* links, double omega, int sweeps_per_trial,
+                         int* best_variant, float* best_us_per_half_sweep, void* stream);
 int culgt_get_sweep_variant(void);
 
 const char* culgt_strerror(int status);

@@ -257,6 +257,11 @@ CONFIGS = {
                         eps=0.0, scramble=False, omega=1.5, seed=1001),
     "su2_32_fp32": dict(dims=(32, 32, 32, 32), group=2, precision=32, params=4, kind="haar",
                         eps=0.0, scramble=False, omega=1.5, seed=1001),
+    # L2-resident SU(3) volumes (measurement only: the SM-side limit of the sweep kernel)
+    "l2_24_fp32": dict(dims=(24, 24, 24, 24), group=3, precision=32, params=12,
+                       kind="near_identity", eps=0.8, scramble=True, omega=1.7, seed=1003),
+    "l2_20_fp64": dict(dims=(20, 20, 20, 20), group=3, precision=64, params=18,
+                       kind="near_identity", eps=0.8, scramble=True, omega=1.7, seed=1003),
     "cfg4_fp32": dict(dims=(48, 48, 48, 96), group=3, precision=32, params=12, kind="haar",
                       eps=0.0, scramble=False, omega=1.7, seed=1004),
     "cfg4_fp64": dict(dims=(64, 64, 64, 64), group=3, precision=64, params=18, kind="haar",

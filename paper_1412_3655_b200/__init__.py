@@ -77,6 +77,8 @@ def lib() -> ctypes.CDLL:
     L.culgt_coulomb_fix.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
                                     ctypes.POINTER(ctypes.c_int), dp, dp, vp]
     L.culgt_set_sweep_variant.argtypes = [ctypes.c_int]
+    L.culgt_autotune_sweep.argtypes = [latp, vp, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int),
+                                       ctypes.POINTER(ctypes.c_float), vp]
     L.culgt_strerror.argtypes = [ctypes.c_int]
     L.culgt_strerror.restype = ctypes.c_char_p
     L.culgt_last_cuda_error.restype = ctypes.c_char_p
@@ -297,6 +299,17 @@ def culgt_coulomb_fix(lat: Lattice, links, workspace, omega: float, theta_target
 
 def culgt_set_sweep_variant(variant: int) -> None:
     _check(lib().culgt_set_sweep_variant(int(variant)), "culgt_set_sweep_variant")
+
+
+def culgt_autotune_sweep(lat: Lattice, links, omega: float, sweeps_per_trial: int = 3, stream=None):
+    """Times every result-equivalent sweep mapping on `links` (real sweeps), selects the fastest
+    process-wide.  Returns (variant, microseconds per half-sweep)."""
+    _require_cuda()
+    v = ctypes.c_int(0)
+    us = ctypes.c_float(0.0)
+    _check(lib().culgt_autotune_sweep(ctypes.byref(lat.c()), _ptr(links), float(omega), int(sweeps_per_trial),
+                                      ctypes.byref(v), ctypes.byref(us), _stream(stream)), "culgt_autotune_sweep")
+    return v.value, us.value
 
 
 def culgt_get_sweep_variant() -> int:

@@ -362,6 +362,51 @@ int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, do
   return CULGT_OK;
 }
 
+// Run-time autotuner (the paper's selection of the fastest kernel set-up per GPU at run time,
+// P:L89 (d)): times every result-equivalent sweep mapping built for this storage format
+// on the caller's field and makes the fastest one the process-wide choice.
+int culgt_autotune_sweep(const culgt_lattice* lat, void* links, double omega, int sweeps_per_trial,
+                         int* best_variant, float* best_us_per_half_sweep, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (sweeps_per_trial < 1) return CULGT_ERR_ARG;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return cuda_fail(cudaGetLastError());
+  int best = 0;
+  float best_us = -1.f;
+  for (int v = 0; v < 40; ++v) {
+    // 11, 14, 25: all-fp32 arithmetic (different precision); 28: measurement-only (no K / solve)
+    if (v == 11 || v == 14 || v == 25 || v == 28) continue;
+    if (d.group == 2 && v != 0) continue;
+    cudaError_t e = cudaSuccess;
+    for (int parity = 0; parity < 2 && e == cudaSuccess; ++parity) e = launch_or_sweep(d, links, parity, omega, v, st);
+    if (e == cudaErrorInvalidValue) continue;                     // mapping not built for this format
+    if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+    cudaEventRecord(e0, st);
+    for (int i = 0; i < sweeps_per_trial && e == cudaSuccess; ++i)
+      for (int parity = 0; parity < 2 && e == cudaSuccess; ++parity) e = launch_or_sweep(d, links, parity, omega, v, st);
+    cudaEventRecord(e1, st);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const float us = ms * 1e3f / (2.f * sweeps_per_trial);
+    if (best_us < 0.f || us < best_us) { best_us = us; best = v; }
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (rc != CULGT_OK) return rc;
+  g_variant = best;
+  if (best_variant) *best_variant = best;
+  if (best_us_per_half_sweep) *best_us_per_half_sweep = best_us;
+  return CULGT_OK;
+}
+
 int culgt_set_sweep_variant(int variant) {
   if (variant < 0 || variant > 99) return CULGT_ERR_ARG;
   g_variant = variant;

@@ -184,3 +184,23 @@ def test_sweep_is_asynchronous():
     ev.record()
     assert not ev.query()          # work still in flight when the calls have returned
     torch.cuda.synchronize()
+
+
+def test_autotuner_picks_a_result_equivalent_mapping():
+    """culgt_autotune_sweep (PAPER.md L89 (d), L134): returns one of the built mappings with a
+    positive time, leaves it selected, and sweeps with it still match the oracle."""
+    dims = (8, 8, 8, 8)
+    u = make(dims, 3, 47)
+    for precision, params in SU3_STORES:
+        scratch = GpuField(dims, 3, precision, params, u)
+        try:
+            v, us = culgt.culgt_autotune_sweep(scratch.lat, scratch.links, 1.7, 2)
+            assert v in variants_for(precision, params) + [20] and us > 0
+            assert culgt.culgt_get_sweep_variant() == v
+            ref = storage_input(u, precision, params)
+            oracle.full_sweep(dims, ref, 1.7)
+            f = GpuField(dims, 3, precision, params, u)
+            f.sweep(1.7)
+            assert np.abs(f.download() - li.from_real(ref)).max() < TOL_LINK[precision]
+        finally:
+            culgt.culgt_set_sweep_variant(0)
