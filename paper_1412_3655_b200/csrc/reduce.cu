@@ -80,21 +80,33 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
       double K[18];
 #pragma unroll
       for (int i = 0; i < 18; ++i) K[i] = 0;
+      // the loads of a batch of directions are issued before any of them is used (memory-level
+      // parallelism); fp32 storage batches 2 directions = 4 links, fp64 storage 1 direction
+      constexpr int MU_BATCH = (sizeof(Real) == 4) ? 2 : 1;
 #pragma unroll
-      for (int mu = 0; mu < ND; ++mu) {
-        Real U[18];
-        double Ud[18];                       // widened first: the third row is rebuilt in fp64
-        load_params<S>(link_base<S>(links, g, parity, mu, h), g.vh, U);
+      for (int mu0 = 0; mu0 < ND; mu0 += MU_BATCH) {
+        Real U[2 * MU_BATCH][S::NP];
 #pragma unroll
-        for (int i = 0; i < S::NP; ++i) Ud[i] = (double)U[i];
-        if (S::NP == 12) reconstruct_row2(Ud);
-        f += Ud[CULGT_RE(0, 0)] + Ud[CULGT_RE(1, 1)] + Ud[CULGT_RE(2, 2)];
-        accumulate(K, Ud, false);
-        load_params<S>(link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu)), g.vh, U);
+        for (int b = 0; b < MU_BATCH; ++b)
+          if (mu0 + b < ND) {
+            load_params<S>(link_base<S>(links, g, parity, mu0 + b, h), g.vh, U[2 * b]);
+            load_params<S>(link_base<S>(links, g, 1 - parity, mu0 + b, down_index(g, h, sc, mu0 + b)), g.vh,
+                           U[2 * b + 1]);
+          }
 #pragma unroll
-        for (int i = 0; i < S::NP; ++i) Ud[i] = (double)U[i];
-        if (S::NP == 12) reconstruct_row2(Ud);
-        accumulate(K, Ud, true);
+        for (int b = 0; b < MU_BATCH; ++b)
+          if (mu0 + b < ND) {
+            double Ud[18];                   // widened first: the third row is rebuilt in fp64
+#pragma unroll
+            for (int i = 0; i < S::NP; ++i) Ud[i] = (double)U[2 * b][i];
+            if (S::NP == 12) reconstruct_row2(Ud);
+            f += Ud[CULGT_RE(0, 0)] + Ud[CULGT_RE(1, 1)] + Ud[CULGT_RE(2, 2)];
+            accumulate(K, Ud, false);
+#pragma unroll
+            for (int i = 0; i < S::NP; ++i) Ud[i] = (double)U[2 * b + 1][i];
+            if (S::NP == 12) reconstruct_row2(Ud);
+            accumulate(K, Ud, true);
+          }
       }
       th = theta_from_K(K);
     } else {
