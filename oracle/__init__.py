@@ -60,6 +60,9 @@ def _load():
     lib.oracle_plaquette.restype = ctypes.c_double
     lib.oracle_reconstruct12.argtypes = [ctypes.c_int64, dp]
     lib.oracle_reunitarize.argtypes = [ctypes.c_int64, ctypes.c_int, dp]
+    lib.oracle_su2_pow_series.argtypes = [dp, ctypes.c_double, ctypes.c_int, dp]
+    lib.oracle_site_G_series.argtypes = [ctypes.c_int, dp, ctypes.c_double, ctypes.c_int, dp]
+    lib.oracle_or_sweep_series.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double, ctypes.c_int]
     lib.oracle_K_coulomb.argtypes = [i32p, ctypes.c_int, dp, dp]
     lib.oracle_delta_coulomb.argtypes = [i32p, ctypes.c_int, dp, dp]
     lib.oracle_or_sweep_coulomb.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double]
@@ -216,3 +219,29 @@ def reunitarize(m: np.ndarray) -> None:
     if m.shape[-3:] != (nc, nc, 2) or nc not in (2, 3):
         raise ValueError("need [...,nc,nc,2] with nc = 2 or 3")
     _load().oracle_reunitarize(int(m.size // (2 * nc * nc)), nc, _dp(m))
+
+
+# ---- truncated-series overrelaxation (reading C-24) ------------------------------------
+
+def su2_pow_series(q, omega: float, order: int) -> np.ndarray:
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    out = np.empty(4)
+    _load().oracle_su2_pow_series(_dp(q), float(omega), int(order), _dp(out))
+    return out
+
+
+def site_G_series(K: np.ndarray, omega: float, order: int) -> np.ndarray:
+    K = np.ascontiguousarray(K, dtype=np.float64)
+    out = np.empty_like(K)
+    _load().oracle_site_G_series(K.shape[0], _dp(K), float(omega), int(order), _dp(out))
+    return out
+
+
+def or_sweep_series(dims, u: np.ndarray, parity: int, omega: float, order: int) -> None:
+    nc = _check_links(dims, u)
+    _load().oracle_or_sweep_series(_dims(dims), nc, _dp(u), int(parity), float(omega), int(order))
+
+
+def full_sweep_series(dims, u: np.ndarray, omega: float, order: int) -> None:
+    or_sweep_series(dims, u, 0, omega, order)
+    or_sweep_series(dims, u, 1, omega, order)

@@ -534,3 +534,93 @@ void oracle_reunitarize(int64_t n, int nc, double* M) {
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// Truncated-series overrelaxation (reading C-24; SURVEY.md 8(f) NEXT-2b).  The paper
+// only says "replacing g(x) by g^omega(x)" (citing Mandula-Ogilvie); reading C-8 takes the
+// exact power.  This selectable variant takes the binomial series instead,
+//     g^omega ~ S_N = sum_{n=0}^{N} binom(omega, n) (g - 1)^n ,
+// truncated after order N and projected back to SU(2) by dividing by sqrt(det S_N) (S_N is a
+// complex polynomial in g, hence of the form a + i b n.sigma with det = a^2 + b^2).  Everything is
+// written out literally with 2x2 complex matrices.  The rest of the update is unchanged.
+// ---------------------------------------------------------------------------------------------
+namespace {
+void su2_pow_series(const double q[4], double omega, int order, double out[4]) {
+  Mat g = embed_su2(q, 0, 1, 2);
+  Mat m = add(g, unit_mat(2), 2);                       // m = g - 1
+  m.e[0][0] -= cd(2.0, 0.0);
+  m.e[1][1] -= cd(2.0, 0.0);
+  Mat term = unit_mat(2);                               // binom(omega, n) (g-1)^n, n = 0
+  Mat sum = unit_mat(2);
+  for (int n = 1; n <= order; ++n) {
+    term = mul(term, m, 2);
+    double ratio = (omega - (double)(n - 1)) / (double)n;   // binom(w,n) = binom(w,n-1) (w-n+1)/n
+    for (int a = 0; a < 2; ++a)
+      for (int b = 0; b < 2; ++b) term.e[a][b] *= ratio;
+    sum = add(sum, term, 2);
+  }
+  cd det = sum.e[0][0] * sum.e[1][1] - sum.e[0][1] * sum.e[1][0];
+  double nrm = std::sqrt(det.real());
+  // back to (a0,a1,a2,a3): [[a0 + i a3, a2 + i a1], ...]   (C-7)
+  out[0] = sum.e[0][0].real() / nrm;
+  out[3] = sum.e[0][0].imag() / nrm;
+  out[2] = sum.e[0][1].real() / nrm;
+  out[1] = sum.e[0][1].imag() / nrm;
+}
+
+bool subgroup_step_series(const Mat& K, int i, int j, double omega, int order, int nc, Mat* gs) {
+  double p0 = K.e[i][i].real() + K.e[j][j].real();
+  double p1 = K.e[i][j].imag() + K.e[j][i].imag();
+  double p2 = K.e[i][j].real() - K.e[j][i].real();
+  double p3 = K.e[i][i].imag() - K.e[j][j].imag();
+  double n = std::sqrt(p0 * p0 + p1 * p1 + p2 * p2 + p3 * p3);
+  if (n == 0.0) { *gs = unit_mat(nc); return false; }
+  double g[4] = {p0 / n, -p1 / n, -p2 / n, -p3 / n};
+  double q[4];
+  su2_pow_series(g, omega, order, q);
+  *gs = embed_su2(q, i, j, nc);
+  return true;
+}
+
+Mat site_G_series(Mat K, double omega, int order, int nc) {
+  Mat G = unit_mat(nc);
+  static const int pairs[3][2] = {{0, 1}, {0, 2}, {1, 2}};
+  int npairs = (nc == 2) ? 1 : 3;
+  for (int t = 0; t < npairs; ++t) {
+    Mat gs;
+    if (!subgroup_step_series(K, pairs[t][0], pairs[t][1], omega, order, nc, &gs)) continue;
+    K = mul(gs, K, nc);
+    G = mul(gs, G, nc);
+  }
+  return G;
+}
+}  // namespace
+
+extern "C" {
+
+void oracle_su2_pow_series(const double* q, double omega, int order, double* out) {
+  su2_pow_series(q, omega, order, out);
+}
+
+void oracle_site_G_series(int nc, const double* K, double omega, int order, double* G) {
+  store_mat(G, nc, site_G_series(load_mat(K, nc), omega, order, nc));
+}
+
+// One HALF sweep with the truncated-series power, in place (Landau gauge).
+void oracle_or_sweep_series(const int32_t* dims, int nc, double* U, int parity, double omega, int order) {
+  Lat L = make_lat(dims, nc);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    if (parity_of(L, s) != parity) continue;
+    Mat G = site_G_series(gather_K(U, L, s), omega, order, nc);
+    Mat Gd = dagger(G, nc);
+    for (int mu = 0; mu < 4; ++mu) {
+      double* up = link_ptr(U, L, s, mu);
+      store_mat(up, nc, mul(G, load_mat(up, nc), nc));
+      double* dn = link_ptr(U, L, neighbour(L, s, mu, -1), mu);
+      store_mat(dn, nc, mul(load_mat(dn, nc), Gd, nc));
+    }
+  }
+}
+
+}  // extern "C"
