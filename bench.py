@@ -55,6 +55,8 @@ def parse_args():
     ap.add_argument("--variant", type=int, default=0, help="sweep kernel variant (0 = default)")
     ap.add_argument("--gauge", default="landau", choices=["landau", "coulomb"],
                     help="coulomb: K(x) from the spatial links, per-slice theta_t/F_t (DESIGN.md C-22)")
+    ap.add_argument("--series-order", type=int, default=0,
+                    help="> 0: truncated-series g^omega of that order instead of the exact power (DESIGN.md C-24)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -216,7 +218,7 @@ def flops_per_site(cfg, gauge="landau"):
 
 def workload_config(args, cfg):
     return {
-        "gauge": args.gauge,
+        "gauge": args.gauge, "power": f"series order {args.series_order}" if args.series_order > 0 else "exact",
         "workload": f"{args.workload}: {'x'.join(str(d) for d in cfg['dims'])} SU({cfg['group']}) "
                     f"fp{cfg['precision']} {cfg['params']}-parameter, omega={cfg['omega']}, "
                     f"{cfg['kind']} eps={cfg['eps']} scramble={cfg['scramble']} seed={cfg['seed']}",
@@ -279,6 +281,10 @@ def main():
     if coulomb:
         scal = torch.zeros(2 * n3, dtype=torch.float64, device="cuda")     # theta_t, F_t per slice
     sweeps = culgt.culgt_or_sweeps_coulomb if coulomb else culgt.culgt_or_sweeps
+    if args.series_order > 0:
+        if coulomb:
+            raise SystemExit("--series-order applies to Landau gauge")
+        sweeps = lambda lat_, links_, n_, om_: culgt.culgt_or_sweeps_series(lat_, links_, n_, om_, args.series_order)  # noqa: E731
 
     def check():
         if coulomb:

@@ -132,6 +132,15 @@ int culgt_fix_host(const culgt_lattice* lat, void* canonical_host, void* canonic
                    void* links_dev, void* workspace, int n_sweeps, double omega,
                    double* theta_out, double* F_out, void* stream);
 
+/* ---- Truncated-series overrelaxation (reading C-24; the paper says only "replacing g(x)
+ * by g^omega(x)"): the same half-sweep with g^omega replaced by the binomial series
+ * sum_{n<=order} binom(omega,n) (g-1)^n projected back to SU(2) (order 0..16; the series converges
+ * to the exact power only while |g-1| < 1, i.e. on smooth fields).  Landau gauge. */
+int culgt_or_sweep_series(const culgt_lattice* lat, void* links, int parity, double omega, int order,
+                          void* stream);
+int culgt_or_sweeps_series(const culgt_lattice* lat, void* links, int n_sweeps, double omega, int order,
+                           void* stream);
+
 /* ---- Coulomb gauge (named by the paper, P:L7; reading C-22): the same update
  * with mu restricted to the 3 spatial directions, time-slice by time-slice:
  *   K_C(x) = sum_{i<3} [ U_i(x) + U_i(x-i)^dagger ],  G from K_C as above,

@@ -71,6 +71,8 @@ def lib() -> ctypes.CDLL:
     L.culgt_landau_fix.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                    ctypes.c_int, ctypes.POINTER(ctypes.c_int), dp, dp, vp]
     L.culgt_fix_host.argtypes = [latp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_double, dp, dp, vp]
+    L.culgt_or_sweep_series.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, ctypes.c_int, vp]
+    L.culgt_or_sweeps_series.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, ctypes.c_int, vp]
     L.culgt_or_sweep_coulomb.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_or_sweeps_coulomb.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_coulomb_precision_functional.argtypes = [latp, vp, vp, vp, vp, vp]
@@ -259,6 +261,20 @@ def culgt_fix_host(lat: Lattice, canonical_host, canonical_dev, links_dev, works
                                 _ptr(links_dev), _ptr(workspace), int(n_sweeps), float(omega),
                                 ctypes.byref(theta), ctypes.byref(F), _stream(stream)), "culgt_fix_host")
     return theta.value, F.value
+
+
+# ---- truncated-series overrelaxation (reading C-24) -----------------------------------
+
+def culgt_or_sweep_series(lat: Lattice, links, parity: int, omega: float, order: int, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_or_sweep_series(ctypes.byref(lat.c()), _ptr(links), int(parity), float(omega),
+                                       int(order), _stream(stream)), "culgt_or_sweep_series")
+
+
+def culgt_or_sweeps_series(lat: Lattice, links, n_sweeps: int, omega: float, order: int, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_or_sweeps_series(ctypes.byref(lat.c()), _ptr(links), int(n_sweeps), float(omega),
+                                        int(order), _stream(stream)), "culgt_or_sweeps_series")
 
 
 # ---- Coulomb gauge (reading C-22) ----------------------------------------------------

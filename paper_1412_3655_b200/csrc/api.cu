@@ -260,6 +260,39 @@ int culgt_fix_host(const culgt_lattice* lat, void* canonical_host, void* canonic
   return CULGT_OK;
 }
 
+// ---- truncated-series overrelaxation (reading C-24) ------------------------------------
+
+int culgt_or_sweep_series(const culgt_lattice* lat, void* links, int parity, double omega, int order,
+                          void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (parity != 0 && parity != 1) return CULGT_ERR_PARITY;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  if (order < 0 || order > 16) return CULGT_ERR_ARG;
+  cudaError_t e = launch_or_sweep_series(d, links, parity, omega, order, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_or_sweeps_series(const culgt_lattice* lat, void* links, int n_sweeps, double omega, int order,
+                           void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (n_sweeps < 0 || order < 0 || order > 16) return CULGT_ERR_ARG;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  for (int i = 0; i < n_sweeps; ++i)
+    for (int parity = 0; parity < 2; ++parity) {
+      cudaError_t e = launch_or_sweep_series(d, links, parity, omega, order, (cudaStream_t)stream);
+      if (e != cudaSuccess) return cuda_fail(e);
+    }
+  return CULGT_OK;
+}
+
 // ---- Coulomb gauge (reading C-22) -----------------------------------------------------
 
 int culgt_or_sweep_coulomb(const culgt_lattice* lat, void* links, int parity, double omega, void* stream) {

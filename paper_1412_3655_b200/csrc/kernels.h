@@ -30,6 +30,12 @@ inline size_t reduce_workspace_doubles(const Geom& g) { return reduce_partial_do
 // coulomb = true: Coulomb-gauge half-sweep (K from the spatial links; production mapping only)
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
                             int variant, cudaStream_t st, bool coulomb = false);
+struct SeriesPower;
+// truncated-series overrelaxation (reading C-24), production mappings only
+cudaError_t launch_or_sweep_series(const LatticeDesc& d, void* links, int parity, double omega, int order,
+                                   cudaStream_t st);
+cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int parity, const SeriesPower& pw,
+                                          cudaStream_t st);
 cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
                                    int variant, bool coulomb, cudaStream_t st);
 cudaError_t launch_pack(const LatticeDesc& d, const void* canonical, void* links, cudaStream_t st);

@@ -92,10 +92,10 @@ or_sweep_su3_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
 // for SU(3), reading C-15); the 8 quaternion products in the storage precision.  Odd-parity
 // launches walk the site blocks in descending order (L2 carry-over, as the SU(3) kernel).
 // ---------------------------------------------------------------------------------------------
-template <typename S, int BLOCK, bool COULOMB>
+template <typename S, int BLOCK, bool COULOMB, typename Power>
 __global__ void __launch_bounds__(BLOCK)
 or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
-                    const double omega, const int reverse) {
+                    const Power omega, const int reverse) {
   typedef typename S::Real Real;
   const int blk = reverse ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x;
   const int h = blk * BLOCK + threadIdx.x;
@@ -143,13 +143,29 @@ static cudaError_t launch_su3(void* links, const Geom& g, int parity, double ome
   return cudaGetLastError();
 }
 
-template <typename S>
-static cudaError_t launch_su2(void* links, const Geom& g, int parity, double omega, bool coulomb, cudaStream_t st) {
+template <typename S, typename Power>
+static cudaError_t launch_su2(void* links, const Geom& g, int parity, Power omega, bool coulomb, cudaStream_t st) {
   constexpr int BLOCK = 128;
   const unsigned grid = (unsigned)((g.vh + BLOCK - 1) / BLOCK);
-  if (coulomb) or_sweep_su2_kernel<S, BLOCK, true><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g, parity, omega, parity);
-  else or_sweep_su2_kernel<S, BLOCK, false><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g, parity, omega, parity);
+  if (coulomb) or_sweep_su2_kernel<S, BLOCK, true, Power><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g, parity, omega, parity);
+  else or_sweep_su2_kernel<S, BLOCK, false, Power><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g, parity, omega, parity);
   return cudaGetLastError();
+}
+
+// Truncated-series overrelaxation (reading C-24): b_n = binom(omega, n) by the recurrence
+// b_n = b_{n-1} (omega - n + 1)/n; production mappings only.
+cudaError_t launch_or_sweep_series(const LatticeDesc& d, void* links, int parity, double omega, int order,
+                                   cudaStream_t st) {
+  if (order < 0 || order > kMaxSeriesOrder) return cudaErrorInvalidValue;
+  SeriesPower pw;
+  pw.order = order;
+  pw.b[0] = 1.0;
+  for (int n = 1; n <= kMaxSeriesOrder; ++n) pw.b[n] = n <= order ? pw.b[n - 1] * ((omega - (double)(n - 1)) / (double)n) : 0.0;
+  if (d.group == 2) {
+    if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, d.geom, parity, pw, false, st);
+    return launch_su2<Storage<double, 2, 4> >(links, d.geom, parity, pw, false, st);
+  }
+  return launch_or_sweep_staged_series(d, links, parity, pw, st);
 }
 
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,

@@ -30,6 +30,11 @@
 
 namespace culgt {
 
+// omega as a plain double for the all-fp32 measurement kernels (which only know the exact power)
+__device__ __forceinline__ double power_omega(double w) { return w; }
+__device__ __forceinline__ double power_omega(const ExactPower& p) { return p.omega; }
+__device__ __forceinline__ double power_omega(const SeriesPower&) { return 0.0; }
+
 // Option bits of the OPT template parameter.
 constexpr int OPT_PREFETCH = 1;    // persistent only: prefetch.global.L2 of the next site block
 constexpr int OPT_CHUNKED = 4;     // persistent only: contiguous chunk of site blocks per CTA
@@ -121,10 +126,10 @@ __device__ __forceinline__ typename S::Vec* vec_ptr(typename S::Vec* links, cons
   return base + (unsigned)r.idx[l];
 }
 
-template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int OPT>
+template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int OPT, typename Power>
 __global__ void __launch_bounds__(BLOCK, MINB)
 or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
-                           const double omega, const int n_site_blocks, const int reverse) {
+                           const Power omega, const int n_site_blocks, const int reverse) {
   typedef typename S::Real Real;
   typedef typename S::Vec Vec;
   constexpr int LPT = 8 / TPS;          // links per thread
@@ -251,7 +256,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
       for (int i = 0; i < 18; ++i) G[i] = (Real)Gd[i];
     } else {
       Acc Ga[18];
-      su3_site_G(K, Ga, (Acc)omega);
+      su3_site_G(K, Ga, (Acc)power_omega(omega));
 #pragma unroll
       for (int i = 0; i < 18; ++i) G[i] = (Real)Ga[i];
     }
@@ -300,11 +305,11 @@ static int sm_count() {
   return n;
 }
 
-template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int OPT>
-static cudaError_t launch_staged(void* links, const Geom& g, int parity, double omega, bool reverse_odd,
+template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int OPT, typename Power>
+static cudaError_t launch_staged(void* links, const Geom& g, int parity, Power omega, bool reverse_odd,
                                  cudaStream_t st) {
   typedef typename S::Vec Vec;
-  auto kern = or_sweep_su3_staged_kernel<S, Acc, TPS, BLOCK, STAGES, MINB, OPT>;
+  auto kern = or_sweep_su3_staged_kernel<S, Acc, TPS, BLOCK, STAGES, MINB, OPT, Power>;
   constexpr size_t smem = (size_t)STAGES * (8 / TPS) * S::NV * BLOCK * sizeof(Vec);
   static bool configured = false;
   if (!configured) {
@@ -395,6 +400,20 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
     case 32: return launch_staged<S, double, 1, 96, 2, 1, 0>(links, g, parity, omega, true, st);             // pers, 2 stages
     default: return cudaErrorInvalidValue;
   }
+}
+
+// Truncated-series overrelaxation (reading C-24) on the production mapping of each format.
+cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int parity, const SeriesPower& pw,
+                                          cudaStream_t st) {
+  const Geom& g = d.geom;
+  if (d.group != 3) return cudaErrorInvalidValue;
+  if (d.precision == 32 && d.params == 12)
+    return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT>(links, g, parity, pw, true, st);
+  if (d.precision == 32)
+    return launch_staged<Storage<float, 3, 18>, double, 2, 256, 1, 2, 0>(links, g, parity, pw, true, st);
+  if (d.params == 12)
+    return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT>(links, g, parity, pw, true, st);
+  return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT>(links, g, parity, pw, true, st);
 }
 
 }  // namespace culgt

@@ -131,4 +131,47 @@ __device__ __forceinline__ bool su2_update_power(const double* p, double omega, 
   return true;
 }
 
+// ---- how g is raised to the power omega: a policy object passed down from the kernel parameter ----
+// ExactPower: the exact group power of reading C-8 (above).  SeriesPower: the truncated binomial
+// series of reading C-24,  g^omega ~ S_N = sum_{n<=N} binom(omega,n) (g-1)^n, projected back to
+// SU(2).  (g-1)^n lives in span{1, i n.sigma}, so with z = (cos a - 1) + i sin a the series is the
+// complex polynomial w = sum b_n z^n and the result is (Re w, n Im w)/|w|: a Horner loop, no
+// transcendental function at all.  b_n = binom(omega, n) is filled in on the host.
+struct ExactPower {
+  double omega;
+};
+constexpr int kMaxSeriesOrder = 16;
+struct SeriesPower {
+  int order;
+  double b[kMaxSeriesOrder + 1];
+};
+
+template <bool FULL>
+__device__ __forceinline__ bool su2_update_power(const double* p, const ExactPower& pw, double* q) {
+  return su2_update_power<FULL>(p, pw.omega, q);
+}
+
+template <bool FULL>
+__device__ __forceinline__ bool su2_update_power(const double* p, const SeriesPower& pw, double* q) {
+  const double r2 = p[1] * p[1] + p[2] * p[2] + p[3] * p[3];
+  const double n2 = fma(p[0], p[0], r2);
+  if (n2 < 1e-280) return false;                           // |p| = 0: the update is skipped (C-9)
+  const double rinv = (r2 < 1e-280) ? 0.0 : rsqrt_newton<true>(r2);   // g = +-1: z is real, v part 0
+  const double ninv = rsqrt_newton<true>(n2);
+  const double zr = p[0] * ninv - 1.0;                     // cos a - 1
+  const double zi = r2 * rinv * ninv;                      // sin a
+  double wr = 0.0, wi = 0.0;
+#pragma unroll
+  for (int n = kMaxSeriesOrder; n >= 0; --n)
+    if (n <= pw.order) {                                   // warp-uniform; b[n] is a compile-time slot
+      const double tr = fma(wr, zr, fma(-wi, zi, pw.b[n]));
+      wi = fma(wr, zi, wi * zr);
+      wr = tr;
+    }
+  const double winv = rsqrt_newton<true>(fma(wr, wr, wi * wi));
+  const double f = -wi * winv * rinv;                      // v/|v| = -pv/|pv|
+  q[0] = wr * winv; q[1] = p[1] * f; q[2] = p[2] * f; q[3] = p[3] * f;
+  return true;
+}
+
 }  // namespace culgt

@@ -17,8 +17,8 @@
 namespace culgt {
 
 // p = real-quaternion part (x2) of the (I,J) block of K; q = (conj(p)/|p|)^omega.
-template <int I, int J, bool FULL>
-__device__ __forceinline__ bool subgroup_quaternion(const double* K, double omega, double* q) {
+template <int I, int J, bool FULL, typename Power>
+__device__ __forceinline__ bool subgroup_quaternion(const double* K, const Power& omega, double* q) {
   double p[4];
   p[0] = K[CULGT_RE(I, I)] + K[CULGT_RE(J, J)];
   p[1] = K[CULGT_IM(I, J)] + K[CULGT_IM(J, I)];
@@ -51,8 +51,9 @@ __device__ __forceinline__ void rotate_col(T* M, int c, T ar, T ai, T br, T bi) 
 // K (fp64, destroyed) -> G (type GT).  g_s embeds q = (c, v1, v2, v3) as
 // [I][I] = a = c + i v3, [I][J] = b = v2 + i v1, [J][I] = -conj(b), [J][J] = conj(a)  (C-7).
 // FULL selects full-length (fp64 storage) or shortened (fp32 storage) series in su2_power.cuh.
-template <bool FULL, typename GT>
-__device__ __forceinline__ void su3_solve(double* K, GT* G, double omega) {
+// Power = double (omega; exact power), ExactPower or SeriesPower (su2_power.cuh).
+template <bool FULL, typename GT, typename Power>
+__device__ __forceinline__ void su3_solve(double* K, GT* G, const Power& omega) {
   double q[4];
   // ---- subgroup (0,1)
   bool ok = subgroup_quaternion<0, 1, FULL>(K, omega, q);
