@@ -413,8 +413,8 @@ int culgt_autotune_sweep(const culgt_lattice* lat, void* links, double omega, in
   int best = 0;
   float best_us = -1.f;
   for (int v = 0; v < 40; ++v) {
-    // 11, 14, 25: all-fp32 arithmetic (different precision); 28: measurement-only (no K / solve)
-    if (v == 11 || v == 14 || v == 25 || v == 28) continue;
+    // 11, 14, 25: all-fp32 arithmetic (different precision); 28, 32: measurement-only (no solve)
+    if (v == 11 || v == 14 || v == 25 || v == 28 || v == 32) continue;
     if (d.group == 2 && v != 0) continue;
     cudaError_t e = cudaSuccess;
     for (int parity = 0; parity < 2 && e == cudaSuccess; ++parity) e = launch_or_sweep(d, links, parity, omega, v, st);

@@ -41,6 +41,7 @@ constexpr int OPT_CHUNKED = 4;     // persistent only: contiguous chunk of site 
 constexpr int OPT_NOMATH = 8;      // measurement only: G = 1 (memory pattern + products, no K / solve)
 constexpr int OPT_FLAT = 16;       // one CTA per site block (hardware block scheduler), not persistent
 constexpr int OPT_STREAM_ST = 32;  // st.global.cs stores
+constexpr int OPT_NOSOLVE = 256;   // measurement only: K is accumulated but G = 1 (no subgroup solve)
 constexpr int OPT_COULOMB = 64;    // Coulomb gauge (reading C-22): K(x) from the 6 spatial links only
 
 __device__ __forceinline__ void cp_async_vec(float4* smem, const float4* gmem) {
@@ -251,6 +252,12 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
       // G = g_3 g_2 g_1 is accumulated in fp64 and rounded once: accumulating it in fp32 costs
       // 0.7 % less time but doubles the worst link error at 32^4 (1.08e-5 vs 5.8e-6)
       double Gd[18];
+      if (OPT & OPT_NOSOLVE) {
+        double acc = 0;
+#pragma unroll
+        for (int i = 0; i < 18; ++i) { acc += Kd[i]; Gd[i] = (i == 0 || i == 8 || i == 16) ? 1.0 : 0.0; }
+        Gd[1] = acc * 1e-300;      // keeps K alive
+      } else
       su3_solve<(sizeof(Real) == 8), double>(Kd, Gd, omega);
 #pragma unroll
       for (int i = 0; i < 18; ++i) G[i] = (Real)Gd[i];
@@ -359,6 +366,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
       case 27: return launch_staged<S, double, 1, 256, 1, 2, OPT_CHUNKED>(links, g, parity, omega, true, st);
       case 28: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT | OPT_NOMATH>(links, g, parity, omega, true, st);
       case 29: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT | OPT_STREAM_ST>(links, g, parity, omega, true, st);
+      case 32: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT | OPT_NOSOLVE>(links, g, parity, omega, true, st);
       case 30: return launch_staged<S, double, 1, 256, 1, 2, OPT_FLAT>(links, g, parity, omega, true, st);
       case 31: return launch_staged<S, double, 1, 32, 1, 16, OPT_FLAT>(links, g, parity, omega, true, st);
       default: return cudaErrorInvalidValue;
