@@ -60,6 +60,11 @@ def _load():
     lib.oracle_plaquette.restype = ctypes.c_double
     lib.oracle_reconstruct12.argtypes = [ctypes.c_int64, dp]
     lib.oracle_reunitarize.argtypes = [ctypes.c_int64, ctypes.c_int, dp]
+    u32p = ctypes.POINTER(ctypes.c_uint32)
+    lib.oracle_philox4x32_10.argtypes = [u32p, u32p, u32p]
+    lib.oracle_su2_heatbath_samples.argtypes = [dp, ctypes.c_double, ctypes.c_uint64, ctypes.c_int64, dp]
+    lib.oracle_sa_sweep.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double, ctypes.c_uint64,
+                                    ctypes.c_uint32]
     lib.oracle_su2_pow_series.argtypes = [dp, ctypes.c_double, ctypes.c_int, dp]
     lib.oracle_site_G_series.argtypes = [ctypes.c_int, dp, ctypes.c_double, ctypes.c_int, dp]
     lib.oracle_or_sweep_series.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double, ctypes.c_int]
@@ -245,3 +250,27 @@ def or_sweep_series(dims, u: np.ndarray, parity: int, omega: float, order: int) 
 def full_sweep_series(dims, u: np.ndarray, omega: float, order: int) -> None:
     or_sweep_series(dims, u, 0, omega, order)
     or_sweep_series(dims, u, 1, omega, order)
+
+
+# ---- simulated annealing (reading C-25) --------------------------------------------------
+
+def philox4x32_10(ctr, key) -> np.ndarray:
+    c = np.ascontiguousarray(ctr, dtype=np.uint32)
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.empty(4, dtype=np.uint32)
+    u32p = ctypes.POINTER(ctypes.c_uint32)
+    _load().oracle_philox4x32_10(c.ctypes.data_as(u32p), k.ctypes.data_as(u32p), out.ctypes.data_as(u32p))
+    return out
+
+
+def su2_heatbath_samples(p, T: float, seed: int, n: int) -> np.ndarray:
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    out = np.empty((int(n), 4))
+    _load().oracle_su2_heatbath_samples(_dp(p), float(T), int(seed), int(n), _dp(out))
+    return out
+
+
+def sa_sweep(dims, u: np.ndarray, parity: int, T: float, seed: int, counter: int) -> None:
+    """One simulated-annealing half-sweep at temperature T, in place."""
+    nc = _check_links(dims, u)
+    _load().oracle_sa_sweep(_dims(dims), nc, _dp(u), int(parity), float(T), int(seed), int(counter))

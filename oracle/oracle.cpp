@@ -624,3 +624,145 @@ void oracle_or_sweep_series(const int32_t* dims, int nc, double* U, int parity, 
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// Simulated annealing (named by the paper as the companion of overrelaxation, P:L7; its
+// details are in the unavailable ref. [2] -- DESIGN.md reading C-25).
+// Reading, from first principles: at temperature T the site's gauge transformation is not the
+// maximiser of Re tr[g K(x)] but a sample of the Boltzmann weight exp(Re tr[g K(x)]/T) dg (Haar
+// dg), per SU(2) subgroup for SU(3), with the same checkerboard, subgroup order and K <- g_s K,
+// G <- g_s G bookkeeping as the overrelaxation sweep.  In a subgroup with quaternion p (as in
+// subgroup_step) Re tr[g_s K] = |p| h_0 + const for h = q * (p/|p|), so h_0 has the density
+// sqrt(1 - h_0^2) exp(a h_0), a = |p|/T, and the direction of the vector part of h is uniform on
+// S^2; then q = h * conj(p)/|p|.  h_0 by the Kennedy-Pendleton method:
+//     lambda^2 = -( ln r1 + cos^2(2 pi r2) ln r3 ) / (2 a),  accept if r4^2 <= 1 - lambda^2,  h_0 = 1 - 2 lambda^2.
+// Random numbers: the counter-based Philox4x32-10 generator (Salmon et al., SC'11), restated here;
+// counter = (canonical site, half-sweep counter, subgroup | draw << 8, 0), key = 64-bit seed, so a
+// site's numbers do not depend on the traversal order or the thread count.  Uniforms in (0,1]:
+// 53 bits from two 32-bit words.
+// ---------------------------------------------------------------------------------------------
+namespace {
+void philox4x32_10(const uint32_t ctr_in[4], const uint32_t key_in[2], uint32_t out[4]) {
+  uint32_t c0 = ctr_in[0], c1 = ctr_in[1], c2 = ctr_in[2], c3 = ctr_in[3];
+  uint32_t k0 = key_in[0], k1 = key_in[1];
+  for (int r = 0; r < 10; ++r) {
+    uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+    uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+    uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    uint32_t n1 = (uint32_t)p1;
+    uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    uint32_t n3 = (uint32_t)p0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// two uniforms in (0,1] from one Philox block
+void uniforms2(const uint32_t w[4], double u[2]) {
+  u[0] = ((double)(((uint64_t)(w[0] >> 5) << 26) + (w[1] >> 6)) + 1.0) * (1.0 / 9007199254740992.0);
+  u[1] = ((double)(((uint64_t)(w[2] >> 5) << 26) + (w[3] >> 6)) + 1.0) * (1.0 / 9007199254740992.0);
+}
+
+struct SiteRng {
+  uint32_t ctr[4];
+  uint32_t key[2];
+  uint32_t draw;
+  void next2(double u[2]) {
+    uint32_t c[4] = {ctr[0], ctr[1], ctr[2] | (draw << 8), ctr[3]};
+    uint32_t w[4];
+    philox4x32_10(c, key, w);
+    uniforms2(w, u);
+    ++draw;
+  }
+};
+
+// q = h * conj(p)/|p| with h sampled as described above; a = |p|/T.
+void su2_heatbath(const double p[4], double n, double T, SiteRng* rng, double q[4]) {
+  const double a = n / T;
+  double lam2;
+  for (;;) {
+    double u[2], v[2];
+    rng->next2(u);                                   // r1, r2
+    rng->next2(v);                                   // r3, r4
+    double c = std::cos(2.0 * M_PI * u[1]);
+    lam2 = -(std::log(u[0]) + c * c * std::log(v[0])) / (2.0 * a);
+    if (v[1] * v[1] <= 1.0 - lam2) break;
+  }
+  double h0 = 1.0 - 2.0 * lam2;
+  double u[2];
+  rng->next2(u);                                     // direction of the vector part
+  double ct = 2.0 * u[0] - 1.0;
+  double st = std::sqrt(std::fmax(0.0, 1.0 - ct * ct));
+  double phi = 2.0 * M_PI * u[1];
+  double r = std::sqrt(std::fmax(0.0, 1.0 - h0 * h0));
+  double h[4] = {h0, r * st * std::cos(phi), r * st * std::sin(phi), r * ct};
+  // q = h * conj(p)/|p|   (quaternion product of convention C-7: (ab)_0 = a0 b0 - a.b, (ab)_v = a0 b + b0 a - a x b)
+  double b[4] = {p[0] / n, -p[1] / n, -p[2] / n, -p[3] / n};
+  q[0] = h[0] * b[0] - h[1] * b[1] - h[2] * b[2] - h[3] * b[3];
+  q[1] = h[0] * b[1] + b[0] * h[1] - (h[2] * b[3] - h[3] * b[2]);
+  q[2] = h[0] * b[2] + b[0] * h[2] - (h[3] * b[1] - h[1] * b[3]);
+  q[3] = h[0] * b[3] + b[0] * h[3] - (h[1] * b[2] - h[2] * b[1]);
+}
+
+Mat site_G_heatbath(Mat K, double T, int nc, uint32_t site, uint32_t counter, uint64_t seed) {
+  Mat G = unit_mat(nc);
+  static const int pairs[3][2] = {{0, 1}, {0, 2}, {1, 2}};
+  int npairs = (nc == 2) ? 1 : 3;
+  for (int t = 0; t < npairs; ++t) {
+    int i = pairs[t][0], j = pairs[t][1];
+    double p[4] = {K.e[i][i].real() + K.e[j][j].real(), K.e[i][j].imag() + K.e[j][i].imag(),
+                   K.e[i][j].real() - K.e[j][i].real(), K.e[i][i].imag() - K.e[j][j].imag()};
+    double n = std::sqrt(p[0] * p[0] + p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
+    if (n == 0.0) continue;
+    SiteRng rng;
+    rng.ctr[0] = site; rng.ctr[1] = counter; rng.ctr[2] = (uint32_t)t; rng.ctr[3] = 0;
+    rng.key[0] = (uint32_t)seed; rng.key[1] = (uint32_t)(seed >> 32);
+    rng.draw = 0;
+    double q[4];
+    su2_heatbath(p, n, T, &rng, q);
+    Mat gs = embed_su2(q, i, j, nc);
+    K = mul(gs, K, nc);
+    G = mul(gs, G, nc);
+  }
+  return G;
+}
+}  // namespace
+
+extern "C" {
+
+void oracle_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
+
+// n samples of q for a given quaternion p at temperature T (site = sample index): out double[n][4].
+void oracle_su2_heatbath_samples(const double* p, double T, uint64_t seed, int64_t n, double* out) {
+  double nrm = std::sqrt(p[0] * p[0] + p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
+  for (int64_t k = 0; k < n; ++k) {
+    SiteRng rng;
+    rng.ctr[0] = (uint32_t)k; rng.ctr[1] = 0; rng.ctr[2] = 0; rng.ctr[3] = 0;
+    rng.key[0] = (uint32_t)seed; rng.key[1] = (uint32_t)(seed >> 32);
+    rng.draw = 0;
+    su2_heatbath(p, nrm, T, &rng, out + 4 * k);
+  }
+}
+
+// One HALF sweep of simulated annealing at temperature T over the sites of `parity`, in place.
+// `counter` must be different for every half-sweep of a run (it selects the random numbers).
+void oracle_sa_sweep(const int32_t* dims, int nc, double* U, int parity, double T, uint64_t seed,
+                     uint32_t counter) {
+  Lat L = make_lat(dims, nc);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    if (parity_of(L, s) != parity) continue;
+    Mat G = site_G_heatbath(gather_K(U, L, s), T, nc, (uint32_t)s, counter, seed);
+    Mat Gd = dagger(G, nc);
+    for (int mu = 0; mu < 4; ++mu) {
+      double* up = link_ptr(U, L, s, mu);
+      store_mat(up, nc, mul(G, load_mat(up, nc), nc));
+      double* dn = link_ptr(U, L, neighbour(L, s, mu, -1), mu);
+      store_mat(dn, nc, mul(load_mat(dn, nc), Gd, nc));
+    }
+  }
+}
+
+}  // extern "C"
