@@ -57,6 +57,8 @@ def parse_args():
                     help="coulomb: K(x) from the spatial links, per-slice theta_t/F_t (DESIGN.md C-22)")
     ap.add_argument("--series-order", type=int, default=0,
                     help="> 0: truncated-series g^omega of that order instead of the exact power (DESIGN.md C-24)")
+    ap.add_argument("--sa-temperature", type=float, default=0.0,
+                    help="> 0: time simulated-annealing sweeps at this temperature instead of overrelaxation (DESIGN.md C-25)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -218,7 +220,8 @@ def flops_per_site(cfg, gauge="landau"):
 
 def workload_config(args, cfg):
     return {
-        "gauge": args.gauge, "power": f"series order {args.series_order}" if args.series_order > 0 else "exact",
+        "gauge": args.gauge, "power": (f"heat bath at T={args.sa_temperature}" if args.sa_temperature > 0 else
+                                       f"series order {args.series_order}" if args.series_order > 0 else "exact"),
         "workload": f"{args.workload}: {'x'.join(str(d) for d in cfg['dims'])} SU({cfg['group']}) "
                     f"fp{cfg['precision']} {cfg['params']}-parameter, omega={cfg['omega']}, "
                     f"{cfg['kind']} eps={cfg['eps']} scramble={cfg['scramble']} seed={cfg['seed']}",
@@ -281,6 +284,10 @@ def main():
     if coulomb:
         scal = torch.zeros(2 * n3, dtype=torch.float64, device="cuda")     # theta_t, F_t per slice
     sweeps = culgt.culgt_or_sweeps_coulomb if coulomb else culgt.culgt_or_sweeps
+    if args.sa_temperature > 0:
+        if coulomb or args.series_order > 0:
+            raise SystemExit("--sa-temperature applies to Landau gauge and excludes --series-order")
+        sweeps = lambda lat_, links_, n_, om_: culgt.culgt_sa_anneal(lat_, links_, args.sa_temperature, args.sa_temperature, n_, 2024)  # noqa: E731
     if args.series_order > 0:
         if coulomb:
             raise SystemExit("--series-order applies to Landau gauge")

@@ -141,6 +141,18 @@ int culgt_or_sweep_series(const culgt_lattice* lat, void* links, int parity, dou
 int culgt_or_sweeps_series(const culgt_lattice* lat, void* links, int n_sweeps, double omega, int order,
                            void* stream);
 
+/* ---- Simulated annealing (named by the paper beside overrelaxation, P:L7; DESIGN.md reading
+ * C-25): a half-sweep in which the site's transformation is a SAMPLE of exp(Re tr[g K(x)]/T) dg
+ * (per SU(2) subgroup for SU(3); Kennedy-Pendleton heat bath) instead of its maximiser.  Random
+ * numbers: Philox4x32-10 with counter (canonical site, `counter`, subgroup | draw << 8, 0) and key
+ * `seed`; `counter` must differ between the half-sweeps of a run.  T > 0.  Landau gauge.
+ * culgt_sa_anneal: n_sweeps full sweeps with T going linearly from T_max to T_min, half-sweep
+ * counters 0, 1, 2, ...; asynchronous (follow it with overrelaxation to converge). */
+int culgt_sa_sweep(const culgt_lattice* lat, void* links, int parity, double T, unsigned long long seed,
+                   unsigned counter, void* stream);
+int culgt_sa_anneal(const culgt_lattice* lat, void* links, double T_max, double T_min, int n_sweeps,
+                    unsigned long long seed, void* stream);
+
 /* ---- Coulomb gauge (named by the paper, P:L7; reading C-22): the same update
  * with mu restricted to the 3 spatial directions, time-slice by time-slice:
  *   K_C(x) = sum_{i<3} [ U_i(x) + U_i(x-i)^dagger ],  G from K_C as above,

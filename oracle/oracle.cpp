@@ -634,8 +634,10 @@ void oracle_or_sweep_series(const int32_t* dims, int nc, double* U, int parity, 
 // G <- g_s G bookkeeping as the overrelaxation sweep.  In a subgroup with quaternion p (as in
 // subgroup_step) Re tr[g_s K] = |p| h_0 + const for h = q * (p/|p|), so h_0 has the density
 // sqrt(1 - h_0^2) exp(a h_0), a = |p|/T, and the direction of the vector part of h is uniform on
-// S^2; then q = h * conj(p)/|p|.  h_0 by the Kennedy-Pendleton method:
-//     lambda^2 = -( ln r1 + cos^2(2 pi r2) ln r3 ) / (2 a),  accept if r4^2 <= 1 - lambda^2,  h_0 = 1 - 2 lambda^2.
+// S^2; then q = h * conj(p)/|p|.  h_0 for a >= 2 by the Kennedy-Pendleton method:
+//     lambda^2 = -( ln r1 + cos^2(2 pi r2) ln r3 ) / (2 a),  accept if r4^2 <= 1 - lambda^2,  h_0 = 1 - 2 lambda^2,
+// and for a < 2 (where that method accepts too rarely) by Creutz's: h_0 = 1 + ln(x)/a with x uniform
+// in [e^{-2a}, 1], accepted with probability sqrt(1 - h_0^2).
 // Random numbers: the counter-based Philox4x32-10 generator (Salmon et al., SC'11), restated here;
 // counter = (canonical site, half-sweep counter, subgroup | draw << 8, 0), key = 64-bit seed, so a
 // site's numbers do not depend on the traversal order or the thread count.  Uniforms in (0,1]:
@@ -681,16 +683,31 @@ struct SiteRng {
 // q = h * conj(p)/|p| with h sampled as described above; a = |p|/T.
 void su2_heatbath(const double p[4], double n, double T, SiteRng* rng, double q[4]) {
   const double a = n / T;
-  double lam2;
-  for (;;) {
-    double u[2], v[2];
-    rng->next2(u);                                   // r1, r2
-    rng->next2(v);                                   // r3, r4
-    double c = std::cos(2.0 * M_PI * u[1]);
-    lam2 = -(std::log(u[0]) + c * c * std::log(v[0])) / (2.0 * a);
-    if (v[1] * v[1] <= 1.0 - lam2) break;
+  double h0;
+  if (a < 2.0) {
+    // small a (hot / nearly cancelling K): Kennedy-Pendleton accepts with probability ~a^{3/2} there;
+    // Creutz's method instead: x uniform in [e^{-2a}, 1], h_0 = 1 + ln(x)/a has density exp(a h_0)
+    // on [-1, 1]; accept with probability sqrt(1 - h_0^2)
+    const double emin = std::exp(-2.0 * a);
+    for (;;) {
+      double u[2];
+      rng->next2(u);
+      double x = emin + u[0] * (1.0 - emin);
+      h0 = 1.0 + std::log(x) / a;
+      if (u[1] * u[1] <= 1.0 - h0 * h0) break;
+    }
+  } else {
+    double lam2;
+    for (;;) {
+      double u[2], v[2];
+      rng->next2(u);                                   // r1, r2
+      rng->next2(v);                                   // r3, r4
+      double c = std::cos(2.0 * M_PI * u[1]);
+      lam2 = -(std::log(u[0]) + c * c * std::log(v[0])) / (2.0 * a);
+      if (v[1] * v[1] <= 1.0 - lam2) break;
+    }
+    h0 = 1.0 - 2.0 * lam2;
   }
-  double h0 = 1.0 - 2.0 * lam2;
   double u[2];
   rng->next2(u);                                     // direction of the vector part
   double ct = 2.0 * u[0] - 1.0;

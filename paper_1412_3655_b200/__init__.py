@@ -73,6 +73,8 @@ def lib() -> ctypes.CDLL:
     L.culgt_fix_host.argtypes = [latp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_double, dp, dp, vp]
     L.culgt_or_sweep_series.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, ctypes.c_int, vp]
     L.culgt_or_sweeps_series.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, ctypes.c_int, vp]
+    L.culgt_sa_sweep.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, ctypes.c_ulonglong, ctypes.c_uint, vp]
+    L.culgt_sa_anneal.argtypes = [latp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_ulonglong, vp]
     L.culgt_or_sweep_coulomb.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_or_sweeps_coulomb.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_coulomb_precision_functional.argtypes = [latp, vp, vp, vp, vp, vp]
@@ -275,6 +277,20 @@ def culgt_or_sweeps_series(lat: Lattice, links, n_sweeps: int, omega: float, ord
     _require_cuda()
     _check(lib().culgt_or_sweeps_series(ctypes.byref(lat.c()), _ptr(links), int(n_sweeps), float(omega),
                                         int(order), _stream(stream)), "culgt_or_sweeps_series")
+
+
+# ---- simulated annealing (reading C-25) -----------------------------------------------
+
+def culgt_sa_sweep(lat: Lattice, links, parity: int, T: float, seed: int, counter: int, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_sa_sweep(ctypes.byref(lat.c()), _ptr(links), int(parity), float(T), int(seed),
+                                int(counter), _stream(stream)), "culgt_sa_sweep")
+
+
+def culgt_sa_anneal(lat: Lattice, links, T_max: float, T_min: float, n_sweeps: int, seed: int, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_sa_anneal(ctypes.byref(lat.c()), _ptr(links), float(T_max), float(T_min),
+                                 int(n_sweeps), int(seed), _stream(stream)), "culgt_sa_anneal")
 
 
 # ---- Coulomb gauge (reading C-22) ----------------------------------------------------

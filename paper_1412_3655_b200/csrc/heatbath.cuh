@@ -1,0 +1,93 @@
+// heatbath.cuh -- simulated annealing: the site's gauge transformation sampled from the Boltzmann
+// weight exp(Re tr[g K(x)]/T) instead of maximising it (PAPER.md L7, L11 name simulated annealing;
+// DESIGN.md reading C-25).  Per SU(2) subgroup with quaternion p:  h = q * p/|p| has
+// h_0 ~ sqrt(1 - h_0^2) exp(a h_0), a = |p|/T, vector part uniform on S^2;  q = h * conj(p)/|p|.
+// h_0 by the Kennedy-Pendleton method for a >= 2 and by Creutz's for a < 2; random numbers from the counter-based Philox4x32-10
+// generator with counter (canonical site, half-sweep counter, subgroup | draw << 8, 0) and the
+// 64-bit seed as key, so a site's numbers do not depend on the thread mapping.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace culgt {
+
+struct HeatBathPower {
+  double inv_T;
+  uint32_t seed_lo, seed_hi;
+  uint32_t counter;          // half-sweep counter: must differ between the half-sweeps of a run
+};
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t* out) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// two uniforms in (0,1], 53 bits each, from the block with draw index `draw`
+__device__ __forceinline__ void heatbath_uniforms(const HeatBathPower& pw, uint32_t site, uint32_t sub,
+                                                  uint32_t draw, double* u0, double* u1) {
+  uint32_t w[4];
+  philox4x32_10(site, pw.counter, sub | (draw << 8), 0u, pw.seed_lo, pw.seed_hi, w);
+  *u0 = ((double)(((uint64_t)(w[0] >> 5) << 26) + (w[1] >> 6)) + 1.0) * (1.0 / 9007199254740992.0);
+  *u1 = ((double)(((uint64_t)(w[2] >> 5) << 26) + (w[3] >> 6)) + 1.0) * (1.0 / 9007199254740992.0);
+}
+
+// q sampled for the un-normalised subgroup quaternion p; false when p == 0 (no update, C-9).
+__device__ __forceinline__ bool su2_heatbath(const double* p, const HeatBathPower& pw, uint32_t site,
+                                             uint32_t sub, double* q) {
+  const double n2 = p[0] * p[0] + p[1] * p[1] + p[2] * p[2] + p[3] * p[3];
+  if (!(n2 > 0.0) || !(n2 < 1e300)) return false;      // p = 0 (C-9); also keeps NaN/Inf out of the loop
+  const double n = sqrt(n2);
+  const double a = n * pw.inv_T;
+  uint32_t draw = 0;
+  double h0;
+  if (a < 2.0) {
+    // Creutz's method where Kennedy-Pendleton would accept with probability ~a^{3/2}
+    const double emin = exp(-2.0 * a);
+    for (;;) {
+      if (draw >= (1u << 22)) { h0 = 1.0; break; }       // unreachable; never spin forever
+      double r1, r2;
+      heatbath_uniforms(pw, site, sub, draw, &r1, &r2);
+      draw += 1;
+      h0 = 1.0 + log(emin + r1 * (1.0 - emin)) / a;
+      if (r2 * r2 <= 1.0 - h0 * h0) break;
+    }
+  } else {
+    double lam2;
+    for (;;) {
+      if (draw >= (1u << 22)) { lam2 = 0.0; break; }     // unreachable for finite a; never spin forever
+      double r1, r2, r3, r4;
+      heatbath_uniforms(pw, site, sub, draw, &r1, &r2);
+      heatbath_uniforms(pw, site, sub, draw + 1, &r3, &r4);
+      draw += 2;
+      const double c = cospi(2.0 * r2);
+      lam2 = -(log(r1) + c * c * log(r3)) / (2.0 * a);
+      if (r4 * r4 <= 1.0 - lam2) break;
+    }
+    h0 = 1.0 - 2.0 * lam2;
+  }
+  double u0, u1;
+  heatbath_uniforms(pw, site, sub, draw, &u0, &u1);
+  const double ct = 2.0 * u0 - 1.0;
+  const double st = sqrt(fmax(0.0, 1.0 - ct * ct));
+  double sp, cp;
+  sincospi(2.0 * u1, &sp, &cp);
+  const double r = sqrt(fmax(0.0, 1.0 - h0 * h0));
+  const double h[4] = {h0, r * st * cp, r * st * sp, r * ct};
+  const double b[4] = {p[0] / n, -p[1] / n, -p[2] / n, -p[3] / n};
+  q[0] = h[0] * b[0] - h[1] * b[1] - h[2] * b[2] - h[3] * b[3];
+  q[1] = h[0] * b[1] + b[0] * h[1] - (h[2] * b[3] - h[3] * b[2]);
+  q[2] = h[0] * b[2] + b[0] * h[2] - (h[3] * b[1] - h[1] * b[3]);
+  q[3] = h[0] * b[3] + b[0] * h[3] - (h[1] * b[2] - h[2] * b[1]);
+  return true;
+}
+
+}  // namespace culgt

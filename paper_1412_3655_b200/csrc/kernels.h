@@ -31,6 +31,12 @@ inline size_t reduce_workspace_doubles(const Geom& g) { return reduce_partial_do
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
                             int variant, cudaStream_t st, bool coulomb = false);
 struct SeriesPower;
+struct HeatBathPower;
+// simulated-annealing half-sweep (reading C-25), production mappings only
+cudaError_t launch_sa_sweep(const LatticeDesc& d, void* links, int parity, double T, unsigned long long seed,
+                            unsigned counter, cudaStream_t st);
+cudaError_t launch_or_sweep_staged_heatbath(const LatticeDesc& d, void* links, int parity, const HeatBathPower& pw,
+                                            cudaStream_t st);
 // truncated-series overrelaxation (reading C-24), production mappings only
 cudaError_t launch_or_sweep_series(const LatticeDesc& d, void* links, int parity, double omega, int order,
                                    cudaStream_t st);

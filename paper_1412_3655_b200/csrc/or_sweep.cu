@@ -118,8 +118,11 @@ or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
 #pragma unroll
     for (int i = 1; i < 4; ++i) k[i] += (double)U[2 * mu][i] - (double)U[2 * mu + 1][i];
   }
+  // the subgroup quaternion of the 2x2 K is p = 2k (the scale only matters to the heat bath, a = |p|/T)
+#pragma unroll
+  for (int i = 0; i < 4; ++i) k[i] *= 2.0;
   double Gd[4];
-  if (!su2_update_power<(sizeof(Real) == 8)>(k, omega, Gd)) return;   // K = 0: skip the update (C-9)
+  if (!su2_update_at<(sizeof(Real) == 8)>(k, omega, Gd, (uint32_t)canonical_site(g, h, sc), 0u)) return;   // K = 0: skip (C-9)
   const Real G[4] = {(Real)Gd[0], (Real)Gd[1], (Real)Gd[2], (Real)Gd[3]};
 #pragma unroll
   for (int l = 0; l < 8; ++l) {
@@ -166,6 +169,21 @@ cudaError_t launch_or_sweep_series(const LatticeDesc& d, void* links, int parity
     return launch_su2<Storage<double, 2, 4> >(links, d.geom, parity, pw, false, st);
   }
   return launch_or_sweep_staged_series(d, links, parity, pw, st);
+}
+
+// Simulated-annealing half-sweep at temperature T (reading C-25); production mappings only.
+cudaError_t launch_sa_sweep(const LatticeDesc& d, void* links, int parity, double T, unsigned long long seed,
+                            unsigned counter, cudaStream_t st) {
+  HeatBathPower pw;
+  pw.inv_T = 1.0 / T;
+  pw.seed_lo = (uint32_t)seed;
+  pw.seed_hi = (uint32_t)(seed >> 32);
+  pw.counter = counter;
+  if (d.group == 2) {
+    if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, d.geom, parity, pw, false, st);
+    return launch_su2<Storage<double, 2, 4> >(links, d.geom, parity, pw, false, st);
+  }
+  return launch_or_sweep_staged_heatbath(d, links, parity, pw, st);
 }
 
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,

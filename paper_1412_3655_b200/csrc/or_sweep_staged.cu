@@ -34,6 +34,7 @@ namespace culgt {
 __device__ __forceinline__ double power_omega(double w) { return w; }
 __device__ __forceinline__ double power_omega(const ExactPower& p) { return p.omega; }
 __device__ __forceinline__ double power_omega(const SeriesPower&) { return 0.0; }
+__device__ __forceinline__ double power_omega(const HeatBathPower&) { return 0.0; }
 
 // Option bits of the OPT template parameter.
 constexpr int OPT_PREFETCH = 1;    // persistent only: prefetch.global.L2 of the next site block
@@ -96,6 +97,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 template <int LPT>
 struct SiteRef {
   int idx[LPT];
+  unsigned site;   // canonical site index (selects the heat bath's random numbers)
   bool active;
 };
 
@@ -107,6 +109,7 @@ __device__ __forceinline__ SiteRef<8 / TPS> locate(const Geom& g, int parity, in
   r.active = h < g.vh;
   if (!r.active) h = g.vh - 1;
   const SiteCoord sc = decode_site(g, h, parity);
+  r.site = (unsigned)canonical_site(g, h, sc);
 #pragma unroll
   for (int l = 0; l < LPT; ++l) {
     const int slot = q * LPT + l;
@@ -257,8 +260,14 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
 #pragma unroll
         for (int i = 0; i < 18; ++i) { acc += Kd[i]; Gd[i] = (i == 0 || i == 8 || i == 16) ? 1.0 : 0.0; }
         Gd[1] = acc * 1e-300;      // keeps K alive
-      } else
-      su3_solve<(sizeof(Real) == 8), double>(Kd, Gd, omega);
+      } else if (cur.active) {
+        // idle lanes of a ragged last block hold uninitialised shared memory: they must not enter
+        // the solve (the heat bath's rejection loop would never end on NaN input)
+        su3_solve<(sizeof(Real) == 8), double>(Kd, Gd, omega, cur.site);
+      } else {
+#pragma unroll
+        for (int i = 0; i < 18; ++i) Gd[i] = 0.0;
+      }
 #pragma unroll
       for (int i = 0; i < 18; ++i) G[i] = (Real)Gd[i];
     } else {
@@ -410,9 +419,10 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
   }
 }
 
-// Truncated-series overrelaxation (reading C-24) on the production mapping of each format.
-cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int parity, const SeriesPower& pw,
-                                          cudaStream_t st) {
+// Truncated-series overrelaxation (reading C-24) / simulated annealing (C-25) on the production
+// mapping of each format.
+template <typename Power>
+static cudaError_t launch_production(const LatticeDesc& d, void* links, int parity, const Power& pw, cudaStream_t st) {
   const Geom& g = d.geom;
   if (d.group != 3) return cudaErrorInvalidValue;
   if (d.precision == 32 && d.params == 12)
@@ -422,6 +432,15 @@ cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int
   if (d.params == 12)
     return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT>(links, g, parity, pw, true, st);
   return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT>(links, g, parity, pw, true, st);
+}
+
+cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int parity, const SeriesPower& pw,
+                                          cudaStream_t st) {
+  return launch_production(d, links, parity, pw, st);
+}
+cudaError_t launch_or_sweep_staged_heatbath(const LatticeDesc& d, void* links, int parity, const HeatBathPower& pw,
+                                            cudaStream_t st) {
+  return launch_production(d, links, parity, pw, st);
 }
 
 }  // namespace culgt

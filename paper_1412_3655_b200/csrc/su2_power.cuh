@@ -17,6 +17,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <math.h>
+#include "heatbath.cuh"
 
 namespace culgt {
 
@@ -172,6 +173,26 @@ __device__ __forceinline__ bool su2_update_power(const double* p, const SeriesPo
   const double f = -wi * winv * rinv;                      // v/|v| = -pv/|pv|
   q[0] = wr * winv; q[1] = p[1] * f; q[2] = p[2] * f; q[3] = p[3] * f;
   return true;
+}
+
+// Uniform entry used by the solvers: (site, subgroup) select the random numbers of the heat bath
+// and are ignored by the deterministic powers.
+template <bool FULL>
+__device__ __forceinline__ bool su2_update_at(const double* p, double omega, double* q, uint32_t, uint32_t) {
+  return su2_update_power<FULL>(p, omega, q);
+}
+template <bool FULL>
+__device__ __forceinline__ bool su2_update_at(const double* p, const ExactPower& pw, double* q, uint32_t, uint32_t) {
+  return su2_update_power<FULL>(p, pw.omega, q);
+}
+template <bool FULL>
+__device__ __forceinline__ bool su2_update_at(const double* p, const SeriesPower& pw, double* q, uint32_t, uint32_t) {
+  return su2_update_power<FULL>(p, pw, q);
+}
+template <bool FULL>
+__device__ __forceinline__ bool su2_update_at(const double* p, const HeatBathPower& pw, double* q, uint32_t site,
+                                              uint32_t sub) {
+  return su2_heatbath(p, pw, site, sub, q);
 }
 
 }  // namespace culgt

@@ -18,13 +18,13 @@ namespace culgt {
 
 // p = real-quaternion part (x2) of the (I,J) block of K; q = (conj(p)/|p|)^omega.
 template <int I, int J, bool FULL, typename Power>
-__device__ __forceinline__ bool subgroup_quaternion(const double* K, const Power& omega, double* q) {
+__device__ __forceinline__ bool subgroup_quaternion(const double* K, const Power& omega, double* q, uint32_t site) {
   double p[4];
   p[0] = K[CULGT_RE(I, I)] + K[CULGT_RE(J, J)];
   p[1] = K[CULGT_IM(I, J)] + K[CULGT_IM(J, I)];
   p[2] = K[CULGT_RE(I, J)] - K[CULGT_RE(J, I)];
   p[3] = K[CULGT_IM(I, I)] - K[CULGT_IM(J, J)];
-  return su2_update_power<FULL>(p, omega, q);
+  return su2_update_at<FULL>(p, omega, q, site, (uint32_t)(I + J - 1));   // subgroups 0, 1, 2
 }
 
 // (x, y) <- (a x + b y, -conj(b) x + conj(a) y) for complex x = M[I][c], y = M[J][c];
@@ -51,12 +51,13 @@ __device__ __forceinline__ void rotate_col(T* M, int c, T ar, T ai, T br, T bi) 
 // K (fp64, destroyed) -> G (type GT).  g_s embeds q = (c, v1, v2, v3) as
 // [I][I] = a = c + i v3, [I][J] = b = v2 + i v1, [J][I] = -conj(b), [J][J] = conj(a)  (C-7).
 // FULL selects full-length (fp64 storage) or shortened (fp32 storage) series in su2_power.cuh.
-// Power = double (omega; exact power), ExactPower or SeriesPower (su2_power.cuh).
+// Power = double (omega; exact power), ExactPower, SeriesPower (su2_power.cuh) or HeatBathPower
+// (heatbath.cuh; `site` = canonical site index, selects its random numbers).
 template <bool FULL, typename GT, typename Power>
-__device__ __forceinline__ void su3_solve(double* K, GT* G, const Power& omega) {
+__device__ __forceinline__ void su3_solve(double* K, GT* G, const Power& omega, uint32_t site = 0) {
   double q[4];
   // ---- subgroup (0,1)
-  bool ok = subgroup_quaternion<0, 1, FULL>(K, omega, q);
+  bool ok = subgroup_quaternion<0, 1, FULL>(K, omega, q, site);
   if (!ok) { q[0] = 1.0; q[1] = 0.0; q[2] = 0.0; q[3] = 0.0; }
   {
     const double ar = q[0], ai = q[3], br = q[2], bi = q[1];
@@ -67,7 +68,7 @@ __device__ __forceinline__ void su3_solve(double* K, GT* G, const Power& omega) 
   // G = g_1
   const GT a1r = (GT)q[0], a1i = (GT)q[3], b1r = (GT)q[2], b1i = (GT)q[1];
   // ---- subgroup (0,2)
-  ok = subgroup_quaternion<0, 2, FULL>(K, omega, q);
+  ok = subgroup_quaternion<0, 2, FULL>(K, omega, q, site);
   if (!ok) { q[0] = 1.0; q[1] = 0.0; q[2] = 0.0; q[3] = 0.0; }
   {
     const double ar = q[0], ai = q[3], br = q[2], bi = q[1];
@@ -90,7 +91,7 @@ __device__ __forceinline__ void su3_solve(double* K, GT* G, const Power& omega) 
     G[CULGT_RE(2, 2)] = a2r;                    G[CULGT_IM(2, 2)] = -a2i;
   }
   // ---- subgroup (1,2)
-  ok = subgroup_quaternion<1, 2, FULL>(K, omega, q);
+  ok = subgroup_quaternion<1, 2, FULL>(K, omega, q, site);
   if (ok) {
     const GT ar = (GT)q[0], ai = (GT)q[3], br = (GT)q[2], bi = (GT)q[1];
 #pragma unroll
