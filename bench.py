@@ -2,6 +2,7 @@
 """bench.py -- SU(3) Landau overrelaxation throughput on B200 (BASELINE.json metric, configs[3]).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+                    [--gauge landau|coulomb] [--series-order N] [--sa-temperature T] [--variant V]
 
 A STEP is one full overrelaxation sweep (black half-sweep + white half-sweep = V site updates,
 PAPER.md L54) of the resident field; every --check-every steps the timed region also computes

@@ -88,6 +88,21 @@ def test_argument_errors_by_return_code():
     assert lib.culgt_landau_fix(ref, ok_ptr, ok_ptr, 1.7, 1e-10, 10, 0, None, None, None, None) == E["CULGT_ERR_ARG"]
     assert lib.culgt_fix_host(ref, None, ok_ptr, ok_ptr, ok_ptr, 1, 1.7, None, None, None) == E["CULGT_ERR_NULL"]
     assert lib.culgt_set_sweep_variant(-3) == E["CULGT_ERR_ARG"]
+    # the widened entry points (Coulomb gauge, series power, annealing, re-unitarisation, autotuner)
+    assert lib.culgt_or_sweep_coulomb(ref, None, 0, 1.7, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_or_sweep_coulomb(ref, ok_ptr, 3, 1.7, None) == E["CULGT_ERR_PARITY"]
+    assert lib.culgt_or_sweeps_coulomb(ref, ok_ptr, -1, 1.7, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_coulomb_precision_functional(ref, ok_ptr, ok_ptr, None, ok_ptr, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_coulomb_fix(ref, ok_ptr, ok_ptr, 1.7, 1e-10, 10, 0, None, None, None, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_or_sweep_series(ref, ok_ptr, 0, 1.7, 17, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_or_sweep_series(ref, ok_ptr, 0, 2.5, 4, None) == E["CULGT_ERR_OMEGA"]
+    assert lib.culgt_or_sweeps_series(ref, ok_ptr + 8, 1, 1.7, 4, None) == E["CULGT_ERR_ALIGN"]
+    assert lib.culgt_sa_sweep(ref, ok_ptr, 0, 0.0, 1, 0, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_sa_sweep(ref, ok_ptr, 2, 1.0, 1, 0, None) == E["CULGT_ERR_PARITY"]
+    assert lib.culgt_sa_anneal(ref, ok_ptr, 0.1, 1.0, 5, 1, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_reunitarize(ref, None, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_autotune_sweep(ref, ok_ptr, 1.7, 0, None, None, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_gauge_precision_functional(ref, ok_ptr, ok_ptr, ok_ptr, None, None) == E["CULGT_ERR_NULL"]
     for code in E.values():
         assert culgt.culgt_strerror(code) != "unknown status"
     assert culgt.culgt_strerror(-99) == "unknown status"
