@@ -1,4 +1,7 @@
-// or_sweep.cu -- the checkerboard overrelaxation half-sweep kernels.
+// or_sweep.cu -- half-sweep dispatch (launch_or_sweep and friends), the SU(2) kernel, and the first
+// generation of SU(3) kernels that keep all links in registers (variants 1-14, the measured
+// alternatives of DESIGN.md 6.1).  The production SU(3) kernel is in or_sweep_staged.cu.
+// (SURVEY.md 8(a) rows a1-a6.)
 //
 // For every site x of one parity:
 //   gather the 8 links touching x, K = sum_mu U_mu(x) + U_mu(x-mu)^dagger      (eq. 3)
