@@ -1,0 +1,48 @@
+"""The bench.py output contract on a GPU box: one JSON line with the keys the driver reads, for our
+arm (small step count) and for the reference arm."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def run(*args):
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *args], capture_output=True, text=True,
+                       timeout=900, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout[-2000:]
+    return json.loads(lines[0])
+
+
+def test_our_arm_json_line():
+    d = run("--steps", "6", "--warmup", "3", "--check-every", "3", "--workload", "cfg2")
+    assert d["metric"] == "su3_landau_or_site_updates_per_s" and d["unit"] == "site-updates/s"
+    assert d["n_gpus"] == 1 and d["steps"] == 6 and d["warmup"] >= 3 and d["higher_is_better"] is True
+    assert d["scaling"] == "weak" and d["vs_baseline"] is None and d["dtype"] == "f32" and d["data"] == "synthetic"
+    assert d["value"] > 0 and d["ms_per_step"] > 0
+    assert d["gpu_launches"] == 2 * 6 + 2 * 2          # half-sweeps + (partial, final) per check
+    assert "workload" in d["config"] and "model" not in d["config"]
+    r = d["roofline"]
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["peak"] > 1000
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    assert r["bytes_per_launch"] == 2 * 4 * 16 ** 4 * 48
+    e = d["e2e"]
+    assert e["unit"] == d["unit"] and e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
+    assert e["value"] != d["value"]
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["unit"] == d["unit"] and c["sample"]
+    assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    assert d["value"] > 20 * c["value"]               # the GPU path, not a CPU fallback
+
+
+def test_reference_arm_json_line():
+    d = run("--impl", "reference", "--steps", "2", "--warmup", "1", "--workload", "cfg2")
+    assert d["impl"] == "reference" and d["metric"] == "su3_landau_or_site_updates_per_s"
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"]
+    assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
