@@ -163,10 +163,16 @@ int culgt_sa_anneal(const culgt_lattice* lat, void* links, double T_max, double 
  *   t = x3 = 0..N3-1, Vs = N0*N1*N2.
  * culgt_or_sweep_coulomb / culgt_or_sweeps_coulomb: as the Landau calls.
  * culgt_coulomb_precision_functional: theta_t_dev, F_t_dev are DEVICE arrays of dims[3] doubles.
- * culgt_coulomb_fix: full sweeps until max_t theta_t < theta_target or max_sweeps; SYNCHRONISES at
- *   each check; theta_t_out / F_t_out: HOST arrays of dims[3] doubles (may be NULL). */
+ * culgt_or_sweep_coulomb_masked: the half-sweep over the time-slices t with slice_active_dev[t] != 0
+ *   only (DEVICE array of dims[3] bytes); slices decouple, so frozen slices keep their spatial links.
+ * culgt_coulomb_fix: every slice is swept until ITS theta_t < theta_target (checked every
+ *   check_every sweeps; converged slices are frozen, the others go on) or max_sweeps; SYNCHRONISES
+ *   at each check; sweeps_done = sweeps of the slowest slice; theta_t_out / F_t_out: HOST arrays of
+ *   dims[3] doubles (may be NULL). */
 int culgt_or_sweep_coulomb(const culgt_lattice* lat, void* links, int parity, double omega, void* stream);
 int culgt_or_sweeps_coulomb(const culgt_lattice* lat, void* links, int n_sweeps, double omega, void* stream);
+int culgt_or_sweep_coulomb_masked(const culgt_lattice* lat, void* links, int parity, double omega,
+                                  const unsigned char* slice_active_dev, void* stream);
 int culgt_coulomb_precision_functional(const culgt_lattice* lat, const void* links, void* workspace,
                                        double* theta_t_dev, double* F_t_dev, void* stream);
 int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, double omega,

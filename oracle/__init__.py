@@ -72,6 +72,8 @@ def _load():
     lib.oracle_delta_coulomb.argtypes = [i32p, ctypes.c_int, dp, dp]
     lib.oracle_or_sweep_coulomb.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double]
     lib.oracle_coulomb_theta_F.argtypes = [i32p, ctypes.c_int, dp, dp, dp]
+    lib.oracle_or_sweep_coulomb_masked.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double,
+                                                   ctypes.POINTER(ctypes.c_uint8)]
     _lib = lib
     return lib
 
@@ -201,6 +203,16 @@ def or_sweep_coulomb(dims, u: np.ndarray, parity: int, omega: float) -> None:
     """One Coulomb-gauge half-sweep, in place."""
     nc = _check_links(dims, u)
     _load().oracle_or_sweep_coulomb(_dims(dims), nc, _dp(u), int(parity), float(omega))
+
+
+def or_sweep_coulomb_masked(dims, u: np.ndarray, parity: int, omega: float, active) -> None:
+    """Coulomb half-sweep over the time-slices t with active[t] != 0 only."""
+    nc = _check_links(dims, u)
+    a = np.ascontiguousarray(active, dtype=np.uint8)
+    if a.shape != (int(dims[3]),):
+        raise ValueError("active must have dims[3] entries")
+    _load().oracle_or_sweep_coulomb_masked(_dims(dims), nc, _dp(u), int(parity), float(omega),
+                                           a.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8)))
 
 
 def full_sweep_coulomb(dims, u: np.ndarray, omega: float) -> None:

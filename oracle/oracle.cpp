@@ -472,6 +472,27 @@ void oracle_or_sweep_coulomb(const int32_t* dims, int nc, double* U, int parity,
   }
 }
 
+// The same half-sweep restricted to the time-slices with active[t] != 0 (slices decouple, so a
+// slice whose theta_t has reached the target can stop while the others go on; SURVEY.md 8(f) NEXT-1
+// "each slice its own theta_t and stop").  active is uint8[N3].
+void oracle_or_sweep_coulomb_masked(const int32_t* dims, int nc, double* U, int parity, double omega,
+                                    const uint8_t* active) {
+  Lat L = make_lat(dims, nc);
+  const int64_t Vs = (int64_t)L.N[0] * L.N[1] * L.N[2];
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    if (parity_of(L, s) != parity || !active[s / Vs]) continue;
+    Mat G = site_G(gather_K_spatial(U, L, s), omega, nc);
+    Mat Gd = dagger(G, nc);
+    for (int mu = 0; mu < 4; ++mu) {
+      double* up = link_ptr(U, L, s, mu);
+      store_mat(up, nc, mul(G, load_mat(up, nc), nc));
+      double* dn = link_ptr(U, L, neighbour(L, s, mu, -1), mu);
+      store_mat(dn, nc, mul(load_mat(dn, nc), Gd, nc));
+    }
+  }
+}
+
 // theta_t and F_t for every time-slice t = x3: both are double[N3].
 void oracle_coulomb_theta_F(const int32_t* dims, int nc, const double* U, double* theta_t, double* F_t) {
   Lat L = make_lat(dims, nc);

@@ -76,6 +76,7 @@ def lib() -> ctypes.CDLL:
     L.culgt_sa_sweep.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, ctypes.c_ulonglong, ctypes.c_uint, vp]
     L.culgt_sa_anneal.argtypes = [latp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_ulonglong, vp]
     L.culgt_or_sweep_coulomb.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
+    L.culgt_or_sweep_coulomb_masked.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp, vp]
     L.culgt_or_sweeps_coulomb.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_coulomb_precision_functional.argtypes = [latp, vp, vp, vp, vp, vp]
     L.culgt_coulomb_fix.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
@@ -299,6 +300,13 @@ def culgt_or_sweep_coulomb(lat: Lattice, links, parity: int, omega: float, strea
     _require_cuda()
     _check(lib().culgt_or_sweep_coulomb(ctypes.byref(lat.c()), _ptr(links), int(parity), float(omega),
                                         _stream(stream)), "culgt_or_sweep_coulomb")
+
+
+def culgt_or_sweep_coulomb_masked(lat: Lattice, links, parity: int, omega: float, slice_active, stream=None) -> None:
+    """slice_active: device uint8 tensor of dims[3] entries; slices with 0 are left untouched."""
+    _require_cuda()
+    _check(lib().culgt_or_sweep_coulomb_masked(ctypes.byref(lat.c()), _ptr(links), int(parity), float(omega),
+                                               _ptr(slice_active), _stream(stream)), "culgt_or_sweep_coulomb_masked")
 
 
 def culgt_or_sweeps_coulomb(lat: Lattice, links, n_sweeps: int, omega: float, stream=None) -> None:

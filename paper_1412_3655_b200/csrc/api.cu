@@ -4,6 +4,7 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <vector>
 #include "../../include/culgt_b200.h"
 #include "kernels.h"
 
@@ -340,6 +341,20 @@ int culgt_or_sweep_coulomb(const culgt_lattice* lat, void* links, int parity, do
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
+int culgt_or_sweep_coulomb_masked(const culgt_lattice* lat, void* links, int parity, double omega,
+                                  const unsigned char* slice_active_dev, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !slice_active_dev) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (parity != 0 && parity != 1) return CULGT_ERR_PARITY;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  d.geom.slice_active = slice_active_dev;
+  cudaError_t e = launch_or_sweep(d, links, parity, omega, 0, (cudaStream_t)stream, true);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
 int culgt_or_sweeps_coulomb(const culgt_lattice* lat, void* links, int n_sweeps, double omega, void* stream) {
   LatticeDesc d;
   int rc = describe(lat, &d);
@@ -368,35 +383,17 @@ int culgt_coulomb_precision_functional(const culgt_lattice* lat, const void* lin
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
-// max_t theta_t and mean_t F_t through the result slots of the workspace (synchronises).
-static int read_coulomb(const LatticeDesc& d, const void* links, void* workspace, cudaStream_t st,
-                        double* theta_max, double* F_mean, double* theta_t_host, double* F_t_host) {
+// theta_t and F_t of every slice through the result slots of the workspace into host[0..2*N3)
+// (synchronises).
+static int read_coulomb(const LatticeDesc& d, const void* links, void* workspace, cudaStream_t st, double* host) {
   const int n3 = d.geom.n[3];
   double* ws = (double*)workspace;
   double* res = ws + reduce_partial_doubles(d.geom);
   cudaError_t e = launch_coulomb_theta_functional(d, links, ws, res, res + n3, st);
   if (e != cudaSuccess) return cuda_fail(e);
-  double stack_buf[512];
-  double* host = (2 * n3 <= 512) ? stack_buf : (double*)malloc(2 * (size_t)n3 * sizeof(double));
-  if (!host) return CULGT_ERR_ARG;
   e = cudaMemcpyAsync(host, res, 2 * (size_t)n3 * sizeof(double), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  int rc = CULGT_OK;
-  if (e != cudaSuccess) {
-    rc = cuda_fail(e);
-  } else {
-    double tmax = 0, fsum = 0;
-    for (int t = 0; t < n3; ++t) {
-      if (host[t] > tmax || host[t] != host[t]) tmax = host[t];
-      fsum += host[n3 + t];
-      if (theta_t_host) theta_t_host[t] = host[t];
-      if (F_t_host) F_t_host[t] = host[n3 + t];
-    }
-    *theta_max = tmax;
-    *F_mean = fsum / n3;
-  }
-  if (host != stack_buf) free(host);
-  return rc;
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
 int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, double omega,
@@ -410,21 +407,39 @@ int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, do
   if (max_sweeps < 0 || check_every < 1) return CULGT_ERR_ARG;
   if ((rc = check_omega(omega)) != CULGT_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  double tmax = 0, fmean = 0;
+  const int n3 = d.geom.n[3];
+  std::vector<double> host(2 * (size_t)n3);
+  std::vector<unsigned char> active((size_t)n3, 1);
+  // the per-slice activity mask lives behind the result slots of the workspace
+  unsigned char* mask_dev = (unsigned char*)((double*)workspace + reduce_partial_doubles(d.geom) + 2 * (size_t)n3);
   int done = 0;
-  if ((rc = read_coulomb(d, links, workspace, st, &tmax, &fmean, theta_t_out, F_t_out)) != CULGT_OK) return rc;
-  while (tmax >= theta_target && done < max_sweeps) {
+  for (;;) {
+    if ((rc = read_coulomb(d, links, workspace, st, host.data())) != CULGT_OK) return rc;
+    // slices decouple: a slice whose theta_t is below the target stops, the others go on
+    int n_active = 0;
+    for (int t = 0; t < n3; ++t) {
+      active[t] = !(host[t] < theta_target);          // NaN keeps a slice active until max_sweeps
+      n_active += active[t];
+    }
+    if (n_active == 0 || done >= max_sweeps) break;
+    cudaError_t e = cudaMemcpyAsync(mask_dev, active.data(), (size_t)n3, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    LatticeDesc dm = d;
+    dm.geom.slice_active = mask_dev;
     int n = check_every;
     if (done + n > max_sweeps) n = max_sweeps - done;
     for (int i = 0; i < n; ++i)
       for (int parity = 0; parity < 2; ++parity) {
-        cudaError_t e = launch_or_sweep(d, links, parity, omega, 0, st, true);
+        e = launch_or_sweep(dm, links, parity, omega, 0, st, true);
         if (e != cudaSuccess) return cuda_fail(e);
       }
     done += n;
-    if ((rc = read_coulomb(d, links, workspace, st, &tmax, &fmean, theta_t_out, F_t_out)) != CULGT_OK) return rc;
   }
   if (sweeps_done) *sweeps_done = done;
+  for (int t = 0; t < n3; ++t) {
+    if (theta_t_out) theta_t_out[t] = host[t];
+    if (F_t_out) F_t_out[t] = host[n3 + t];
+  }
   return CULGT_OK;
 }
 

@@ -25,7 +25,10 @@ inline size_t reduce_partial_doubles(const Geom& g) {
   if (c > n) n = c;
   return n > 4096 ? n : 4096;
 }
-inline size_t reduce_workspace_doubles(const Geom& g) { return reduce_partial_doubles(g) + 2 * (size_t)g.n[3]; }
+// ... and N3 bytes (rounded up to doubles) for the Coulomb driver's per-slice activity mask
+inline size_t reduce_workspace_doubles(const Geom& g) {
+  return reduce_partial_doubles(g) + 2 * (size_t)g.n[3] + ((size_t)g.n[3] + 7) / 8;
+}
 
 // coulomb = true: Coulomb-gauge half-sweep (K from the spatial links; production mapping only)
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,

@@ -33,6 +33,9 @@ struct Geom {
   int32_t vh;        // V/2 sites per parity
   int32_t stride[4]; // half-index strides: 1 (unused for mu=0), N0/2, N0/2*N1, N0/2*N1*N2
   FastDiv d_nh0, d_n1, d_n2;
+  // Coulomb gauge only: device array of N3 bytes, a site of time-slice t is swept iff
+  // slice_active[t] != 0; nullptr = every slice (set by the API layer per call)
+  const unsigned char* slice_active;
 };
 
 inline Geom make_geom(const int32_t dims[4]) {
@@ -47,6 +50,7 @@ inline Geom make_geom(const int32_t dims[4]) {
   g.d_nh0.init((uint32_t)g.nh0);
   g.d_n1.init((uint32_t)dims[1]);
   g.d_n2.init((uint32_t)dims[2]);
+  g.slice_active = nullptr;
   return g;
 }
 

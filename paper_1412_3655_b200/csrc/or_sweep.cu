@@ -104,6 +104,7 @@ or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
   const int h = blk * BLOCK + threadIdx.x;
   if (h >= g.vh) return;
   const SiteCoord sc = decode_site(g, h, parity);
+  if (COULOMB && g.slice_active != nullptr && g.slice_active[sc.x3] == 0) return;   // frozen slice
   Real U[8][4];
   typename S::Vec* ptr[8];
 #pragma unroll

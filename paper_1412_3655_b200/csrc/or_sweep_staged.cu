@@ -101,7 +101,7 @@ struct SiteRef {
   bool active;
 };
 
-template <int BLOCK, int TPS>
+template <int BLOCK, int TPS, bool MASKED>
 __device__ __forceinline__ SiteRef<8 / TPS> locate(const Geom& g, int parity, int site_block, int q) {
   constexpr int LPT = 8 / TPS;
   SiteRef<LPT> r;
@@ -110,6 +110,7 @@ __device__ __forceinline__ SiteRef<8 / TPS> locate(const Geom& g, int parity, in
   if (!r.active) h = g.vh - 1;
   const SiteCoord sc = decode_site(g, h, parity);
   r.site = (unsigned)canonical_site(g, h, sc);
+  if (MASKED && g.slice_active != nullptr && g.slice_active[sc.x3] == 0) r.active = false;   // frozen slice
 #pragma unroll
   for (int l = 0; l < LPT; ++l) {
     const int slot = q * LPT + l;
@@ -177,7 +178,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
   if (n_it <= 0) return;
 
   // prologue: STAGES-1 sites in flight
-  SiteRef<LPT> cur = locate<BLOCK, TPS>(g, parity, block_of(0), q);
+  SiteRef<LPT> cur = locate<BLOCK, TPS, (OPT & OPT_COULOMB) != 0>(g, parity, block_of(0), q);
   SiteRef<LPT> nxt = cur;
   if (STAGES == 1) {
     // nothing in flight yet
@@ -192,7 +193,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
       if ((OPT & OPT_PREFETCH) && it + 1 < n_it) {
         // pull the NEXT site block's lines into L2 while this one is computed: the blocking
         // cp.async of the next iteration then pays L2 latency, not HBM latency
-        nxt = locate<BLOCK, TPS>(g, parity, block_of(it + 1), q);
+        nxt = locate<BLOCK, TPS, (OPT & OPT_COULOMB) != 0>(g, parity, block_of(it + 1), q);
         if (nxt.active) {
 #pragma unroll
           for (int l = 0; l < LPT; ++l)
@@ -203,7 +204,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
       cp_async_wait<0>();
     } else {
       if (it + 1 < n_it) {
-        nxt = locate<BLOCK, TPS>(g, parity, block_of(it + 1), q);
+        nxt = locate<BLOCK, TPS, (OPT & OPT_COULOMB) != 0>(g, parity, block_of(it + 1), q);
         issue(nxt, stage ^ 1);
         cp_async_wait<1>();
       } else {
@@ -301,7 +302,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
       }
     }
     if (STAGES == 1 && !(OPT & OPT_PREFETCH)) {
-      if (it + 1 < n_it) cur = locate<BLOCK, TPS>(g, parity, block_of(it + 1), q);
+      if (it + 1 < n_it) cur = locate<BLOCK, TPS, (OPT & OPT_COULOMB) != 0>(g, parity, block_of(it + 1), q);
     } else {
       cur = nxt;
     }

@@ -104,6 +104,42 @@ def test_headline_size_links_after_one_sweep(name):
         assert np.all(np.abs(th - th_o) <= 1e-3 * th_o) and np.all(np.abs(F - F_o) <= 2e-6)
 
 
+def test_masked_sweep_and_per_slice_stopping():
+    """Frozen slices keep their spatial links, active ones are swept exactly as by the oracle; the
+    driver stops every slice at ITS theta_t like the same rule applied to
+    the oracle."""
+    dims = (6, 4, 4, 8)
+    u = li.make_config(dims, 3, "near_identity", 83, eps=0.3, scramble=True)
+    ref = storage_input(u, 64, 18)
+    f = GpuField(dims, 3, 64, 18, u)
+    active = np.array([1, 0, 1, 1, 0, 0, 1, 0], dtype=np.uint8)
+    mask = torch.from_numpy(active).cuda()
+    for parity in (0, 1):
+        oracle.or_sweep_coulomb_masked(dims, ref, parity, 1.7, active)
+        culgt.culgt_or_sweep_coulomb_masked(f.lat, f.links, parity, 1.7, mask)
+    assert np.abs(f.download() - li.from_real(ref)).max() < TOL_LINK[64]
+    # per-slice stopping, theta checked after every sweep
+    target = 1e-16
+    ref = storage_input(u, 64, 18)
+    stop_o = np.zeros(dims[3], dtype=int)
+    n = 0
+    while True:
+        th_o, F_o = oracle.coulomb_theta_F(dims, ref)
+        act = (~(th_o < target)).astype(np.uint8)
+        if act.sum() == 0 or n >= 3000:
+            break
+        for parity in (0, 1):
+            oracle.or_sweep_coulomb_masked(dims, ref, parity, 1.7, act)
+        n += 1
+        stop_o[act == 1] = n
+    f = GpuField(dims, 3, 64, 18, u)
+    done, th, F = culgt.culgt_coulomb_fix(f.lat, f.links, f.ws, 1.7, target, 3000, 1)
+    assert abs(done - n) <= 1 and max(th) < target
+    assert len(set(stop_o)) > 1                              # the slices really stop at different sweeps
+    assert np.abs(np.array(F) - F_o).max() < 1e-9
+    assert np.abs(f.download() - li.from_real(ref)).max() < 1e-6   # same copy reached (a +-1 sweep near the target moves links by ~sqrt(target))
+
+
 def test_argument_errors():
     lat = culgt.Lattice((4, 4, 4, 4), 3, 64, 18)
     links = culgt.alloc_links(lat)

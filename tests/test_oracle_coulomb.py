@@ -171,6 +171,25 @@ def test_pure_gauge_reaches_the_vacuum_in_every_slice(group, seed):
     assert np.abs(c @ dag(c) - np.eye(group)).max() < 1e-13
 
 
+def test_masked_sweep_freezes_inactive_slices_and_matches_the_full_sweep_elsewhere():
+    u = scrambled(DIMS, 3, 79)
+    t = slice_of(DIMS)
+    active = np.array([1, 0, 1, 1, 0, 0, 1, 0], dtype=np.uint8)
+    a, b = real(u), real(u)
+    for parity in (0, 1):
+        oracle.or_sweep_coulomb_masked(DIMS, a, parity, 1.7, active)
+        oracle.or_sweep_coulomb(DIMS, b, parity, 1.7)
+    for k in range(DIMS[3]):
+        if active[k]:      # spatial links of an active slice: exactly the unmasked sweep (slices decouple)
+            assert np.array_equal(a[t == k, :3], b[t == k, :3])
+        else:              # spatial links of a frozen slice: untouched
+            assert np.array_equal(a[t == k, :3], real(u)[t == k, :3])
+    assert abs(oracle.plaquette(DIMS, a) - oracle.plaquette(DIMS, real(u))) < 1e-12
+    none = real(u)
+    oracle.or_sweep_coulomb_masked(DIMS, none, 0, 1.7, np.zeros(DIMS[3], dtype=np.uint8))
+    assert np.array_equal(none, real(u))
+
+
 def test_threads_do_not_change_results():
     u = scrambled(DIMS, 3, 78)
     a, b = real(u), real(u)
