@@ -62,6 +62,27 @@ def test_anneal_schedule_and_overrelax_reaches_the_maximum():
     assert theta < 1e-22 and F > 0.999999
 
 
+@pytest.mark.parametrize("name", ["cfg3_fp32", "cfg3_fp64"])
+def test_headline_size_one_sweep(name):
+    """32^4 in the launch configuration `bench.py --sa-temperature` times: all 4V links after a black and
+    a white annealing half-sweep at T = 0.5, each from a common stored state."""
+    c = li.CONFIGS[name]
+    dims, prec = c["dims"], c["precision"]
+    u = li.make_named(name)
+    f = GpuField(dims, 3, prec, c["params"], u)
+    del u
+    oracle.set_threads(16)
+    try:
+        for n in range(2):
+            ref = li.to_real(np.ascontiguousarray(f.download()))
+            oracle.sa_sweep(dims, ref, n, 0.5, 31, n)
+            culgt.culgt_sa_sweep(f.lat, f.links, n, 0.5, 31, n)
+            err = np.abs(f.download() - li.from_real(ref)).max()
+            assert err < TOL_LINK[prec], (n, err)
+    finally:
+        oracle.set_threads(1)
+
+
 def test_argument_errors():
     lat = culgt.Lattice((4, 4, 4, 4), 3, 64, 18)
     links = culgt.alloc_links(lat)
