@@ -661,8 +661,8 @@ void oracle_or_sweep_series(const int32_t* dims, int nc, double* U, int parity, 
 // in [e^{-2a}, 1], accepted with probability sqrt(1 - h_0^2).
 // Random numbers: the counter-based Philox4x32-10 generator (Salmon et al., SC'11), restated here;
 // counter = (canonical site, half-sweep counter, subgroup | draw << 8, 0), key = 64-bit seed, so a
-// site's numbers do not depend on the traversal order or the thread count.  Uniforms in (0,1]:
-// 53 bits from two 32-bit words.
+// site's numbers do not depend on the traversal order or the thread count.  Uniforms in (0,1):
+// u = (w + 1/2) 2^-32 from each 32-bit word, one Philox block (4 uniforms) per trial / per direction.
 // ---------------------------------------------------------------------------------------------
 namespace {
 void philox4x32_10(const uint32_t ctr_in[4], const uint32_t key_in[2], uint32_t out[4]) {
@@ -682,21 +682,20 @@ void philox4x32_10(const uint32_t ctr_in[4], const uint32_t key_in[2], uint32_t 
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// two uniforms in (0,1] from one Philox block
-void uniforms2(const uint32_t w[4], double u[2]) {
-  u[0] = ((double)(((uint64_t)(w[0] >> 5) << 26) + (w[1] >> 6)) + 1.0) * (1.0 / 9007199254740992.0);
-  u[1] = ((double)(((uint64_t)(w[2] >> 5) << 26) + (w[3] >> 6)) + 1.0) * (1.0 / 9007199254740992.0);
+// four uniforms in (0,1) from one Philox block: u_i = (w_i + 1/2) 2^-32
+void uniforms4(const uint32_t w[4], double u[4]) {
+  for (int i = 0; i < 4; ++i) u[i] = ((double)w[i] + 0.5) * (1.0 / 4294967296.0);
 }
 
 struct SiteRng {
   uint32_t ctr[4];
   uint32_t key[2];
   uint32_t draw;
-  void next2(double u[2]) {
+  void next4(double u[4]) {
     uint32_t c[4] = {ctr[0], ctr[1], ctr[2] | (draw << 8), ctr[3]};
     uint32_t w[4];
     philox4x32_10(c, key, w);
-    uniforms2(w, u);
+    uniforms4(w, u);
     ++draw;
   }
 };
@@ -711,8 +710,8 @@ void su2_heatbath(const double p[4], double n, double T, SiteRng* rng, double q[
     // on [-1, 1]; accept with probability sqrt(1 - h_0^2)
     const double emin = std::exp(-2.0 * a);
     for (;;) {
-      double u[2];
-      rng->next2(u);
+      double u[4];
+      rng->next4(u);                                   // one block per trial (u[2], u[3] unused)
       double x = emin + u[0] * (1.0 - emin);
       h0 = 1.0 + std::log(x) / a;
       if (u[1] * u[1] <= 1.0 - h0 * h0) break;
@@ -720,17 +719,16 @@ void su2_heatbath(const double p[4], double n, double T, SiteRng* rng, double q[
   } else {
     double lam2;
     for (;;) {
-      double u[2], v[2];
-      rng->next2(u);                                   // r1, r2
-      rng->next2(v);                                   // r3, r4
+      double u[4];
+      rng->next4(u);                                   // r1, r2, r3, r4: one block per trial
       double c = std::cos(2.0 * M_PI * u[1]);
-      lam2 = -(std::log(u[0]) + c * c * std::log(v[0])) / (2.0 * a);
-      if (v[1] * v[1] <= 1.0 - lam2) break;
+      lam2 = -(std::log(u[0]) + c * c * std::log(u[2])) / (2.0 * a);
+      if (u[3] * u[3] <= 1.0 - lam2) break;
     }
     h0 = 1.0 - 2.0 * lam2;
   }
-  double u[2];
-  rng->next2(u);                                     // direction of the vector part
+  double u[4];
+  rng->next4(u);                                     // direction of the vector part (u[2], u[3] unused)
   double ct = 2.0 * u[0] - 1.0;
   double st = std::sqrt(std::fmax(0.0, 1.0 - ct * ct));
   double phi = 2.0 * M_PI * u[1];

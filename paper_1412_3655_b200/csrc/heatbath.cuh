@@ -31,13 +31,16 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// two uniforms in (0,1], 53 bits each, from the block with draw index `draw`
+// four uniforms in (0,1), u_i = (w_i + 1/2) 2^-32, from the block with draw index `draw`.  The
+// 32-bit word is widened exactly by the 2^52 exponent trick (an FP64 add instead of a conversion
+// on the slow XU pipe).
 __device__ __forceinline__ void heatbath_uniforms(const HeatBathPower& pw, uint32_t site, uint32_t sub,
-                                                  uint32_t draw, double* u0, double* u1) {
+                                                  uint32_t draw, double* u) {
   uint32_t w[4];
   philox4x32_10(site, pw.counter, sub | (draw << 8), 0u, pw.seed_lo, pw.seed_hi, w);
-  *u0 = ((double)(((uint64_t)(w[0] >> 5) << 26) + (w[1] >> 6)) + 1.0) * (1.0 / 9007199254740992.0);
-  *u1 = ((double)(((uint64_t)(w[2] >> 5) << 26) + (w[3] >> 6)) + 1.0) * (1.0 / 9007199254740992.0);
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+    u[i] = (__hiloint2double(0x43300000, (int)w[i]) - 4503599627370496.0 + 0.5) * (1.0 / 4294967296.0);
 }
 
 // q sampled for the un-normalised subgroup quaternion p; false when p == 0 (no update, C-9).
@@ -54,28 +57,28 @@ __device__ __forceinline__ bool su2_heatbath(const double* p, const HeatBathPowe
     const double emin = exp(-2.0 * a);
     for (;;) {
       if (draw >= (1u << 22)) { h0 = 1.0; break; }       // unreachable; never spin forever
-      double r1, r2;
-      heatbath_uniforms(pw, site, sub, draw, &r1, &r2);
+      double u[4];
+      heatbath_uniforms(pw, site, sub, draw, u);
       draw += 1;
-      h0 = 1.0 + log(emin + r1 * (1.0 - emin)) / a;
-      if (r2 * r2 <= 1.0 - h0 * h0) break;
+      h0 = 1.0 + log(emin + u[0] * (1.0 - emin)) / a;
+      if (u[1] * u[1] <= 1.0 - h0 * h0) break;
     }
   } else {
     double lam2;
     for (;;) {
       if (draw >= (1u << 22)) { lam2 = 0.0; break; }     // unreachable for finite a; never spin forever
-      double r1, r2, r3, r4;
-      heatbath_uniforms(pw, site, sub, draw, &r1, &r2);
-      heatbath_uniforms(pw, site, sub, draw + 1, &r3, &r4);
-      draw += 2;
-      const double c = cospi(2.0 * r2);
-      lam2 = -(log(r1) + c * c * log(r3)) / (2.0 * a);
-      if (r4 * r4 <= 1.0 - lam2) break;
+      double u[4];
+      heatbath_uniforms(pw, site, sub, draw, u);         // r1, r2, r3, r4: one block per trial
+      draw += 1;
+      const double c = cospi(2.0 * u[1]);
+      lam2 = -(log(u[0]) + c * c * log(u[2])) / (2.0 * a);
+      if (u[3] * u[3] <= 1.0 - lam2) break;
     }
     h0 = 1.0 - 2.0 * lam2;
   }
-  double u0, u1;
-  heatbath_uniforms(pw, site, sub, draw, &u0, &u1);
+  double ud[4];
+  heatbath_uniforms(pw, site, sub, draw, ud);
+  const double u0 = ud[0], u1 = ud[1];
   const double ct = 2.0 * u0 - 1.0;
   const double st = sqrt(fmax(0.0, 1.0 - ct * ct));
   double sp, cp;
