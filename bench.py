@@ -337,7 +337,8 @@ def main():
     sweep_launches = 2 * args.steps
     gpu_launches = sweep_launches + n_checks * 2        # fused theta+F: partial + final kernel
     launch_ms = (elapsed_ms - check_ms) / sweep_launches
-    field_bytes = culgt.culgt_links_bytes(lat)
+    # algorithmic bytes: the stored parameters (fp32-18 keeps 2 pad floats per link that are not counted)
+    field_bytes = 4 * V * cfg["params"] * (cfg["precision"] // 8)
     alg_bytes_per_launch = 2 * field_bytes
     achieved_gbs = alg_bytes_per_launch / (launch_ms * 1e-3) / 1e9
     peak, peak_src = measured_peak()

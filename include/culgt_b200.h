@@ -27,7 +27,7 @@
  *   INTERNAL field   : links[parity][mu][j][h], parity-split, site-fastest structure of arrays
  *                      ("site index runs faster than Lorentz and matrix indices") of
  *                      vectors: SU(3) 12-parameter fp32 = 3 x float4, fp64 = 6 x double2;
- *                      18-parameter fp32 = 9 x float2, fp64 = 9 x double2; SU(2) 4-parameter
+ *                      18-parameter fp32 = 5 x float4 (the last half used), fp64 = 9 x double2; SU(2) 4-parameter
  *                      fp32 = 1 x float4 (a0,a1,a2,a3), fp64 = 2 x double2.  h = s>>1 is the
  *                      index of the site inside its parity.  Opaque to the caller: use
  *                      culgt_pack / culgt_unpack.  `real` = float (precision 32) or double (64)
@@ -61,7 +61,8 @@ typedef struct {
 } culgt_lattice;
 
 /* Sizes in bytes; 0 if the descriptor is invalid. */
-size_t culgt_links_bytes(const culgt_lattice* lat);      /* internal field: 4*V*params*sizeof(real) */
+size_t culgt_links_bytes(const culgt_lattice* lat);      /* internal field: 4*V*params*sizeof(real)
+                                                            (fp32 18-parameter: 4*V*80, 2 pad floats) */
 size_t culgt_canonical_bytes(const culgt_lattice* lat);  /* V*4*Nc*Nc*2*sizeof(real)                */
 size_t culgt_gfield_bytes(const culgt_lattice* lat);     /* V*Nc*Nc*2*sizeof(real)                  */
 size_t culgt_workspace_bytes(const culgt_lattice* lat);  /* reductions: block partials + 2 scalars;

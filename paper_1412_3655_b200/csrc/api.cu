@@ -54,7 +54,10 @@ int culgt_validate(const culgt_lattice* lat) { return describe(lat, nullptr); }
 size_t culgt_links_bytes(const culgt_lattice* lat) {
   LatticeDesc d;
   if (describe(lat, &d) != CULGT_OK) return 0;
-  return (size_t)4 * (size_t)d.V * (size_t)d.params * (size_t)(d.precision / 8);
+  // fp32 18-parameter links are stored as 5 float4 (80 bytes, 2 pad floats): 16-byte accesses
+  const size_t link_bytes = (d.group == 3 && d.precision == 32 && d.params == 18)
+                                ? 80 : (size_t)d.params * (size_t)(d.precision / 8);
+  return (size_t)4 * (size_t)d.V * link_bytes;
 }
 
 size_t culgt_canonical_bytes(const culgt_lattice* lat) {

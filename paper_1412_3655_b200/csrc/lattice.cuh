@@ -2,7 +2,7 @@
 //
 // Internal field ("reorder the lattice into its black and white sublattices ...
 // the site index runs faster than Lorentz and matrix indices"; L103: "three float4"):
-//     links[parity][mu][j][h]   vectors of 16 bytes (8 for fp32 18-parameter),
+//     links[parity][mu][j][h]   vectors of 16 bytes (fp32 18-parameter: 5 float4, the last half used),
 // h = canonical_site >> 1 = x0/2 + (N0/2)*(x1 + N1*(x2 + N2*x3)), valid because N0 is even.
 // Every [parity][mu][j] plane is a contiguous run of V/2 vectors, so a warp that walks
 // consecutive h reads consecutive addresses in every plane.
@@ -104,11 +104,14 @@ __device__ __forceinline__ int64_t canonical_site(const Geom& g, int h, const Si
   return 2 * (int64_t)h + c.odd;   // h enumerates pairs (2k, 2k+1) of the canonical order
 }
 
+// Registers of a link as loaded / stored through its vectors (>= 18 matrix reals, >= NPAD).
+constexpr int kLinkRegs = 20;
+
 // ---- storage traits: how one link is cut into vectors ---------------------------------------
 template <typename Real, int NP> struct VecOf;
 template <> struct VecOf<float, 12> { typedef float4 type; };
 template <> struct VecOf<float, 4>  { typedef float4 type; };
-template <> struct VecOf<float, 18> { typedef float2 type; };
+template <> struct VecOf<float, 18> { typedef float4 type; };   // 18 floats in 5 float4 (2 pad floats)
 template <> struct VecOf<double, 12> { typedef double2 type; };
 template <> struct VecOf<double, 18> { typedef double2 type; };
 template <> struct VecOf<double, 4>  { typedef double2 type; };
@@ -120,15 +123,14 @@ struct Storage {
   static constexpr int NC = NC_;                       // 2 or 3
   static constexpr int NP = NP_;                       // reals stored per link
   static constexpr int VL = sizeof(Vec) / sizeof(Real_);  // reals per vector
-  static constexpr int NV = NP_ / VL;                  // vectors per link
+  static constexpr int NV = (NP_ + VL - 1) / VL;       // vectors per link (fp32-18: 5, last half used)
+  static constexpr int NPAD = NV * VL;                 // reals moved per link (= NP except fp32-18: 20)
   static constexpr int NFULL = 2 * NC_ * NC_;          // reals of the full matrix
 };
 
 __device__ __forceinline__ void vec_get(const float4& v, float* r) { r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
-__device__ __forceinline__ void vec_get(const float2& v, float* r) { r[0] = v.x; r[1] = v.y; }
 __device__ __forceinline__ void vec_get(const double2& v, double* r) { r[0] = v.x; r[1] = v.y; }
 __device__ __forceinline__ void vec_set(float4& v, const float* r) { v = make_float4(r[0], r[1], r[2], r[3]); }
-__device__ __forceinline__ void vec_set(float2& v, const float* r) { v = make_float2(r[0], r[1]); }
 __device__ __forceinline__ void vec_set(double2& v, const double* r) { v = make_double2(r[0], r[1]); }
 
 // Pointer to vector j=0 of link (parity, mu, h); vector j is at +j*vh.

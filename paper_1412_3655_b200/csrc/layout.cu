@@ -22,9 +22,9 @@ layout_kernel(typename S::Real* __restrict__ canonical, typename S::Vec* __restr
   Real* cptr = canonical + (s * 4 + mu) * S::NFULL;
   typename S::Vec* lptr = link_base<S>(links, g, parity, mu, h);
   if (PACK) {
-    Real m[S::NFULL];
+    Real m[kLinkRegs];
 #pragma unroll
-    for (int i = 0; i < S::NFULL; ++i) m[i] = cptr[i];
+    for (int i = 0; i < kLinkRegs; ++i) m[i] = i < S::NFULL ? cptr[i] : (Real)0;   // pad reals stay 0
     if (S::NC == 3) {
       store_params<S>(lptr, g.vh, m);              // first NP reals = first NP/6 rows
     } else {
@@ -34,7 +34,7 @@ layout_kernel(typename S::Real* __restrict__ canonical, typename S::Vec* __restr
     }
   } else {
     if (S::NC == 3) {
-      Real m[18];
+      Real m[kLinkRegs];
       load_params<S>(lptr, g.vh, m);
       if (S::NP == 12) reconstruct_row2(m);
 #pragma unroll
@@ -89,7 +89,7 @@ reunitarize_kernel(typename S::Vec* __restrict__ links, const Geom g) {
   const int pm = (int)(t / g.vh);
   const int h = (int)(t - (long long)pm * g.vh);
   typename S::Vec* p = links + ((size_t)pm * S::NV) * (size_t)g.vh + (size_t)h;
-  Real r[S::NP];
+  Real r[kLinkRegs];
   load_params<S>(p, g.vh, r);
   if (S::NC == 2) {
     double a[4] = {(double)r[0], (double)r[1], (double)r[2], (double)r[3]};

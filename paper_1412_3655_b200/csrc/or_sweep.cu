@@ -43,7 +43,7 @@ or_sweep_su3_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
   if (!active) h = g.vh - 1;     // keep the lane alive for the shuffles; it stores nothing
   const SiteCoord sc = decode_site(g, h, parity);
 
-  Real U[LPT][18];
+  Real U[LPT][kLinkRegs];
   typename S::Vec* ptr[LPT];
 #pragma unroll
   for (int l = 0; l < LPT; ++l) {
@@ -81,7 +81,8 @@ or_sweep_su3_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
   constexpr int NR = (S::NP == 12) ? 2 : 3;   // rows that are stored
 #pragma unroll
   for (int l = 0; l < LPT; ++l) {
-    Real R[18];
+    Real R[kLinkRegs];
+    R[18] = 0; R[19] = 0;
     if (((q * LPT + l) & 1) == 0) mul_ab<NR>(G, U[l], R);
     else mul_abd<NR>(U[l], G, R);
     store_params<S>(ptr[l], g.vh, R);

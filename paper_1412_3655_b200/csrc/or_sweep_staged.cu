@@ -53,10 +53,6 @@ __device__ __forceinline__ void cp_async_vec(double2* smem, const double2* gmem)
   const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
 }
-__device__ __forceinline__ void cp_async_vec(float2* smem, const float2* gmem) {
-  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem) : "memory");
-}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 // Shared-memory reads as asm.  VOL = true emits ld.volatile: ptxas otherwise recognises the apply
 // pass's reads as repeats of the K pass's reads and keeps all 8 links live in registers across the
@@ -71,19 +67,11 @@ __device__ __forceinline__ void lds_vec(unsigned addr, double2& v) {
   if (VOL) asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
   else asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
 }
-template <bool VOL>
-__device__ __forceinline__ void lds_vec(unsigned addr, float2& v) {
-  if (VOL) asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
-  else asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
-}
 __device__ __forceinline__ void st_cs(float4* p, const float4& v) {
   asm volatile("st.global.cs.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 __device__ __forceinline__ void st_cs(double2* p, const double2& v) {
   asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
-}
-__device__ __forceinline__ void st_cs(float2* p, const float2& v) {
-  asm volatile("st.global.cs.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.x), "f"(v.y) : "memory");
 }
 __device__ __forceinline__ void prefetch_l2(const void* gmem) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(gmem));
@@ -224,7 +212,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
 #pragma unroll
     for (int l = 0; l < LPT; ++l) {
       if ((OPT & OPT_COULOMB) && ((q * LPT + l) >> 1) == 3) continue;   // time links do not enter K_C
-      Real U[18];
+      Real U[kLinkRegs];
       asm volatile("" ::: "memory");   // keep the shared-memory reads of link l behind link l-1's use
       load_link(stage, l, U, std::false_type());
       if (S::NP == 12 && sizeof(Real) < sizeof(Acc)) {
@@ -283,7 +271,8 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
     if (cur.active) {
 #pragma unroll
       for (int l = 0; l < LPT; ++l) {
-        Real U[18], R[18];
+        Real U[kLinkRegs], R[kLinkRegs];
+        R[18] = 0; R[19] = 0;
         asm volatile("" ::: "memory");
         load_link(stage, l, U, std::true_type());
         if (((q * LPT + l) & 1) == 0) {
@@ -358,7 +347,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
     if (d.precision == 32 && d.params == 12)
       return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
     if (d.precision == 32)
-      return launch_staged<Storage<float, 3, 18>, double, 2, 256, 1, 2, OPT_COULOMB>(links, g, parity, omega, true, st);
+      return launch_staged<Storage<float, 3, 18>, double, 1, 64, 1, 5, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
     if (d.params == 12)
       return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
     return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
@@ -385,10 +374,11 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
   if (d.precision == 32) {
     typedef Storage<float, 3, 18> S;
     switch (variant) {
-      case 20: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
-      case 21: return launch_staged<S, double, 1, 192, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
-      case 22: return launch_staged<S, double, 1, 128, 1, 3, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 20: return launch_staged<S, double, 1, 64, 1, 5, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 21: return launch_staged<S, double, 1, 128, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
+      case 22: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
       case 23: return launch_staged<S, double, 2, 256, 1, 2, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 24: return launch_staged<S, double, 1, 128, 1, 2, OPT_FLAT>(links, g, parity, omega, true, st);
       default: return cudaErrorInvalidValue;
     }
   }
@@ -429,7 +419,7 @@ static cudaError_t launch_production(const LatticeDesc& d, void* links, int pari
   if (d.precision == 32 && d.params == 12)
     return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT>(links, g, parity, pw, true, st);
   if (d.precision == 32)
-    return launch_staged<Storage<float, 3, 18>, double, 2, 256, 1, 2, 0>(links, g, parity, pw, true, st);
+    return launch_staged<Storage<float, 3, 18>, double, 1, 64, 1, 5, OPT_FLAT>(links, g, parity, pw, true, st);
   if (d.params == 12)
     return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT>(links, g, parity, pw, true, st);
   return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT>(links, g, parity, pw, true, st);

@@ -85,7 +85,7 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
       constexpr int MU_BATCH = (sizeof(Real) == 4) ? 2 : 1;
 #pragma unroll
       for (int mu0 = 0; mu0 < ND; mu0 += MU_BATCH) {
-        Real U[2 * MU_BATCH][S::NP];
+        Real U[2 * MU_BATCH][kLinkRegs];
 #pragma unroll
         for (int b = 0; b < MU_BATCH; ++b)
           if (mu0 + b < ND) {

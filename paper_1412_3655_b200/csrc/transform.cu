@@ -26,7 +26,8 @@ gauge_transform_kernel(typename S::Vec* __restrict__ links, const typename S::Re
       // forward neighbour x+mu lives in the other parity; its canonical site is 2*h' + odd'
       const int hu = up_index(g, h, sc, mu);
       const int64_t su = 2 * (int64_t)hu + (1 - sc.odd) * (mu == 0) + sc.odd * (mu != 0);
-      Real gu[18], U[18], T[18], R[18];
+      Real gu[18], U[kLinkRegs], T[18], R[kLinkRegs];
+      R[18] = 0; R[19] = 0;
 #pragma unroll
       for (int i = 0; i < 18; ++i) gu[i] = gf[su * 18 + i];
       typename S::Vec* p = link_base<S>(links, g, parity, mu, h);

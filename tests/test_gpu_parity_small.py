@@ -52,7 +52,7 @@ def variants_for(precision, params):
     if precision == 32 and params == 12:
         return [0, 1, 2, 4, 21, 22, 23, 24, 26, 27, 29, 30, 31]
     if precision == 32:
-        return [0, 2, 4, 21, 22, 23]
+        return [0, 2, 4, 21, 22, 23, 24]
     if params == 12:
         return [0, 2, 4, 8, 21, 22, 23, 24]
     return [0, 4, 8, 21, 22, 23, 24, 26, 27, 30, 31, 32]
