@@ -7,55 +7,83 @@
 
 namespace culgt {
 
-// One thread per (parity, h, mu).  Canonical link (s, mu) is NFULL contiguous reals.
-template <typename S, bool PACK, int BLOCK>
+// A CTA converts TILE consecutive canonical sites (= TILE/2 consecutive half indices h of BOTH
+// parities, 4*TILE links).  The canonical side of the tile is one contiguous run of
+// TILE*4*NFULL reals and moves with coalesced 16-byte accesses through shared memory; the internal
+// side is written / read with consecutive threads on consecutive h of one (parity, mu) plane set.
+// (A thread per link touching its 18 canonical reals directly reached 40 % of the copy rate.)
+template <typename S, bool PACK, int TILE, int BLOCK>
 __global__ void __launch_bounds__(BLOCK)
-layout_kernel(typename S::Real* __restrict__ canonical, typename S::Vec* __restrict__ links, const Geom g) {
+layout_tiled_kernel(typename S::Real* __restrict__ canonical, typename S::Vec* __restrict__ links, const Geom g,
+                    const long long V) {
   typedef typename S::Real Real;
-  const long long t = (long long)blockIdx.x * BLOCK + threadIdx.x;   // t = (h*4 + mu) within a parity
-  const int parity = blockIdx.y;
-  if (t >= 4ll * g.vh) return;
-  const int h = (int)(t >> 2);
-  const int mu = (int)(t & 3);
-  const SiteCoord sc = decode_site(g, h, parity);
-  const int64_t s = canonical_site(g, h, sc);
-  Real* cptr = canonical + (s * 4 + mu) * S::NFULL;
-  typename S::Vec* lptr = link_base<S>(links, g, parity, mu, h);
+  typedef typename S::Vec Vec;
+  constexpr int NF = S::NFULL;
+  extern __shared__ __align__(16) unsigned char tile_raw[];
+  Real* tile = reinterpret_cast<Real*>(tile_raw);          // [site in tile][mu][NF]
+  const long long s0 = (long long)blockIdx.x * TILE;
+  const int nsite = (int)((V - s0 < TILE) ? (V - s0) : TILE);   // even: every extent is even
+  const int nvec = nsite * 4 * NF * (int)sizeof(Real) / 16;
+  Vec* tile_v = reinterpret_cast<Vec*>(tile_raw);
+  Vec* can_v = reinterpret_cast<Vec*>(canonical + s0 * 4 * NF);
   if (PACK) {
-    Real m[kLinkRegs];
-#pragma unroll
-    for (int i = 0; i < kLinkRegs; ++i) m[i] = i < S::NFULL ? cptr[i] : (Real)0;   // pad reals stay 0
-    if (S::NC == 3) {
-      store_params<S>(lptr, g.vh, m);              // first NP reals = first NP/6 rows
-    } else {
-      // SU(2): [[a0+i a3, a2+i a1],[..]] -> (a0,a1,a2,a3)   (C-7)
-      Real a[4] = {m[0], m[3], m[2], m[1]};
-      store_params<S>(lptr, g.vh, a);
-    }
-  } else {
-    if (S::NC == 3) {
+    for (int i = threadIdx.x; i < nvec; i += BLOCK) tile_v[i] = can_v[i];
+    __syncthreads();
+  }
+  const int h0 = (int)(s0 >> 1);
+  const int nh = nsite >> 1;
+  for (int L = threadIdx.x; L < 8 * (TILE / 2); L += BLOCK) {   // link = (parity, mu, hl)
+    const int hl = L % (TILE / 2);
+    const int pm = L / (TILE / 2);
+    const int parity = pm >> 2, mu = pm & 3;
+    if (hl >= nh) continue;
+    const int h = h0 + hl;
+    const SiteCoord sc = decode_site(g, h, parity);
+    Real* c = tile + ((2 * hl + sc.odd) * 4 + mu) * NF;     // canonical site 2h + odd, local index
+    Vec* lptr = link_base<S>(links, g, parity, mu, h);
+    if (PACK) {
       Real m[kLinkRegs];
-      load_params<S>(lptr, g.vh, m);
-      if (S::NP == 12) reconstruct_row2(m);
 #pragma unroll
-      for (int i = 0; i < 18; ++i) cptr[i] = m[i];
+      for (int i = 0; i < kLinkRegs; ++i) m[i] = i < NF ? c[i] : (Real)0;   // pad reals stay 0
+      if (S::NC == 3) {
+        store_params<S>(lptr, g.vh, m);              // first NP reals = first NP/6 rows (L118)
+      } else {
+        // SU(2): [[a0+i a3, a2+i a1],[..]] -> (a0,a1,a2,a3)   (C-7)
+        Real a[4] = {m[0], m[3], m[2], m[1]};
+        store_params<S>(lptr, g.vh, a);
+      }
     } else {
-      Real a[4];
-      load_params<S>(lptr, g.vh, a);
-      cptr[0] = a[0];  cptr[1] = a[3];     // a0 + i a3
-      cptr[2] = a[2];  cptr[3] = a[1];     // a2 + i a1
-      cptr[4] = -a[2]; cptr[5] = a[1];     // -a2 + i a1
-      cptr[6] = a[0];  cptr[7] = -a[3];    // a0 - i a3
+      if (S::NC == 3) {
+        Real m[kLinkRegs];
+        load_params<S>(lptr, g.vh, m);
+        if (S::NP == 12) reconstruct_row2(m);
+#pragma unroll
+        for (int i = 0; i < 18; ++i) c[i] = m[i];
+      } else {
+        Real a[4];
+        load_params<S>(lptr, g.vh, a);
+        c[0] = a[0];  c[1] = a[3];     // a0 + i a3
+        c[2] = a[2];  c[3] = a[1];     // a2 + i a1
+        c[4] = -a[2]; c[5] = a[1];     // -a2 + i a1
+        c[6] = a[0];  c[7] = -a[3];    // a0 - i a3
+      }
     }
+  }
+  if (!PACK) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < nvec; i += BLOCK) can_v[i] = tile_v[i];
   }
 }
 
 template <typename S, bool PACK>
 static cudaError_t launch_layout(void* canonical, void* links, const Geom& g, cudaStream_t st) {
   constexpr int BLOCK = 256;
-  dim3 grid((unsigned)((4ll * g.vh + BLOCK - 1) / BLOCK), 2);
-  layout_kernel<S, PACK, BLOCK><<<grid, BLOCK, 0, st>>>((typename S::Real*)canonical,
-                                                         (typename S::Vec*)links, g);
+  constexpr int TILE = (sizeof(typename S::Real) == 8 && S::NC == 3) ? 64 : 128;   // <= 36 KB of shared memory
+  constexpr size_t smem = (size_t)TILE * 4 * S::NFULL * sizeof(typename S::Real);
+  const long long V = 2ll * g.vh;
+  const unsigned grid = (unsigned)((V + TILE - 1) / TILE);
+  layout_tiled_kernel<S, PACK, TILE, BLOCK><<<grid, BLOCK, smem, st>>>((typename S::Real*)canonical,
+                                                                       (typename S::Vec*)links, g, V);
   return cudaGetLastError();
 }
 
