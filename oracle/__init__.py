@@ -65,6 +65,8 @@ def _load():
     lib.oracle_su2_heatbath_samples.argtypes = [dp, ctypes.c_double, ctypes.c_uint64, ctypes.c_int64, dp]
     lib.oracle_sa_sweep.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double, ctypes.c_uint64,
                                     ctypes.c_uint32]
+    lib.oracle_site_G_micro.argtypes = [ctypes.c_int, dp, dp]
+    lib.oracle_micro_sweep.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int]
     lib.oracle_su2_pow_series.argtypes = [dp, ctypes.c_double, ctypes.c_int, dp]
     lib.oracle_site_G_series.argtypes = [ctypes.c_int, dp, ctypes.c_double, ctypes.c_int, dp]
     lib.oracle_or_sweep_series.argtypes = [i32p, ctypes.c_int, dp, ctypes.c_int, ctypes.c_double, ctypes.c_int]
@@ -286,3 +288,31 @@ def sa_sweep(dims, u: np.ndarray, parity: int, T: float, seed: int, counter: int
     """One simulated-annealing half-sweep at temperature T, in place."""
     nc = _check_links(dims, u)
     _load().oracle_sa_sweep(_dims(dims), nc, _dp(u), int(parity), float(T), int(seed), int(counter))
+
+
+# ---- microcanonical step (DESIGN.md reading C-26) ---------------------------------------------------
+
+def site_G_micro(K: np.ndarray) -> np.ndarray:
+    K = np.ascontiguousarray(K, dtype=np.float64)
+    out = np.empty_like(K)
+    _load().oracle_site_G_micro(K.shape[0], _dp(K), _dp(out))
+    return out
+
+
+def micro_sweep(dims, u: np.ndarray, parity: int) -> None:
+    """One microcanonical half-sweep (per-subgroup reflection g^2, F unchanged), in place."""
+    nc = _check_links(dims, u)
+    _load().oracle_micro_sweep(_dims(dims), nc, _dp(u), int(parity))
+
+
+def sa_anneal_micro(dims, u: np.ndarray, T_max: float, T_min: float, n_sweeps: int, n_micro: int,
+                    seed: int) -> None:
+    """The schedule of culgt_sa_anneal_micro: annealing sweep i (T linear from T_max to T_min,
+    half-sweep counters 2i, 2i+1) followed by n_micro microcanonical full sweeps."""
+    for i in range(int(n_sweeps)):
+        T = T_max - (T_max - T_min) * i / (n_sweeps - 1) if n_sweeps > 1 else T_min
+        for parity in (0, 1):
+            sa_sweep(dims, u, parity, T, seed, 2 * i + parity)
+        for _ in range(int(n_micro)):
+            for parity in (0, 1):
+                micro_sweep(dims, u, parity)

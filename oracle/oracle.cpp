@@ -764,6 +764,33 @@ Mat site_G_heatbath(Mat K, double T, int nc, uint32_t site, uint32_t counter, ui
   }
   return G;
 }
+
+// ---- microcanonical step (SURVEY.md 8(f) NEXT-3 "simulated annealing + microcanonical steps";
+// DESIGN.md reading C-26) ---------------------------------------------------------------------
+// The energy-conserving companion of the heat bath: in each SU(2) subgroup the update is the
+// REFLECTION q = g^2 of the maximiser g = conj(p)/|p| -- with h = q*p/|p| as in C-25 the local
+// weight Re tr[g_s K] = |p| h_0 + const, and q = g^2 gives h = g, h_0 = p_0/|p|, the value q = 1
+// gives as well: the functional is unchanged while the links move.  Written out as the quaternion
+// square (c, v)^2 = (c^2 - v.v, 2 c v) (convention C-7; v x v = 0), no trigonometric function.
+Mat site_G_micro(Mat K, int nc) {
+  Mat G = unit_mat(nc);
+  static const int pairs[3][2] = {{0, 1}, {0, 2}, {1, 2}};
+  int npairs = (nc == 2) ? 1 : 3;
+  for (int t = 0; t < npairs; ++t) {
+    int i = pairs[t][0], j = pairs[t][1];
+    double p[4] = {K.e[i][i].real() + K.e[j][j].real(), K.e[i][j].imag() + K.e[j][i].imag(),
+                   K.e[i][j].real() - K.e[j][i].real(), K.e[i][i].imag() - K.e[j][j].imag()};
+    double n = std::sqrt(p[0] * p[0] + p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
+    if (n == 0.0) continue;                                  // C-9
+    double g[4] = {p[0] / n, -p[1] / n, -p[2] / n, -p[3] / n};
+    double q[4] = {g[0] * g[0] - (g[1] * g[1] + g[2] * g[2] + g[3] * g[3]),
+                   2.0 * g[0] * g[1], 2.0 * g[0] * g[2], 2.0 * g[0] * g[3]};
+    Mat gs = embed_su2(q, i, j, nc);
+    K = mul(gs, K, nc);
+    G = mul(gs, G, nc);
+  }
+  return G;
+}
 }  // namespace
 
 extern "C" {
@@ -791,6 +818,28 @@ void oracle_sa_sweep(const int32_t* dims, int nc, double* U, int parity, double 
   for (int64_t s = 0; s < L.V; ++s) {
     if (parity_of(L, s) != parity) continue;
     Mat G = site_G_heatbath(gather_K(U, L, s), T, nc, (uint32_t)s, counter, seed);
+    Mat Gd = dagger(G, nc);
+    for (int mu = 0; mu < 4; ++mu) {
+      double* up = link_ptr(U, L, s, mu);
+      store_mat(up, nc, mul(G, load_mat(up, nc), nc));
+      double* dn = link_ptr(U, L, neighbour(L, s, mu, -1), mu);
+      store_mat(dn, nc, mul(load_mat(dn, nc), Gd, nc));
+    }
+  }
+}
+
+// G of the microcanonical step for a given K (one site): K, G are double[nc][nc][2].
+void oracle_site_G_micro(int nc, const double* K, double* G) {
+  store_mat(G, nc, site_G_micro(load_mat(K, nc), nc));
+}
+
+// One microcanonical HALF sweep over the sites of `parity`, in place (reading C-26).
+void oracle_micro_sweep(const int32_t* dims, int nc, double* U, int parity) {
+  Lat L = make_lat(dims, nc);
+#pragma omp parallel for num_threads(g_threads) schedule(static)
+  for (int64_t s = 0; s < L.V; ++s) {
+    if (parity_of(L, s) != parity) continue;
+    Mat G = site_G_micro(gather_K(U, L, s), nc);
     Mat Gd = dagger(G, nc);
     for (int mu = 0; mu < 4; ++mu) {
       double* up = link_ptr(U, L, s, mu);
