@@ -2,7 +2,7 @@
 """bench.py -- SU(3) Landau overrelaxation throughput on B200 (BASELINE.json metric, configs[3]).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
-                    [--gauge landau|coulomb] [--series-order N] [--sa-temperature T] [--variant V]
+                    [--gauge landau|coulomb] [--series-order N] [--sa-temperature T] [--micro] [--variant V]
 
 A STEP is one full overrelaxation sweep (black half-sweep + white half-sweep = V site updates,
 PAPER.md L54) of the resident field; every --check-every steps the timed region also computes
@@ -58,6 +58,8 @@ def parse_args():
                     help="coulomb: K(x) from the spatial links, per-slice theta_t/F_t (DESIGN.md C-22)")
     ap.add_argument("--series-order", type=int, default=0,
                     help="> 0: truncated-series g^omega of that order instead of the exact power (DESIGN.md C-24)")
+    ap.add_argument("--micro", action="store_true",
+                    help="microcanonical sweeps (reflection g^2, DESIGN.md C-26) instead of overrelaxation")
     ap.add_argument("--sa-temperature", type=float, default=0.0,
                     help="> 0: time simulated-annealing sweeps at this temperature instead of overrelaxation (DESIGN.md C-25)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -221,7 +223,8 @@ def flops_per_site(cfg, gauge="landau"):
 
 def workload_config(args, cfg):
     return {
-        "gauge": args.gauge, "power": (f"heat bath at T={args.sa_temperature}" if args.sa_temperature > 0 else
+        "gauge": args.gauge, "power": ("microcanonical g^2" if args.micro else
+                                       f"heat bath at T={args.sa_temperature}" if args.sa_temperature > 0 else
                                        f"series order {args.series_order}" if args.series_order > 0 else "exact"),
         "workload": f"{args.workload}: {'x'.join(str(d) for d in cfg['dims'])} SU({cfg['group']}) "
                     f"fp{cfg['precision']} {cfg['params']}-parameter, omega={cfg['omega']}, "
@@ -289,6 +292,10 @@ def main():
         if coulomb or args.series_order > 0:
             raise SystemExit("--sa-temperature applies to Landau gauge and excludes --series-order")
         sweeps = lambda lat_, links_, n_, om_: culgt.culgt_sa_anneal(lat_, links_, args.sa_temperature, args.sa_temperature, n_, 2024)  # noqa: E731
+    if args.micro:
+        if coulomb or args.series_order > 0 or args.sa_temperature > 0:
+            raise SystemExit("--micro applies to Landau gauge and excludes --series-order / --sa-temperature")
+        sweeps = lambda lat_, links_, n_, om_: culgt.culgt_micro_sweeps(lat_, links_, n_)  # noqa: E731
     if args.series_order > 0:
         if coulomb:
             raise SystemExit("--series-order applies to Landau gauge")

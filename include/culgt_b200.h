@@ -154,6 +154,19 @@ int culgt_sa_sweep(const culgt_lattice* lat, void* links, int parity, double T, 
 int culgt_sa_anneal(const culgt_lattice* lat, void* links, double T_max, double T_min, int n_sweeps,
                     unsigned long long seed, void* stream);
 
+/* ---- Microcanonical step (SURVEY.md 8(f) NEXT-3 pairs it with simulated annealing; DESIGN.md
+ * reading C-26): the half-sweep whose per-subgroup update is the reflection q = g^2 of the maximiser
+ * g = K^dagger/sqrt(det K^dagger) -- Re tr[g_s K], hence F, is unchanged while the links move
+ * (the omega -> 2 end of "replacing g(x) by g^omega(x)", which culgt_or_sweep excludes).
+ * Deterministic, in place, asynchronous; Landau gauge.
+ * culgt_micro_sweeps: n_sweeps full (black + white) sweeps.
+ * culgt_sa_anneal_micro: the schedule of culgt_sa_anneal with n_micro >= 0 microcanonical full
+ * sweeps after every annealing sweep (annealing half-sweep counters stay 2i, 2i+1). */
+int culgt_micro_sweep(const culgt_lattice* lat, void* links, int parity, void* stream);
+int culgt_micro_sweeps(const culgt_lattice* lat, void* links, int n_sweeps, void* stream);
+int culgt_sa_anneal_micro(const culgt_lattice* lat, void* links, double T_max, double T_min, int n_sweeps,
+                          int n_micro, unsigned long long seed, void* stream);
+
 /* ---- Coulomb gauge (named by the paper, P:L7; reading C-22): the same update
  * with mu restricted to the 3 spatial directions, time-slice by time-slice:
  *   K_C(x) = sum_{i<3} [ U_i(x) + U_i(x-i)^dagger ],  G from K_C as above,

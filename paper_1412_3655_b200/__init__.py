@@ -75,6 +75,10 @@ def lib() -> ctypes.CDLL:
     L.culgt_or_sweeps_series.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, ctypes.c_int, vp]
     L.culgt_sa_sweep.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, ctypes.c_ulonglong, ctypes.c_uint, vp]
     L.culgt_sa_anneal.argtypes = [latp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_ulonglong, vp]
+    L.culgt_micro_sweep.argtypes = [latp, vp, ctypes.c_int, vp]
+    L.culgt_micro_sweeps.argtypes = [latp, vp, ctypes.c_int, vp]
+    L.culgt_sa_anneal_micro.argtypes = [latp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
+                                        ctypes.c_ulonglong, vp]
     L.culgt_or_sweep_coulomb.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_or_sweep_coulomb_masked.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp, vp]
     L.culgt_or_sweeps_coulomb.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
@@ -292,6 +296,28 @@ def culgt_sa_anneal(lat: Lattice, links, T_max: float, T_min: float, n_sweeps: i
     _require_cuda()
     _check(lib().culgt_sa_anneal(ctypes.byref(lat.c()), _ptr(links), float(T_max), float(T_min),
                                  int(n_sweeps), int(seed), _stream(stream)), "culgt_sa_anneal")
+
+
+# ---- microcanonical step (reading C-26) -----------------------------------------------
+
+def culgt_micro_sweep(lat: Lattice, links, parity: int, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_micro_sweep(ctypes.byref(lat.c()), _ptr(links), int(parity), _stream(stream)),
+           "culgt_micro_sweep")
+
+
+def culgt_micro_sweeps(lat: Lattice, links, n_sweeps: int, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_micro_sweeps(ctypes.byref(lat.c()), _ptr(links), int(n_sweeps), _stream(stream)),
+           "culgt_micro_sweeps")
+
+
+def culgt_sa_anneal_micro(lat: Lattice, links, T_max: float, T_min: float, n_sweeps: int, n_micro: int,
+                          seed: int, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_sa_anneal_micro(ctypes.byref(lat.c()), _ptr(links), float(T_max), float(T_min),
+                                       int(n_sweeps), int(n_micro), int(seed), _stream(stream)),
+           "culgt_sa_anneal_micro")
 
 
 # ---- Coulomb gauge (reading C-22) ----------------------------------------------------

@@ -330,6 +330,57 @@ int culgt_sa_anneal(const culgt_lattice* lat, void* links, double T_max, double 
   return CULGT_OK;
 }
 
+// ---- microcanonical step (reading C-26) ------------------------------------------------
+
+int culgt_micro_sweep(const culgt_lattice* lat, void* links, int parity, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (parity != 0 && parity != 1) return CULGT_ERR_PARITY;
+  cudaError_t e = launch_micro_sweep(d, links, parity, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_micro_sweeps(const culgt_lattice* lat, void* links, int n_sweeps, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (n_sweeps < 0) return CULGT_ERR_ARG;
+  for (int i = 0; i < n_sweeps; ++i)
+    for (int parity = 0; parity < 2; ++parity) {
+      cudaError_t e = launch_micro_sweep(d, links, parity, (cudaStream_t)stream);
+      if (e != cudaSuccess) return cuda_fail(e);
+    }
+  return CULGT_OK;
+}
+
+int culgt_sa_anneal_micro(const culgt_lattice* lat, void* links, double T_max, double T_min, int n_sweeps,
+                          int n_micro, unsigned long long seed, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (n_sweeps < 0 || n_micro < 0 || !(T_min > 0.0) || !(T_max >= T_min) || !(T_max < 1e300)) return CULGT_ERR_ARG;
+  for (int i = 0; i < n_sweeps; ++i) {
+    const double T = n_sweeps > 1 ? T_max - (T_max - T_min) * (double)i / (double)(n_sweeps - 1) : T_min;
+    for (int parity = 0; parity < 2; ++parity) {
+      cudaError_t e = launch_sa_sweep(d, links, parity, T, seed, (unsigned)(2 * i + parity), (cudaStream_t)stream);
+      if (e != cudaSuccess) return cuda_fail(e);
+    }
+    for (int m = 0; m < n_micro; ++m)
+      for (int parity = 0; parity < 2; ++parity) {
+        cudaError_t e = launch_micro_sweep(d, links, parity, (cudaStream_t)stream);
+        if (e != cudaSuccess) return cuda_fail(e);
+      }
+  }
+  return CULGT_OK;
+}
+
 // ---- Coulomb gauge (reading C-22) -----------------------------------------------------
 
 int culgt_or_sweep_coulomb(const culgt_lattice* lat, void* links, int parity, double omega, void* stream) {

@@ -40,6 +40,9 @@ cudaError_t launch_sa_sweep(const LatticeDesc& d, void* links, int parity, doubl
                             unsigned counter, cudaStream_t st);
 cudaError_t launch_or_sweep_staged_heatbath(const LatticeDesc& d, void* links, int parity, const HeatBathPower& pw,
                                             cudaStream_t st);
+// microcanonical half-sweep (reading C-26), production mappings only
+cudaError_t launch_micro_sweep(const LatticeDesc& d, void* links, int parity, cudaStream_t st);
+cudaError_t launch_or_sweep_staged_micro(const LatticeDesc& d, void* links, int parity, cudaStream_t st);
 // truncated-series overrelaxation (reading C-24), production mappings only
 cudaError_t launch_or_sweep_series(const LatticeDesc& d, void* links, int parity, double omega, int order,
                                    cudaStream_t st);

@@ -191,6 +191,15 @@ cudaError_t launch_sa_sweep(const LatticeDesc& d, void* links, int parity, doubl
   return launch_or_sweep_staged_heatbath(d, links, parity, pw, st);
 }
 
+// Microcanonical half-sweep (reading C-26); production mappings only.
+cudaError_t launch_micro_sweep(const LatticeDesc& d, void* links, int parity, cudaStream_t st) {
+  if (d.group == 2) {
+    if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, d.geom, parity, MicroPower{0}, false, st);
+    return launch_su2<Storage<double, 2, 4> >(links, d.geom, parity, MicroPower{0}, false, st);
+  }
+  return launch_or_sweep_staged_micro(d, links, parity, st);
+}
+
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
                             int variant, cudaStream_t st, bool coulomb) {
   const Geom& g = d.geom;

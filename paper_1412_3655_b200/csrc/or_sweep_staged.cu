@@ -35,6 +35,7 @@ __device__ __forceinline__ double power_omega(double w) { return w; }
 __device__ __forceinline__ double power_omega(const ExactPower& p) { return p.omega; }
 __device__ __forceinline__ double power_omega(const SeriesPower&) { return 0.0; }
 __device__ __forceinline__ double power_omega(const HeatBathPower&) { return 0.0; }
+__device__ __forceinline__ double power_omega(const MicroPower&) { return 0.0; }
 
 // Option bits of the OPT template parameter.
 constexpr int OPT_PREFETCH = 1;    // persistent only: prefetch.global.L2 of the next site block
@@ -410,7 +411,8 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
   }
 }
 
-// Truncated-series overrelaxation (reading C-24) / simulated annealing (C-25) on the production
+// Truncated-series overrelaxation (reading C-24) / simulated annealing (C-25) / the
+// microcanonical step (C-26) on the production
 // mapping of each format.
 template <typename Power>
 static cudaError_t launch_production(const LatticeDesc& d, void* links, int parity, const Power& pw, cudaStream_t st) {
@@ -428,6 +430,9 @@ static cudaError_t launch_production(const LatticeDesc& d, void* links, int pari
 cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int parity, const SeriesPower& pw,
                                           cudaStream_t st) {
   return launch_production(d, links, parity, pw, st);
+}
+cudaError_t launch_or_sweep_staged_micro(const LatticeDesc& d, void* links, int parity, cudaStream_t st) {
+  return launch_production(d, links, parity, MicroPower{0}, st);
 }
 cudaError_t launch_or_sweep_staged_heatbath(const LatticeDesc& d, void* links, int parity, const HeatBathPower& pw,
                                             cudaStream_t st) {

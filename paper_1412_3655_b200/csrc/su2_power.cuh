@@ -141,6 +141,11 @@ __device__ __forceinline__ bool su2_update_power(const double* p, double omega, 
 struct ExactPower {
   double omega;
 };
+// Microcanonical step (reading C-26): q = g^2, the reflection that leaves Re tr[g_s K]
+// unchanged.  No parameter.
+struct MicroPower {
+  int unused;
+};
 constexpr int kMaxSeriesOrder = 16;
 struct SeriesPower {
   int order;
@@ -175,6 +180,20 @@ __device__ __forceinline__ bool su2_update_power(const double* p, const SeriesPo
   return true;
 }
 
+// q = g^2 for g = conj(p)/|p|:  (c, v)^2 = (c^2 - v.v, 2 c v)  =  (p0^2 - pv.pv, -2 p0 pv)/|p|^2.
+template <bool FULL>
+__device__ __forceinline__ bool su2_update_power(const double* p, const MicroPower&, double* q) {
+  const double r2 = p[1] * p[1] + p[2] * p[2] + p[3] * p[3];
+  const double n2 = fma(p[0], p[0], r2);
+  if (n2 < 1e-280) return false;                           // |p| = 0: the update is skipped (C-9)
+  const double ninv = rsqrt_newton<true>(n2);
+  const double c = p[0] * ninv;
+  const double f = -2.0 * c * ninv;
+  q[0] = fma(c, c, -(r2 * ninv) * ninv);
+  q[1] = p[1] * f; q[2] = p[2] * f; q[3] = p[3] * f;
+  return true;
+}
+
 // Uniform entry used by the solvers: (site, subgroup) select the random numbers of the heat bath
 // and are ignored by the deterministic powers.
 template <bool FULL>
@@ -187,6 +206,10 @@ __device__ __forceinline__ bool su2_update_at(const double* p, const ExactPower&
 }
 template <bool FULL>
 __device__ __forceinline__ bool su2_update_at(const double* p, const SeriesPower& pw, double* q, uint32_t, uint32_t) {
+  return su2_update_power<FULL>(p, pw, q);
+}
+template <bool FULL>
+__device__ __forceinline__ bool su2_update_at(const double* p, const MicroPower& pw, double* q, uint32_t, uint32_t) {
   return su2_update_power<FULL>(p, pw, q);
 }
 template <bool FULL>

@@ -100,6 +100,9 @@ def test_argument_errors_by_return_code():
     assert lib.culgt_sa_sweep(ref, ok_ptr, 0, 0.0, 1, 0, None) == E["CULGT_ERR_ARG"]
     assert lib.culgt_sa_sweep(ref, ok_ptr, 2, 1.0, 1, 0, None) == E["CULGT_ERR_PARITY"]
     assert lib.culgt_sa_anneal(ref, ok_ptr, 0.1, 1.0, 5, 1, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_micro_sweep(ref, ok_ptr, 2, None) == E["CULGT_ERR_PARITY"]
+    assert lib.culgt_micro_sweeps(ref, None, 1, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_sa_anneal_micro(ref, ok_ptr, 1.0, 0.1, 5, -1, 1, None) == E["CULGT_ERR_ARG"]
     assert lib.culgt_reunitarize(ref, None, None) == E["CULGT_ERR_NULL"]
     assert lib.culgt_autotune_sweep(ref, ok_ptr, 1.7, 0, None, None, None) == E["CULGT_ERR_ARG"]
     assert lib.culgt_gauge_precision_functional(ref, ok_ptr, ok_ptr, ok_ptr, None, None) == E["CULGT_ERR_NULL"]

@@ -51,6 +51,8 @@ def test_guard_zones_survive_every_kernel(dims, group, precision, params):
     culgt.culgt_or_sweeps_coulomb(lat, links, 1, 1.7)
     culgt.culgt_or_sweeps_series(lat, links, 1, 1.7, 4)
     culgt.culgt_sa_anneal(lat, links, 1.0, 0.1, 2, 9)
+    culgt.culgt_sa_anneal_micro(lat, links, 1.0, 0.1, 2, 1, 9)
+    culgt.culgt_micro_sweeps(lat, links, 1)
     culgt.culgt_reunitarize(lat, links)
     culgt.culgt_gauge_precision(lat, links, ws, scal[0:1])
     culgt.culgt_functional(lat, links, ws, scal[1:2])
