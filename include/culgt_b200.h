@@ -195,6 +195,10 @@ int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, do
 
 /* Kernel-variant selection for measurement: variant 0 = the default chosen
  * by measurement; other values select alternative thread-to-site mappings where provided.
+ * 40 + k / 50 + k (k = 1..4): the full-sweep calls (culgt_or_sweeps, culgt_landau_fix,
+ * culgt_fix_host) interleave the black and white half-sweeps in slabs of 2^k time-slices, on one
+ * stream / with the white windows on an internal second stream that is joined back into `stream`
+ * before the call returns its work to it; same result bit for bit.
  * Returns CULGT_OK or CULGT_ERR_ARG.  Process-global; not thread-safe. */
 int culgt_set_sweep_variant(int variant);
 

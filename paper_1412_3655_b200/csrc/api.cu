@@ -133,11 +133,10 @@ int culgt_or_sweeps(const culgt_lattice* lat, void* links, int n_sweeps, double 
   if (misaligned(links)) return CULGT_ERR_ALIGN;
   if (n_sweeps < 0) return CULGT_ERR_ARG;
   if ((rc = check_omega(omega)) != CULGT_OK) return rc;
-  for (int i = 0; i < n_sweeps; ++i)
-    for (int parity = 0; parity < 2; ++parity) {
-      cudaError_t e = launch_or_sweep(d, links, parity, omega, g_variant, (cudaStream_t)stream);
-      if (e != cudaSuccess) return cuda_fail(e);
-    }
+  for (int i = 0; i < n_sweeps; ++i) {
+    cudaError_t e = launch_or_full_sweep(d, links, omega, g_variant, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+  }
   return CULGT_OK;
 }
 
@@ -221,11 +220,10 @@ int culgt_landau_fix(const culgt_lattice* lat, void* links, void* workspace, dou
   while (theta >= theta_target && done < max_sweeps) {
     int n = check_every;
     if (done + n > max_sweeps) n = max_sweeps - done;
-    for (int i = 0; i < n; ++i)
-      for (int parity = 0; parity < 2; ++parity) {
-        cudaError_t e = launch_or_sweep(d, links, parity, omega, g_variant, st);
-        if (e != cudaSuccess) return cuda_fail(e);
-      }
+    for (int i = 0; i < n; ++i) {
+      cudaError_t e = launch_or_full_sweep(d, links, omega, g_variant, st);
+      if (e != cudaSuccess) return cuda_fail(e);
+    }
     done += n;
     if ((rc = read_theta_F(d, links, workspace, st, &theta, nullptr)) != CULGT_OK) return rc;
   }
@@ -252,8 +250,7 @@ int culgt_fix_host(const culgt_lattice* lat, void* canonical_host, void* canonic
   if (e != cudaSuccess) return cuda_fail(e);
   if ((e = launch_pack(d, canonical_dev, links_dev, st)) != cudaSuccess) return cuda_fail(e);
   for (int i = 0; i < n_sweeps; ++i)
-    for (int parity = 0; parity < 2; ++parity)
-      if ((e = launch_or_sweep(d, links_dev, parity, omega, g_variant, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = launch_or_full_sweep(d, links_dev, omega, g_variant, st)) != cudaSuccess) return cuda_fail(e);
   if ((e = launch_unpack(d, links_dev, canonical_dev, st)) != cudaSuccess) return cuda_fail(e);
   e = cudaMemcpyAsync(canonical_host, canonical_dev, cbytes, cudaMemcpyDeviceToHost, st);
   if (e != cudaSuccess) return cuda_fail(e);
@@ -519,12 +516,11 @@ int culgt_autotune_sweep(const culgt_lattice* lat, void* links, double omega, in
     if (v == 11 || v == 14 || v == 25 || v == 28 || v == 32) continue;
     if (d.group == 2 && v != 0) continue;
     cudaError_t e = cudaSuccess;
-    for (int parity = 0; parity < 2 && e == cudaSuccess; ++parity) e = launch_or_sweep(d, links, parity, omega, v, st);
+    e = launch_or_full_sweep(d, links, omega, v, st);
     if (e == cudaErrorInvalidValue) continue;                     // mapping not built for this format
     if (e != cudaSuccess) { rc = cuda_fail(e); break; }
     cudaEventRecord(e0, st);
-    for (int i = 0; i < sweeps_per_trial && e == cudaSuccess; ++i)
-      for (int parity = 0; parity < 2 && e == cudaSuccess; ++parity) e = launch_or_sweep(d, links, parity, omega, v, st);
+    for (int i = 0; i < sweeps_per_trial && e == cudaSuccess; ++i) e = launch_or_full_sweep(d, links, omega, v, st);
     cudaEventRecord(e1, st);
     if (e == cudaSuccess) e = cudaEventSynchronize(e1);
     if (e != cudaSuccess) { rc = cuda_fail(e); break; }

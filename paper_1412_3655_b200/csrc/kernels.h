@@ -48,6 +48,13 @@ cudaError_t launch_or_sweep_series(const LatticeDesc& d, void* links, int parity
                                    cudaStream_t st);
 cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int parity, const SeriesPower& pw,
                                           cudaStream_t st);
+// One FULL sweep (black then white).  Variants 40..59 select the slab-blocked schedule of
+// or_sweep_staged.cu (40 + log2(slab slices): one stream; 50 + log2(slab slices): white windows on a
+// second stream); every other variant, and any lattice the slab schedule does not fit, is the two
+// whole half-sweeps of launch_or_sweep.
+cudaError_t launch_or_full_sweep(const LatticeDesc& d, void* links, double omega, int variant, cudaStream_t st);
+cudaError_t launch_or_sweep_staged_slabbed(const LatticeDesc& d, void* links, double omega, int slab_slices,
+                                           bool overlap, cudaStream_t st);
 cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
                                    int variant, bool coulomb, cudaStream_t st);
 cudaError_t launch_pack(const LatticeDesc& d, const void* canonical, void* links, cudaStream_t st);

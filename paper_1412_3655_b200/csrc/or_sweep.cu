@@ -200,9 +200,23 @@ cudaError_t launch_micro_sweep(const LatticeDesc& d, void* links, int parity, cu
   return launch_or_sweep_staged_micro(d, links, parity, st);
 }
 
+cudaError_t launch_or_full_sweep(const LatticeDesc& d, void* links, double omega, int variant, cudaStream_t st) {
+  if (variant >= 40 && variant < 60) {
+    const cudaError_t e = launch_or_sweep_staged_slabbed(d, links, omega, 1 << (variant % 10), variant >= 50, st);
+    if (e != cudaErrorNotSupported) return e;
+    variant = 0;                                         // lattice does not fit the slab schedule
+  }
+  for (int parity = 0; parity < 2; ++parity) {
+    const cudaError_t e = launch_or_sweep(d, links, parity, omega, variant, st);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
                             int variant, cudaStream_t st, bool coulomb) {
   const Geom& g = d.geom;
+  if (variant >= 40 && variant < 60) variant = 0;       // slab schedules exist for full sweeps only
   if (d.group == 2) {
     if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, g, parity, omega, coulomb, st);
     return launch_su2<Storage<double, 2, 4> >(links, g, parity, omega, coulomb, st);

@@ -123,7 +123,8 @@ __device__ __forceinline__ typename S::Vec* vec_ptr(typename S::Vec* links, cons
 template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int OPT, typename Power>
 __global__ void __launch_bounds__(BLOCK, MINB)
 or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
-                           const Power omega, const int n_site_blocks, const int reverse) {
+                           const Power omega, const int n_site_blocks, const int reverse,
+                           const int block_lo) {
   typedef typename S::Real Real;
   typedef typename S::Vec Vec;
   constexpr int LPT = 8 / TPS;          // links per thread
@@ -139,7 +140,7 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
   const int per_cta = (n_site_blocks + (int)gridDim.x - 1) / (int)gridDim.x;
   auto block_of = [&](int it) {
     const int b = (OPT & OPT_CHUNKED) ? (int)blockIdx.x * per_cta + it : it * (int)gridDim.x + (int)blockIdx.x;
-    return reverse ? n_site_blocks - 1 - b : b;
+    return block_lo + (reverse ? n_site_blocks - 1 - b : b);   // window [block_lo, block_lo + n_site_blocks)
   };
   auto issue = [&](const SiteRef<LPT>& r, int stage) {
     if (r.active) {
@@ -314,7 +315,7 @@ static int sm_count() {
 
 template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, int OPT, typename Power>
 static cudaError_t launch_staged(void* links, const Geom& g, int parity, Power omega, bool reverse_odd,
-                                 cudaStream_t st) {
+                                 cudaStream_t st, int win_lo = 0, int win_n = -1, int win_reverse = -1) {
   typedef typename S::Vec Vec;
   auto kern = or_sweep_su3_staged_kernel<S, Acc, TPS, BLOCK, STAGES, MINB, OPT, Power>;
   constexpr size_t smem = (size_t)STAGES * (8 / TPS) * S::NV * BLOCK * sizeof(Vec);
@@ -325,13 +326,15 @@ static cudaError_t launch_staged(void* links, const Geom& g, int parity, Power o
     configured = true;
   }
   constexpr int SITES = BLOCK / TPS;
-  const int n_site_blocks = (g.vh + SITES - 1) / SITES;
+  // the whole parity sublattice, or (slab-blocked schedule) the window [win_lo, win_lo + win_n) of it
+  const int n_site_blocks = win_n >= 0 ? win_n : (g.vh + SITES - 1) / SITES;
+  if (n_site_blocks == 0) return cudaSuccess;
   // OPT bit 16: one CTA per site block (the hardware block scheduler hands out blocks in order)
   // instead of a persistent grid-stride loop
   int grid = (OPT & OPT_FLAT) ? n_site_blocks : sm_count() * MINB;
   if (grid > n_site_blocks) grid = n_site_blocks;
   kern<<<grid, BLOCK, smem, st>>>((Vec*)links, g, parity, omega, n_site_blocks,
-                                  (reverse_odd && parity) ? 1 : 0);
+                                  win_reverse >= 0 ? win_reverse : ((reverse_odd && parity) ? 1 : 0), win_lo);
   return cudaGetLastError();
 }
 
@@ -409,6 +412,88 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
     case 32: return launch_staged<S, double, 1, 96, 2, 1, 0>(links, g, parity, omega, true, st);             // pers, 2 stages
     default: return cudaErrorInvalidValue;
   }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Slab-blocked FULL sweep: the black and the white half-sweep interleaved slab by
+// slab along t, so that a white site finds the links its black neighbours have just written still
+// in the 126 MB L2 -- the field then crosses HBM about once per full sweep instead of twice.
+// Time-slice t is the contiguous half-index range [t*stride3, (t+1)*stride3) of each parity, i.e.
+// a contiguous window of site blocks.  With slab ends e_k = min((k+1)*sl, N3):
+//     for k:  black slices [k*sl, e_k)  ascending;   white slices [max(1, k*sl - 1), e_k - 1)  descending
+//     then    white slice N3-1, white slice 0.
+// A white site of slice t needs its black neighbours of slices t-1, t, t+1 done: t <= e_k - 2 and
+// t >= 1 guarantee it; slices N3-1 and 0 wait for the last / first black slab (periodic wrap).
+// Sites of one parity do not interact, so the result is bit-identical to two whole half-sweeps.
+// overlap: the white windows run on a second stream, concurrently with the next black slab -- they
+// touch disjoint links (black slab k+1 writes links stored at slices >= e_k - 1, the white window
+// links stored at slices <= e_k - 2) -- so neither launch's tail leaves the GPU idle.
+// Returns cudaErrorNotSupported when the lattice does not split into whole site blocks per slice.
+// ---------------------------------------------------------------------------------------------
+struct SlabStreams {
+  cudaStream_t white = nullptr;
+  cudaEvent_t black_done[64];
+  cudaEvent_t white_done = nullptr;
+  bool ready = false;
+};
+static SlabStreams g_slab;
+
+static cudaError_t slab_streams_init() {
+  if (g_slab.ready) return cudaSuccess;
+  cudaError_t e = cudaStreamCreateWithFlags(&g_slab.white, cudaStreamNonBlocking);
+  if (e != cudaSuccess) return e;
+  for (int i = 0; i < 64; ++i)
+    if ((e = cudaEventCreateWithFlags(&g_slab.black_done[i], cudaEventDisableTiming)) != cudaSuccess) return e;
+  if ((e = cudaEventCreateWithFlags(&g_slab.white_done, cudaEventDisableTiming)) != cudaSuccess) return e;
+  g_slab.ready = true;
+  return cudaSuccess;
+}
+
+template <typename S, int BLOCK, int MINB>
+static cudaError_t slab_sweep(void* links, const Geom& g, double omega, int sl, bool overlap, cudaStream_t st) {
+  const int n3 = g.n[3];
+  if (g.stride[3] % BLOCK != 0 || sl < 2 || n3 < 4 || sl > n3 - 2) return cudaErrorNotSupported;
+  const int bps = g.stride[3] / BLOCK;                  // site blocks per time-slice (per parity)
+  const int ns = (n3 + sl - 1) / sl;
+  if (ns > 64) return cudaErrorNotSupported;
+  cudaError_t e;
+  cudaStream_t wst = st;
+  if (overlap) {
+    if ((e = slab_streams_init()) != cudaSuccess) return e;
+    wst = g_slab.white;
+    // the previous work on the caller's stream (e.g. the previous sweep's black slabs) precedes our white windows
+  }
+  auto launch = [&](int parity, int t_lo, int t_hi, cudaStream_t s) {   // slices [t_lo, t_hi)
+    if (t_hi <= t_lo) return cudaSuccess;
+    return launch_staged<S, double, 1, BLOCK, 1, MINB, OPT_FLAT>(links, g, parity, omega, true, s, t_lo * bps,
+                                                                (t_hi - t_lo) * bps, parity);
+  };
+  for (int k = 0; k < ns; ++k) {
+    const int s_k = k * sl, e_k = (k + 1) * sl < n3 ? (k + 1) * sl : n3;
+    if ((e = launch(0, s_k, e_k, st)) != cudaSuccess) return e;
+    if (overlap) {
+      if ((e = cudaEventRecord(g_slab.black_done[k], st)) != cudaSuccess) return e;
+      if ((e = cudaStreamWaitEvent(wst, g_slab.black_done[k], 0)) != cudaSuccess) return e;
+    }
+    if ((e = launch(1, s_k > 1 ? s_k - 1 : 1, e_k - 1, wst)) != cudaSuccess) return e;
+  }
+  if ((e = launch(1, n3 - 1, n3, wst)) != cudaSuccess) return e;
+  if ((e = launch(1, 0, 1, wst)) != cudaSuccess) return e;
+  if (overlap) {     // join: whatever follows on the caller's stream sees the finished sweep
+    if ((e = cudaEventRecord(g_slab.white_done, wst)) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(st, g_slab.white_done, 0)) != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+cudaError_t launch_or_sweep_staged_slabbed(const LatticeDesc& d, void* links, double omega, int slab_slices,
+                                           bool overlap, cudaStream_t st) {
+  const Geom& g = d.geom;
+  if (d.group != 3) return cudaErrorNotSupported;
+  if (d.precision == 32 && d.params == 12) return slab_sweep<Storage<float, 3, 12>, 128, 4>(links, g, omega, slab_slices, overlap, st);
+  if (d.precision == 32) return slab_sweep<Storage<float, 3, 18>, 64, 5>(links, g, omega, slab_slices, overlap, st);
+  if (d.params == 12) return slab_sweep<Storage<double, 3, 12>, 64, 4>(links, g, omega, slab_slices, overlap, st);
+  return slab_sweep<Storage<double, 3, 18>, 64, 3>(links, g, omega, slab_slices, overlap, st);
 }
 
 // Truncated-series overrelaxation (reading C-24) / simulated annealing (C-25) / the

@@ -204,3 +204,29 @@ def test_autotuner_picks_a_result_equivalent_mapping():
             assert np.abs(f.download() - li.from_real(ref)).max() < TOL_LINK[precision]
         finally:
             culgt.culgt_set_sweep_variant(0)
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (8, 8, 8, 12), (16, 8, 8, 6), (4, 6, 2, 8)])
+@pytest.mark.parametrize("precision,params", SU3_STORES)
+def test_slab_blocked_full_sweep_is_the_same_sweep(dims, precision, params):
+    """Variants 41-43 / 51-53 (black and white half-sweeps interleaved slab by slab
+    along t, on one or two streams) reorder launches only: three sweeps must agree with the oracle
+    and be bit-identical to the default schedule; (4,6,2,8) does not split into whole site blocks per
+    slice and takes the fallback."""
+    u = make(dims, 3, 46)
+    ref = storage_input(u, precision, params)
+    oracle.full_sweep(dims, ref, 1.7)
+    outs = {}
+    for variant in (0, 41, 42, 43, 51, 52, 53):
+        culgt.culgt_set_sweep_variant(variant)
+        try:
+            f = GpuField(dims, 3, precision, params, u)
+            f.sweep(1.7, 1)
+            assert np.abs(f.download() - li.from_real(ref)).max() < TOL_LINK[precision], variant
+            f.sweep(1.7, 2)
+            torch.cuda.synchronize()
+            outs[variant] = f.download()
+        finally:
+            culgt.culgt_set_sweep_variant(0)
+    for variant, out in outs.items():
+        assert np.array_equal(out, outs[0]), variant
