@@ -66,7 +66,7 @@ size_t culgt_links_bytes(const culgt_lattice* lat);      /* internal field: 4*V*
 size_t culgt_canonical_bytes(const culgt_lattice* lat);  /* V*4*Nc*Nc*2*sizeof(real)                */
 size_t culgt_gfield_bytes(const culgt_lattice* lat);     /* V*Nc*Nc*2*sizeof(real)                  */
 size_t culgt_workspace_bytes(const culgt_lattice* lat);  /* reductions: block partials + 2 scalars;
-                                                            grows with the volume (V/128 doubles)    */
+                                                            grows with the volume (V/64 doubles)     */
 
 /* Validate a descriptor: CULGT_OK, CULGT_ERR_NULL, CULGT_ERR_DIMS or CULGT_ERR_DESC. */
 int culgt_validate(const culgt_lattice* lat);

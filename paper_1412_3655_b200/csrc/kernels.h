@@ -14,8 +14,9 @@ struct LatticeDesc {
 };
 
 constexpr int kReduceBlock = 256;       // threads per block of the reduction kernels
-// CTAs (= partials per quantity) of the fused theta+F kernel: 128 sites of each parity per CTA
-inline int reduce_blocks_fused(int vh) { return (vh + 127) / 128; }
+// CTAs (= partials per quantity) of the fused theta+F kernel: `half` sites of each parity per CTA
+// (128 for the register path, 64 for the staged fp32 12-parameter path; the workspace is sized for 64)
+inline int reduce_blocks_fused(int vh, int half = 64) { return (vh + half - 1) / half; }
 // doubles in the reduction workspace: block partials (Landau: 2 * vh/128; Coulomb: 2 * N3 *
 // slice/128; never below 4096) followed by 2 * N3 result slots that the *_host / *_fix paths
 // read back (Landau uses the first two).

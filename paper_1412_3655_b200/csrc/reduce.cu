@@ -62,8 +62,20 @@ __device__ __forceinline__ double theta_from_K(const double* K) {
 // per time-slice: blockIdx.y = t, the CTA's sites are the BLOCK/2 sites [bx*BLOCK/2, ...) of each
 // parity INSIDE slice t (a slice is the contiguous index range [t*stride3, (t+1)*stride3) of each
 // parity's sublattice), partials are laid out [t][bx].
-template <typename S, int BLOCK, bool COULOMB>
-__global__ void __launch_bounds__(BLOCK)
+// STAGED = false: the links are loaded straight into registers, a batch of directions at a time.
+// STAGED = true (SU(3)): all 2*ND links of the site are first copied into thread-private shared-memory
+// slots by cp.async.cg, `[vector][thread]` so that a warp's copy of one vector is 512 contiguous bytes
+// on both sides, one commit group per direction, and then widened and accumulated one link at a time
+// as its direction lands: every load of the site is in flight at once without holding registers (the
+// half-sweep's staging), and the conversions of direction mu overlap the loads of the
+// later ones.  No __syncthreads: cp.async.wait_group orders a thread against its own copies.
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+
+template <typename S, int BLOCK, bool COULOMB, bool STAGED>
+__global__ void __launch_bounds__(BLOCK, STAGED ? 512 / BLOCK : 0)
 theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
                         double* __restrict__ partial_theta, double* __restrict__ partial_F) {
   typedef typename S::Real Real;
@@ -80,6 +92,40 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
       double K[18];
 #pragma unroll
       for (int i = 0; i < 18; ++i) K[i] = 0;
+      if constexpr (STAGED) {
+        typedef typename S::Vec Vec;
+        extern __shared__ __align__(16) unsigned char smem_raw[];
+        Vec* const sm = reinterpret_cast<Vec*>(smem_raw) + threadIdx.x;   // vector v of link l at sm[(l*NV+v)*BLOCK]
+#pragma unroll
+        for (int mu = 0; mu < ND; ++mu) {
+          const Vec* up = link_base<S>(links, g, parity, mu, h);
+          const Vec* dn = link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu));
+#pragma unroll
+          for (int j = 0; j < S::NV; ++j) {
+            cp_async16(sm + ((2 * mu) * S::NV + j) * BLOCK, up + (size_t)j * (size_t)g.vh);
+            cp_async16(sm + ((2 * mu + 1) * S::NV + j) * BLOCK, dn + (size_t)j * (size_t)g.vh);
+          }
+          asm volatile("cp.async.commit_group;" ::: "memory");   // one group per direction
+        }
+#pragma unroll
+        for (int l = 0; l < 2 * ND; ++l) {
+          if ((l & 1) == 0) {                    // direction l/2 has landed; the later ones are still in flight
+            if (ND - 1 - l / 2 == 3) asm volatile("cp.async.wait_group 3;" ::: "memory");
+            else if (ND - 1 - l / 2 == 2) asm volatile("cp.async.wait_group 2;" ::: "memory");
+            else if (ND - 1 - l / 2 == 1) asm volatile("cp.async.wait_group 1;" ::: "memory");
+            else asm volatile("cp.async.wait_group 0;" ::: "memory");
+          }
+          Real U[kLinkRegs];
+#pragma unroll
+          for (int j = 0; j < S::NV; ++j) vec_get(sm[(l * S::NV + j) * BLOCK], U + j * S::VL);
+          double Ud[18];                     // widened first: the third row is rebuilt in fp64
+#pragma unroll
+          for (int i = 0; i < S::NP; ++i) Ud[i] = (double)U[i];
+          if (S::NP == 12) reconstruct_row2(Ud);
+          if ((l & 1) == 0) f += Ud[CULGT_RE(0, 0)] + Ud[CULGT_RE(1, 1)] + Ud[CULGT_RE(2, 2)];
+          accumulate(K, Ud, (l & 1) != 0);
+        }
+      } else {
       // the loads of a batch of directions are issued before any of them is used (memory-level
       // parallelism); fp32 storage batches 2 directions = 4 links, fp64 storage 1 direction
       constexpr int MU_BATCH = (sizeof(Real) == 4) ? 2 : 1;
@@ -107,6 +153,7 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
             if (S::NP == 12) reconstruct_row2(Ud);
             accumulate(K, Ud, true);
           }
+      }
       }
       th = theta_from_K(K);
     } else {
@@ -150,13 +197,50 @@ final_sum_kernel(const double* __restrict__ partial, int n, double scale0, doubl
   }
 }
 
+template <typename S, int BLOCK, bool COULOMB>
+static cudaError_t launch_theta_staged(dim3 grid, const void* links, const Geom& g, double* p_theta, double* p_F,
+                                       cudaStream_t st) {
+  auto kern = theta_functional_kernel<S, BLOCK, COULOMB, true>;
+  constexpr size_t smem = (size_t)8 * S::NV * BLOCK * sizeof(typename S::Vec);
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  kern<<<grid, BLOCK, smem, st>>>((const typename S::Vec*)links, g, p_theta, p_F);
+  return cudaGetLastError();
+}
+
+// fp32 12-parameter storage takes the staged kernel (measured); the others the register path
+// fp32 12-parameter storage takes the staged kernel, 64 sites of each parity per 128-thread CTA, 4 CTAs
+// per SM (measured at 32^4: 67 -> 60 us per check inside the sweep loop, 91 -> 56 us back to back;
+// DESIGN.md 6.3); the other formats the register path with 128 sites of each parity per CTA.
+template <typename S>
+static constexpr bool theta_is_staged() { return S::NC == 3 && S::NP == 12 && sizeof(typename S::Real) == 4; }
+
+// group_size sites of each parity per y-slot of the grid (the sublattice, or one time-slice of it);
+// the partials of quantity 1 start at p_theta + ny * blocks
+template <typename S, bool COULOMB>
+static cudaError_t launch_theta_pass(int group_size, int ny, const void* links, const Geom& g, double* p_theta,
+                                     cudaStream_t st, int* blocks_out) {
+  const int nb = reduce_blocks_fused(group_size, theta_is_staged<S>() ? 64 : 128);
+  *blocks_out = nb;
+  double* p_F = p_theta + (size_t)ny * nb;
+  const dim3 grid(nb, ny);
+  if constexpr (theta_is_staged<S>()) {
+    return launch_theta_staged<S, 128, COULOMB>(grid, links, g, p_theta, p_F, st);
+  } else {
+    theta_functional_kernel<S, 256, COULOMB, false><<<grid, 256, 0, st>>>((const typename S::Vec*)links, g, p_theta, p_F);
+    return cudaGetLastError();
+  }
+}
+
 template <typename S>
 static cudaError_t run_theta_functional(const LatticeDesc& d, const void* links, double* ws, double* out_theta,
                                         double* out_F, cudaStream_t st) {
-  constexpr int BLOCK = 256;
-  const int nblk = reduce_blocks_fused(d.geom.vh);
-  theta_functional_kernel<S, BLOCK, false><<<nblk, BLOCK, 0, st>>>((const typename S::Vec*)links, d.geom, ws, ws + nblk);
-  cudaError_t e = cudaGetLastError();
+  int nblk = 0;
+  cudaError_t e = launch_theta_pass<S, false>(d.geom.vh, 1, links, d.geom, ws, st, &nblk);
   if (e != cudaSuccess) return e;
   final_sum_kernel<kReduceBlock><<<dim3(1, 2), kReduceBlock, 0, st>>>(
       ws, nblk, 1.0 / ((double)S::NC * (double)d.V), 1.0 / (4.0 * S::NC * (double)d.V), out_theta, out_F);
@@ -167,13 +251,9 @@ static cudaError_t run_theta_functional(const LatticeDesc& d, const void* links,
 template <typename S>
 static cudaError_t run_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* ws,
                                                 double* out_theta_t, double* out_F_t, cudaStream_t st) {
-  constexpr int BLOCK = 256;
   const int n3 = d.geom.n[3];
-  const int nbx = reduce_blocks_fused(d.geom.stride[3]);
-  const size_t per_quantity = (size_t)n3 * nbx;
-  theta_functional_kernel<S, BLOCK, true><<<dim3(nbx, n3), BLOCK, 0, st>>>((const typename S::Vec*)links, d.geom,
-                                                                           ws, ws + per_quantity);
-  cudaError_t e = cudaGetLastError();
+  int nbx = 0;
+  cudaError_t e = launch_theta_pass<S, true>(d.geom.stride[3], n3, links, d.geom, ws, st, &nbx);
   if (e != cudaSuccess) return e;
   const double vs = (double)d.V / (double)n3;
   final_sum_kernel<kReduceBlock><<<dim3(n3, 2), kReduceBlock, 0, st>>>(

@@ -43,9 +43,10 @@ def test_sizes():
     assert culgt.culgt_links_bytes(culgt.Lattice((64,) * 4, 3, 64, 18)) == 9663676416
     assert culgt.culgt_links_bytes(culgt.Lattice((8,) * 4, 2, 64, 4)) == 524288
     assert culgt.culgt_workspace_bytes(L) >= 8 * 1024
-    # the fused theta+F pass keeps two partials per 128 sites of a parity, plus the 2 scalars
+    # the fused theta+F pass keeps two partials per 64 sites of a parity (the staged fp32 12-parameter
+    # kernel; the other formats use every other slot's worth, 128 sites per partial), plus the 2 scalars
     # + 2 * N3 result slots (theta_t, F_t of the Coulomb driver; the Landau scalars use two) + N3 mask bytes
-    assert culgt.culgt_workspace_bytes(culgt.Lattice((64,) * 4, 3, 64, 18)) == (2 * (64 ** 4 // 2 // 128) + 2 * 64 + 8) * 8
+    assert culgt.culgt_workspace_bytes(culgt.Lattice((64,) * 4, 3, 64, 18)) == (2 * (64 ** 4 // 2 // 64) + 2 * 64 + 8) * 8
     assert culgt.culgt_workspace_bytes(culgt.Lattice((4,) * 4, 3, 64, 18)) == (4096 + 2 * 4 + 1) * 8
 
 
