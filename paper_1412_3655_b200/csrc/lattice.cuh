@@ -164,4 +164,31 @@ __device__ __forceinline__ void store_params(typename S::Vec* p, int vh, const t
   }
 }
 
+// ---- programmatic dependent launch (sm_90+) ----------------------------------------------------
+// A kernel that calls pdl_prologue_done() before its first global access, launched through
+// launch_pdl(), lets the NEXT such launch of the stream be scheduled as soon as all of its own CTAs
+// have started, instead of after its last CTA has drained: the next grid's CTAs take the SM slots
+// the tail frees, do their index arithmetic, and block in griddepcontrol.wait until this grid has
+// completed and its stores are visible.  Stream order is preserved exactly.
+__device__ __forceinline__ void pdl_prologue_done() {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                              Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 }  // namespace culgt

@@ -113,6 +113,7 @@ or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
     ptr[2 * mu] = link_base<S>(links, g, parity, mu, h);
     ptr[2 * mu + 1] = link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu));
   }
+  pdl_prologue_done();    // lattice.cuh: the next half-sweep may be scheduled; the previous one is complete
 #pragma unroll
   for (int l = 0; l < 8; ++l) load_params<S>(ptr[l], g.vh, U[l]);
   // K = k0 + i k.sigma = sum_mu u_up + conj(u_dn)
@@ -155,9 +156,11 @@ template <typename S, typename Power>
 static cudaError_t launch_su2(void* links, const Geom& g, int parity, Power omega, bool coulomb, cudaStream_t st) {
   constexpr int BLOCK = 128;
   const unsigned grid = (unsigned)((g.vh + BLOCK - 1) / BLOCK);
-  if (coulomb) or_sweep_su2_kernel<S, BLOCK, true, Power><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g, parity, omega, parity);
-  else or_sweep_su2_kernel<S, BLOCK, false, Power><<<grid, BLOCK, 0, st>>>((typename S::Vec*)links, g, parity, omega, parity);
-  return cudaGetLastError();
+  if (coulomb)
+    return launch_pdl(or_sweep_su2_kernel<S, BLOCK, true, Power>, dim3(grid), dim3(BLOCK), 0, st,
+                      (typename S::Vec*)links, g, parity, omega, parity);
+  return launch_pdl(or_sweep_su2_kernel<S, BLOCK, false, Power>, dim3(grid), dim3(BLOCK), 0, st,
+                    (typename S::Vec*)links, g, parity, omega, parity);
 }
 
 // Truncated-series overrelaxation (reading C-24): b_n = binom(omega, n) by the recurrence

@@ -44,6 +44,8 @@ constexpr int OPT_NOMATH = 8;      // measurement only: G = 1 (memory pattern + 
 constexpr int OPT_FLAT = 16;       // one CTA per site block (hardware block scheduler), not persistent
 constexpr int OPT_STREAM_ST = 32;  // st.global.cs stores
 constexpr int OPT_NOSOLVE = 256;   // measurement only: K is accumulated but G = 1 (no subgroup solve)
+constexpr int OPT_PDL = 512;       // programmatic dependent launch: the next half-sweep's CTAs are scheduled
+                                   // (index arithmetic done) while this one's last wave drains
 constexpr int OPT_COULOMB = 64;    // Coulomb gauge (reading C-22): K(x) from the 6 spatial links only
 
 __device__ __forceinline__ void cp_async_vec(float4* smem, const float4* gmem) {
@@ -170,6 +172,11 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
   // prologue: STAGES-1 sites in flight
   SiteRef<LPT> cur = locate<BLOCK, TPS, (OPT & OPT_COULOMB) != 0>(g, parity, block_of(0), q);
   SiteRef<LPT> nxt = cur;
+  if (OPT & OPT_PDL) {
+    // let the next launch of the stream be scheduled as soon as every CTA of this one has started,
+    // then wait until the previous launch has completed and its stores are visible
+    pdl_prologue_done();
+  }
   if (STAGES == 1) {
     // nothing in flight yet
   } else {
@@ -333,8 +340,12 @@ static cudaError_t launch_staged(void* links, const Geom& g, int parity, Power o
   // instead of a persistent grid-stride loop
   int grid = (OPT & OPT_FLAT) ? n_site_blocks : sm_count() * MINB;
   if (grid > n_site_blocks) grid = n_site_blocks;
-  kern<<<grid, BLOCK, smem, st>>>((Vec*)links, g, parity, omega, n_site_blocks,
-                                  win_reverse >= 0 ? win_reverse : ((reverse_odd && parity) ? 1 : 0), win_lo);
+  const int rev = win_reverse >= 0 ? win_reverse : ((reverse_odd && parity) ? 1 : 0);
+  if (OPT & OPT_PDL) {
+    return launch_pdl(kern, dim3((unsigned)grid), dim3(BLOCK), smem, st, (Vec*)links, g, parity, omega,
+                      n_site_blocks, rev, win_lo);
+  }
+  kern<<<grid, BLOCK, smem, st>>>((Vec*)links, g, parity, omega, n_site_blocks, rev, win_lo);
   return cudaGetLastError();
 }
 
@@ -349,17 +360,17 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
   if (coulomb) {   // Coulomb gauge: the production mapping of each format with K from spatial links
     if (variant != 20) return cudaErrorInvalidValue;
     if (d.precision == 32 && d.params == 12)
-      return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
+      return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT | OPT_PDL | OPT_COULOMB>(links, g, parity, omega, true, st);
     if (d.precision == 32)
-      return launch_staged<Storage<float, 3, 18>, double, 1, 64, 1, 5, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
+      return launch_staged<Storage<float, 3, 18>, double, 1, 64, 1, 5, OPT_FLAT | OPT_PDL | OPT_COULOMB>(links, g, parity, omega, true, st);
     if (d.params == 12)
-      return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
-    return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT | OPT_COULOMB>(links, g, parity, omega, true, st);
+      return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT | OPT_PDL | OPT_COULOMB>(links, g, parity, omega, true, st);
+    return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT | OPT_PDL | OPT_COULOMB>(links, g, parity, omega, true, st);
   }
   if (d.precision == 32 && d.params == 12) {
     typedef Storage<float, 3, 12> S;
     switch (variant) {
-      case 20: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 20: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT | OPT_PDL>(links, g, parity, omega, true, st);
       case 21: return launch_staged<S, double, 1, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
       case 22: return launch_staged<S, double, 1, 128, 2, 2, 0>(links, g, parity, omega, true, st);          // pers, 2 stages
       case 23: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
@@ -372,13 +383,14 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
       case 32: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT | OPT_NOSOLVE>(links, g, parity, omega, true, st);
       case 30: return launch_staged<S, double, 1, 256, 1, 2, OPT_FLAT>(links, g, parity, omega, true, st);
       case 31: return launch_staged<S, double, 1, 32, 1, 16, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 33: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT>(links, g, parity, omega, true, st);            // no PDL
       default: return cudaErrorInvalidValue;
     }
   }
   if (d.precision == 32) {
     typedef Storage<float, 3, 18> S;
     switch (variant) {
-      case 20: return launch_staged<S, double, 1, 64, 1, 5, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 20: return launch_staged<S, double, 1, 64, 1, 5, OPT_FLAT | OPT_PDL>(links, g, parity, omega, true, st);
       case 21: return launch_staged<S, double, 1, 128, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
       case 22: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
       case 23: return launch_staged<S, double, 2, 256, 1, 2, OPT_FLAT>(links, g, parity, omega, true, st);
@@ -389,7 +401,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
   if (d.params == 12) {
     typedef Storage<double, 3, 12> S;
     switch (variant) {
-      case 20: return launch_staged<S, double, 1, 64, 1, 4, OPT_FLAT>(links, g, parity, omega, true, st);
+      case 20: return launch_staged<S, double, 1, 64, 1, 4, OPT_FLAT | OPT_PDL>(links, g, parity, omega, true, st);
       case 21: return launch_staged<S, double, 1, 128, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
       case 22: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
       case 23: return launch_staged<S, double, 4, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 4 tps, pers
@@ -399,7 +411,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
   }
   typedef Storage<double, 3, 18> S;
   switch (variant) {
-    case 20: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT>(links, g, parity, omega, true, st);
+    case 20: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT | OPT_PDL>(links, g, parity, omega, true, st);
     case 21: return launch_staged<S, double, 1, 192, 1, 1, 0>(links, g, parity, omega, true, st);            // pers
     case 22: return launch_staged<S, double, 2, 192, 1, 2, 0>(links, g, parity, omega, true, st);            // 2 tps, pers
     case 23: return launch_staged<S, double, 4, 256, 1, 2, 0>(links, g, parity, omega, true, st);            // 4 tps, pers
@@ -409,6 +421,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
     case 28: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT | OPT_NOMATH>(links, g, parity, omega, true, st);
     case 30: return launch_staged<S, double, 1, 192, 1, 1, OPT_FLAT>(links, g, parity, omega, true, st);
     case 31: return launch_staged<S, double, 1, 32, 1, 6, OPT_FLAT>(links, g, parity, omega, true, st);
+    case 33: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT>(links, g, parity, omega, true, st);              // no PDL
     case 32: return launch_staged<S, double, 1, 96, 2, 1, 0>(links, g, parity, omega, true, st);             // pers, 2 stages
     default: return cudaErrorInvalidValue;
   }
@@ -504,12 +517,12 @@ static cudaError_t launch_production(const LatticeDesc& d, void* links, int pari
   const Geom& g = d.geom;
   if (d.group != 3) return cudaErrorInvalidValue;
   if (d.precision == 32 && d.params == 12)
-    return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT>(links, g, parity, pw, true, st);
+    return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT | OPT_PDL>(links, g, parity, pw, true, st);
   if (d.precision == 32)
-    return launch_staged<Storage<float, 3, 18>, double, 1, 64, 1, 5, OPT_FLAT>(links, g, parity, pw, true, st);
+    return launch_staged<Storage<float, 3, 18>, double, 1, 64, 1, 5, OPT_FLAT | OPT_PDL>(links, g, parity, pw, true, st);
   if (d.params == 12)
-    return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT>(links, g, parity, pw, true, st);
-  return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT>(links, g, parity, pw, true, st);
+    return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT | OPT_PDL>(links, g, parity, pw, true, st);
+  return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT | OPT_PDL>(links, g, parity, pw, true, st);
 }
 
 cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int parity, const SeriesPower& pw,
