@@ -46,6 +46,11 @@ constexpr int OPT_STREAM_ST = 32;  // st.global.cs stores
 constexpr int OPT_NOSOLVE = 256;   // measurement only: K is accumulated but G = 1 (no subgroup solve)
 constexpr int OPT_PDL = 512;       // programmatic dependent launch: the next half-sweep's CTAs are scheduled
                                    // (index arithmetic done) while this one's last wave drains
+constexpr int OPT_L2HINT = 1024;   // flat grid only: L2 eviction hints by position in the traversal.  The CTAs from
+                                   // `late_from` on (the last ~90 MB of links a launch touches, which the next,
+                                   // reversed launch revisits first) store with evict_last and load normally; the
+                                   // earlier ones load with evict_first (their lines cannot survive until they are
+                                   // revisited) and store normally.  late_from < 0: no preference anywhere.
 constexpr int OPT_COULOMB = 64;    // Coulomb gauge (reading C-22): K(x) from the 6 spatial links only
 
 __device__ __forceinline__ void cp_async_vec(float4* smem, const float4* gmem) {
@@ -75,6 +80,18 @@ __device__ __forceinline__ void st_cs(float4* p, const float4& v) {
 }
 __device__ __forceinline__ void st_cs(double2* p, const double2& v) {
   asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void st_hint(float4* p, const float4& v, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z),
+               "f"(v.w), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_hint(double2* p, const double2& v, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+template <typename V>
+__device__ __forceinline__ void cp_async_vec_hint(V* smem, const V* gmem, uint64_t pol) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void prefetch_l2(const void* gmem) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(gmem));
@@ -126,7 +143,7 @@ template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, in
 __global__ void __launch_bounds__(BLOCK, MINB)
 or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
                            const Power omega, const int n_site_blocks, const int reverse,
-                           const int block_lo) {
+                           const int block_lo, const int late_from) {
   typedef typename S::Real Real;
   typedef typename S::Vec Vec;
   constexpr int LPT = 8 / TPS;          // links per thread
@@ -144,14 +161,28 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
     const int b = (OPT & OPT_CHUNKED) ? (int)blockIdx.x * per_cta + it : it * (int)gridDim.x + (int)blockIdx.x;
     return block_lo + (reverse ? n_site_blocks - 1 - b : b);   // window [block_lo, block_lo + n_site_blocks)
   };
+  constexpr bool L2HINT = (OPT & OPT_L2HINT) != 0;
+  uint64_t pol = 0, pol_st = 0;
+  if (L2HINT) {
+    uint64_t pf, pn, pl;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pf));
+    asm("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pn));
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pl));
+    const bool late = (int)blockIdx.x >= late_from;
+    pol = (late_from < 0 || late) ? pn : pf;
+    pol_st = (late_from >= 0 && late) ? pl : pn;
+  }
   auto issue = [&](const SiteRef<LPT>& r, int stage) {
     if (r.active) {
 #pragma unroll
       for (int l = 0; l < LPT; ++l) {
 #pragma unroll
-        for (int j = 0; j < NV; ++j)
-          cp_async_vec(sm + (size_t)((stage * NVT + l * NV + j) * BLOCK),
-                       vec_ptr<S, LPT>(links, g, parity, r, q, l, j));
+        for (int j = 0; j < NV; ++j) {
+          if (L2HINT) cp_async_vec_hint(sm + (size_t)((stage * NVT + l * NV + j) * BLOCK),
+                                        (const Vec*)vec_ptr<S, LPT>(links, g, parity, r, q, l, j), pol);
+          else cp_async_vec(sm + (size_t)((stage * NVT + l * NV + j) * BLOCK),
+                            vec_ptr<S, LPT>(links, g, parity, r, q, l, j));
+        }
       }
     }
     cp_async_commit();
@@ -294,7 +325,8 @@ or_sweep_su3_staged_kernel(typename S::Vec* __restrict__ links, const Geom g, co
         for (int j = 0; j < NV; ++j) {
           Vec v;
           vec_set(v, R + j * S::VL);
-          if (OPT & OPT_STREAM_ST) st_cs(vec_ptr<S, LPT>(links, g, parity, cur, q, l, j), v);
+          if (L2HINT) st_hint(vec_ptr<S, LPT>(links, g, parity, cur, q, l, j), v, pol_st);
+          else if (OPT & OPT_STREAM_ST) st_cs(vec_ptr<S, LPT>(links, g, parity, cur, q, l, j), v);
           else *vec_ptr<S, LPT>(links, g, parity, cur, q, l, j) = v;
         }
       }
@@ -324,6 +356,15 @@ template <typename S, typename Acc, int TPS, int BLOCK, int STAGES, int MINB, in
 static cudaError_t launch_staged(void* links, const Geom& g, int parity, Power omega, bool reverse_odd,
                                  cudaStream_t st, int win_lo = 0, int win_n = -1, int win_reverse = -1) {
   typedef typename S::Vec Vec;
+  if constexpr ((OPT & OPT_L2HINT) != 0) {
+    // The hints pay where the field is a small multiple of the 126 MB L2 (measured: 201 MB 58.4 -> 55.0 us,
+    // 604 MB 177.3 -> 176.9, 2.0 GB 617 -> 627, 9.7 GB 2863 -> 2924): elsewhere, and for the windowed
+    // (slab) launches, the same mapping without them.
+    const double field_bytes = 8.0 * (double)g.vh * S::NV * sizeof(Vec);
+    if (win_n >= 0 || field_bytes < 110e6 || field_bytes > 700e6)
+      return launch_staged<S, Acc, TPS, BLOCK, STAGES, MINB, OPT & ~OPT_L2HINT, Power>(links, g, parity, omega, reverse_odd,
+                                                                                       st, win_lo, win_n, win_reverse);
+  }
   auto kern = or_sweep_su3_staged_kernel<S, Acc, TPS, BLOCK, STAGES, MINB, OPT, Power>;
   constexpr size_t smem = (size_t)STAGES * (8 / TPS) * S::NV * BLOCK * sizeof(Vec);
   static bool configured = false;
@@ -341,11 +382,14 @@ static cudaError_t launch_staged(void* links, const Geom& g, int parity, Power o
   int grid = (OPT & OPT_FLAT) ? n_site_blocks : sm_count() * MINB;
   if (grid > n_site_blocks) grid = n_site_blocks;
   const int rev = win_reverse >= 0 ? win_reverse : ((reverse_odd && parity) ? 1 : 0);
+  // the last ~90 MB of links of the traversal are kept in L2 for the next (reversed) launch
+  int late_from = -1;
+  if (OPT & OPT_L2HINT) late_from = grid - (int)((double)grid * (90e6 / (8.0 * (double)g.vh * S::NV * sizeof(Vec))));
   if (OPT & OPT_PDL) {
     return launch_pdl(kern, dim3((unsigned)grid), dim3(BLOCK), smem, st, (Vec*)links, g, parity, omega,
-                      n_site_blocks, rev, win_lo);
+                      n_site_blocks, rev, win_lo, late_from);
   }
-  kern<<<grid, BLOCK, smem, st>>>((Vec*)links, g, parity, omega, n_site_blocks, rev, win_lo);
+  kern<<<grid, BLOCK, smem, st>>>((Vec*)links, g, parity, omega, n_site_blocks, rev, win_lo, late_from);
   return cudaGetLastError();
 }
 
@@ -360,17 +404,17 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
   if (coulomb) {   // Coulomb gauge: the production mapping of each format with K from spatial links
     if (variant != 20) return cudaErrorInvalidValue;
     if (d.precision == 32 && d.params == 12)
-      return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT | OPT_PDL | OPT_COULOMB>(links, g, parity, omega, true, st);
+      return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT | OPT_PDL | OPT_L2HINT | OPT_COULOMB>(links, g, parity, omega, true, st);
     if (d.precision == 32)
-      return launch_staged<Storage<float, 3, 18>, double, 1, 64, 1, 5, OPT_FLAT | OPT_PDL | OPT_COULOMB>(links, g, parity, omega, true, st);
+      return launch_staged<Storage<float, 3, 18>, double, 1, 64, 1, 5, OPT_FLAT | OPT_PDL | OPT_L2HINT | OPT_COULOMB>(links, g, parity, omega, true, st);
     if (d.params == 12)
-      return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT | OPT_PDL | OPT_COULOMB>(links, g, parity, omega, true, st);
-    return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT | OPT_PDL | OPT_COULOMB>(links, g, parity, omega, true, st);
+      return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT | OPT_PDL | OPT_L2HINT | OPT_COULOMB>(links, g, parity, omega, true, st);
+    return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT | OPT_PDL | OPT_L2HINT | OPT_COULOMB>(links, g, parity, omega, true, st);
   }
   if (d.precision == 32 && d.params == 12) {
     typedef Storage<float, 3, 12> S;
     switch (variant) {
-      case 20: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT | OPT_PDL>(links, g, parity, omega, true, st);
+      case 20: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT | OPT_PDL | OPT_L2HINT>(links, g, parity, omega, true, st);
       case 21: return launch_staged<S, double, 1, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
       case 22: return launch_staged<S, double, 1, 128, 2, 2, 0>(links, g, parity, omega, true, st);          // pers, 2 stages
       case 23: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
@@ -384,13 +428,14 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
       case 30: return launch_staged<S, double, 1, 256, 1, 2, OPT_FLAT>(links, g, parity, omega, true, st);
       case 31: return launch_staged<S, double, 1, 32, 1, 16, OPT_FLAT>(links, g, parity, omega, true, st);
       case 33: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT>(links, g, parity, omega, true, st);            // no PDL
+      case 34: return launch_staged<S, double, 1, 128, 1, 4, OPT_FLAT | OPT_PDL>(links, g, parity, omega, true, st);  // no L2 hints
       default: return cudaErrorInvalidValue;
     }
   }
   if (d.precision == 32) {
     typedef Storage<float, 3, 18> S;
     switch (variant) {
-      case 20: return launch_staged<S, double, 1, 64, 1, 5, OPT_FLAT | OPT_PDL>(links, g, parity, omega, true, st);
+      case 20: return launch_staged<S, double, 1, 64, 1, 5, OPT_FLAT | OPT_PDL | OPT_L2HINT>(links, g, parity, omega, true, st);
       case 21: return launch_staged<S, double, 1, 128, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
       case 22: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
       case 23: return launch_staged<S, double, 2, 256, 1, 2, OPT_FLAT>(links, g, parity, omega, true, st);
@@ -401,7 +446,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
   if (d.params == 12) {
     typedef Storage<double, 3, 12> S;
     switch (variant) {
-      case 20: return launch_staged<S, double, 1, 64, 1, 4, OPT_FLAT | OPT_PDL>(links, g, parity, omega, true, st);
+      case 20: return launch_staged<S, double, 1, 64, 1, 4, OPT_FLAT | OPT_PDL | OPT_L2HINT>(links, g, parity, omega, true, st);
       case 21: return launch_staged<S, double, 1, 128, 1, 2, 0>(links, g, parity, omega, true, st);          // pers
       case 22: return launch_staged<S, double, 2, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 2 tps, pers
       case 23: return launch_staged<S, double, 4, 256, 1, 2, 0>(links, g, parity, omega, true, st);          // 4 tps, pers
@@ -411,7 +456,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
   }
   typedef Storage<double, 3, 18> S;
   switch (variant) {
-    case 20: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT | OPT_PDL>(links, g, parity, omega, true, st);
+    case 20: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT | OPT_PDL | OPT_L2HINT>(links, g, parity, omega, true, st);
     case 21: return launch_staged<S, double, 1, 192, 1, 1, 0>(links, g, parity, omega, true, st);            // pers
     case 22: return launch_staged<S, double, 2, 192, 1, 2, 0>(links, g, parity, omega, true, st);            // 2 tps, pers
     case 23: return launch_staged<S, double, 4, 256, 1, 2, 0>(links, g, parity, omega, true, st);            // 4 tps, pers
@@ -422,6 +467,7 @@ cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity
     case 30: return launch_staged<S, double, 1, 192, 1, 1, OPT_FLAT>(links, g, parity, omega, true, st);
     case 31: return launch_staged<S, double, 1, 32, 1, 6, OPT_FLAT>(links, g, parity, omega, true, st);
     case 33: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT>(links, g, parity, omega, true, st);              // no PDL
+    case 34: return launch_staged<S, double, 1, 64, 1, 3, OPT_FLAT | OPT_PDL>(links, g, parity, omega, true, st);    // no L2 hints
     case 32: return launch_staged<S, double, 1, 96, 2, 1, 0>(links, g, parity, omega, true, st);             // pers, 2 stages
     default: return cudaErrorInvalidValue;
   }
@@ -517,12 +563,12 @@ static cudaError_t launch_production(const LatticeDesc& d, void* links, int pari
   const Geom& g = d.geom;
   if (d.group != 3) return cudaErrorInvalidValue;
   if (d.precision == 32 && d.params == 12)
-    return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT | OPT_PDL>(links, g, parity, pw, true, st);
+    return launch_staged<Storage<float, 3, 12>, double, 1, 128, 1, 4, OPT_FLAT | OPT_PDL | OPT_L2HINT>(links, g, parity, pw, true, st);
   if (d.precision == 32)
-    return launch_staged<Storage<float, 3, 18>, double, 1, 64, 1, 5, OPT_FLAT | OPT_PDL>(links, g, parity, pw, true, st);
+    return launch_staged<Storage<float, 3, 18>, double, 1, 64, 1, 5, OPT_FLAT | OPT_PDL | OPT_L2HINT>(links, g, parity, pw, true, st);
   if (d.params == 12)
-    return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT | OPT_PDL>(links, g, parity, pw, true, st);
-  return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT | OPT_PDL>(links, g, parity, pw, true, st);
+    return launch_staged<Storage<double, 3, 12>, double, 1, 64, 1, 4, OPT_FLAT | OPT_PDL | OPT_L2HINT>(links, g, parity, pw, true, st);
+  return launch_staged<Storage<double, 3, 18>, double, 1, 64, 1, 3, OPT_FLAT | OPT_PDL | OPT_L2HINT>(links, g, parity, pw, true, st);
 }
 
 cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int parity, const SeriesPower& pw,
