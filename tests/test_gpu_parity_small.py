@@ -49,14 +49,14 @@ def variants_for(precision, params):
     """0 = production mapping (= staged variant 20); 1..8 = direct register kernels with that
     many threads per site; 20+ = shared-memory staged mappings (table in or_sweep_staged.cu):
     flat / persistent grids, 1-2 stages, 1/2/4 threads per site, prefetch, chunked, stream stores,
-    33 = the production mapping without programmatic dependent launch."""
+    33 = the production mapping without programmatic dependent launch, 34 = without L2 eviction hints."""
     if precision == 32 and params == 12:
-        return [0, 1, 2, 4, 21, 22, 23, 24, 26, 27, 29, 30, 31, 33]
+        return [0, 1, 2, 4, 21, 22, 23, 24, 26, 27, 29, 30, 31, 33, 34]
     if precision == 32:
         return [0, 2, 4, 21, 22, 23, 24]
     if params == 12:
         return [0, 2, 4, 8, 21, 22, 23, 24]
-    return [0, 4, 8, 21, 22, 23, 24, 26, 27, 30, 31, 32, 33]
+    return [0, 4, 8, 21, 22, 23, 24, 26, 27, 30, 31, 32, 33, 34]
 
 
 @pytest.mark.parametrize("dims", DIMS)
