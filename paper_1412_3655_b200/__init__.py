@@ -16,7 +16,9 @@ import os
 from dataclasses import dataclass
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libculgt_b200.so")
+# CULGT_MEASURE=1 selects the separately built measurement library (build.py --measure); default: the product
+LIB_PATH = os.path.join(_HERE, "libculgt_b200_measure.so" if os.environ.get("CULGT_MEASURE", "") not in ("", "0")
+                        else "libculgt_b200.so")
 
 CULGT_OK = 0
 ERRORS = {
@@ -64,6 +66,7 @@ def lib() -> ctypes.CDLL:
     L.culgt_reunitarize.argtypes = [latp, vp, vp]
     L.culgt_or_sweep.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_or_sweeps.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
+    L.culgt_or_sweeps_ws.argtypes = [latp, vp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_gauge_precision.argtypes = [latp, vp, vp, vp, vp]
     L.culgt_functional.argtypes = [latp, vp, vp, vp, vp]
     L.culgt_gauge_precision_functional.argtypes = [latp, vp, vp, vp, vp, vp]
@@ -86,7 +89,7 @@ def lib() -> ctypes.CDLL:
     L.culgt_coulomb_fix.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
                                     ctypes.POINTER(ctypes.c_int), dp, dp, vp]
     L.culgt_set_sweep_variant.argtypes = [ctypes.c_int]
-    L.culgt_autotune_sweep.argtypes = [latp, vp, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int),
+    L.culgt_autotune_sweep.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int),
                                        ctypes.POINTER(ctypes.c_float), vp]
     L.culgt_strerror.argtypes = [ctypes.c_int]
     L.culgt_strerror.restype = ctypes.c_char_p
@@ -217,6 +220,12 @@ def culgt_or_sweeps(lat: Lattice, links, n_sweeps: int, omega: float, stream=Non
     _require_cuda()
     _check(lib().culgt_or_sweeps(ctypes.byref(lat.c()), _ptr(links), int(n_sweeps), float(omega),
                                  _stream(stream)), "culgt_or_sweeps")
+
+
+def culgt_or_sweeps_ws(lat: Lattice, links, workspace, n_sweeps: int, omega: float, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_or_sweeps_ws(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace), int(n_sweeps),
+                                    float(omega), _stream(stream)), "culgt_or_sweeps_ws")
 
 
 def culgt_gauge_precision(lat: Lattice, links, workspace, theta_dev, stream=None) -> None:
@@ -367,19 +376,31 @@ def culgt_set_sweep_variant(variant: int) -> None:
     _check(lib().culgt_set_sweep_variant(int(variant)), "culgt_set_sweep_variant")
 
 
-def culgt_autotune_sweep(lat: Lattice, links, omega: float, sweeps_per_trial: int = 3, stream=None):
-    """Times every result-equivalent sweep mapping on `links` (real sweeps), selects the fastest
-    process-wide.  Returns (variant, microseconds per half-sweep)."""
+def culgt_autotune_sweep(lat: Lattice, links, workspace, omega: float, sweeps_per_trial: int = 3, stream=None):
+    """Times every result-equivalent sweep schedule on `links` (real sweeps), selects the fastest
+    for the calling thread.  Returns (variant, microseconds per half-sweep)."""
     _require_cuda()
     v = ctypes.c_int(0)
     us = ctypes.c_float(0.0)
-    _check(lib().culgt_autotune_sweep(ctypes.byref(lat.c()), _ptr(links), float(omega), int(sweeps_per_trial),
+    _check(lib().culgt_autotune_sweep(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace), float(omega),
+                                      int(sweeps_per_trial),
                                       ctypes.byref(v), ctypes.byref(us), _stream(stream)), "culgt_autotune_sweep")
     return v.value, us.value
 
 
 def culgt_get_sweep_variant() -> int:
     return lib().culgt_get_sweep_variant()
+
+
+def culgt_fused_schedule(n_slices: int, lag: int, direction: int):
+    """[(parity, slice), ...] in the order the fused full sweep hands out its slice-tasks (host only)."""
+    buf = (ctypes.c_uint * (2 * int(n_slices)))()
+    _check(lib().culgt_fused_schedule(int(n_slices), int(lag), int(direction), buf), "culgt_fused_schedule")
+    return [(w >> 31, w & 0x7FFFFFFF) for w in buf]
+
+
+def culgt_measure_build() -> bool:
+    return bool(lib().culgt_measure_build())
 
 
 def culgt_version() -> int:

@@ -12,8 +12,11 @@ using namespace culgt;
 
 namespace {
 
-char g_cuda_err[256] = "";
-int g_variant = 0;
+// Per host thread: the text of the last CUDA error and the sweep-variant selection.  The library has
+// no process-global mutable state beyond caches of device properties and of lazily-set function
+// attributes (both per device).
+thread_local char g_cuda_err[256] = "";
+thread_local int g_variant = 0;
 
 int cuda_fail(cudaError_t e) {
   snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
@@ -75,7 +78,8 @@ size_t culgt_gfield_bytes(const culgt_lattice* lat) {
 size_t culgt_workspace_bytes(const culgt_lattice* lat) {
   LatticeDesc d;
   if (describe(lat, &d) != CULGT_OK) return 0;
-  return reduce_workspace_doubles(d.geom) * sizeof(double);   // block partials + 2 * N3 result slots
+  // block partials + 2 * N3 result slots + the Coulomb mask + the driver-loop and fused-sweep control blocks
+  return workspace_doubles(d.geom) * sizeof(double);
 }
 
 int culgt_pack(const culgt_lattice* lat, const void* canonical, void* links, void* stream) {
@@ -133,11 +137,22 @@ int culgt_or_sweeps(const culgt_lattice* lat, void* links, int n_sweeps, double 
   if (misaligned(links)) return CULGT_ERR_ALIGN;
   if (n_sweeps < 0) return CULGT_ERR_ARG;
   if ((rc = check_omega(omega)) != CULGT_OK) return rc;
-  for (int i = 0; i < n_sweeps; ++i) {
-    cudaError_t e = launch_or_full_sweep(d, links, omega, g_variant, (cudaStream_t)stream);
-    if (e != cudaSuccess) return cuda_fail(e);
-  }
-  return CULGT_OK;
+  cudaError_t e = launch_or_full_sweeps(d, links, nullptr, n_sweeps, omega, g_variant, nullptr, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_or_sweeps_ws(const culgt_lattice* lat, void* links, void* workspace, int n_sweeps, double omega,
+                       void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !workspace) return CULGT_ERR_NULL;
+  if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
+  if (n_sweeps < 0) return CULGT_ERR_ARG;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  cudaError_t e = launch_or_full_sweeps(d, links, (double*)workspace, n_sweeps, omega, g_variant, nullptr,
+                                        (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
 int culgt_gauge_precision(const culgt_lattice* lat, const void* links, void* workspace,
@@ -203,6 +218,11 @@ static int read_theta_F(const LatticeDesc& d, const void* links, void* workspace
   return CULGT_OK;
 }
 
+// The driver loop runs on the DEVICE between synchronisations: every check's final reduction kernel
+// records theta and F in a control block in the workspace and raises its stop word once
+// theta < theta_target; sweeps and checks enqueued behind a raised stop word return at entry.  The
+// host enqueues rounds of (check_every sweeps + one check) in batches and reads the control block back
+// once per batch, instead of once per check.
 int culgt_landau_fix(const culgt_lattice* lat, void* links, void* workspace, double omega,
                      double theta_target, int max_sweeps, int check_every,
                      int* sweeps_done, double* theta_out, double* F_out, void* stream) {
@@ -214,23 +234,34 @@ int culgt_landau_fix(const culgt_lattice* lat, void* links, void* workspace, dou
   if (max_sweeps < 0 || check_every < 1) return CULGT_ERR_ARG;
   if ((rc = check_omega(omega)) != CULGT_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  double theta = 0, F = 0;
-  int done = 0;
-  if ((rc = read_theta_F(d, links, workspace, st, &theta, nullptr)) != CULGT_OK) return rc;
-  while (theta >= theta_target && done < max_sweeps) {
-    int n = check_every;
-    if (done + n > max_sweeps) n = max_sweeps - done;
-    for (int i = 0; i < n; ++i) {
-      cudaError_t e = launch_or_full_sweep(d, links, omega, g_variant, st);
-      if (e != cudaSuccess) return cuda_fail(e);
+  double* ws = (double*)workspace;
+  double* scal = ws + reduce_partial_doubles(d.geom);
+  FixCtl* ctl = (FixCtl*)(ws + fix_ctl_offset_doubles(d.geom));
+  cudaError_t e = cudaMemsetAsync(ctl, 0, sizeof(FixCtl), st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  FixCheck chk = {ctl, theta_target, 0};
+  if ((e = launch_theta_functional(d, links, ws, scal, scal + 1, st, &chk)) != cudaSuccess) return cuda_fail(e);
+  // rounds per synchronisation: about 32 sweeps' worth of launches, so that a small lattice is not
+  // bound by the host round trip and a stopped run wastes at most that many empty launches
+  const int rounds_per_sync = check_every >= 32 ? 1 : 32 / check_every;
+  FixCtl host;
+  int enqueued = 0;
+  for (;;) {
+    for (int r = 0; r < rounds_per_sync && enqueued < max_sweeps; ++r) {
+      int n = check_every;
+      if (enqueued + n > max_sweeps) n = max_sweeps - enqueued;
+      if ((e = launch_or_full_sweeps(d, links, ws, n, omega, g_variant, &ctl->stop, st)) != cudaSuccess) return cuda_fail(e);
+      enqueued += n;
+      chk.sweeps_before = enqueued;
+      if ((e = launch_theta_functional(d, links, ws, scal, scal + 1, st, &chk)) != cudaSuccess) return cuda_fail(e);
     }
-    done += n;
-    if ((rc = read_theta_F(d, links, workspace, st, &theta, nullptr)) != CULGT_OK) return rc;
+    if ((e = cudaMemcpyAsync(&host, ctl, sizeof(FixCtl), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+    if (host.stop || enqueued >= max_sweeps) break;
   }
-  if ((rc = read_theta_F(d, links, workspace, st, &theta, &F)) != CULGT_OK) return rc;
-  if (sweeps_done) *sweeps_done = done;
-  if (theta_out) *theta_out = theta;
-  if (F_out) *F_out = F;
+  if (sweeps_done) *sweeps_done = host.stop ? host.sweeps_at_stop : enqueued;
+  if (theta_out) *theta_out = host.theta;
+  if (F_out) *F_out = host.F;
   return CULGT_OK;
 }
 
@@ -249,8 +280,8 @@ int culgt_fix_host(const culgt_lattice* lat, void* canonical_host, void* canonic
   cudaError_t e = cudaMemcpyAsync(canonical_dev, canonical_host, cbytes, cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess) return cuda_fail(e);
   if ((e = launch_pack(d, canonical_dev, links_dev, st)) != cudaSuccess) return cuda_fail(e);
-  for (int i = 0; i < n_sweeps; ++i)
-    if ((e = launch_or_full_sweep(d, links_dev, omega, g_variant, st)) != cudaSuccess) return cuda_fail(e);
+  if ((e = launch_or_full_sweeps(d, links_dev, (double*)workspace, n_sweeps, omega, g_variant, nullptr, st)) != cudaSuccess)
+    return cuda_fail(e);
   if ((e = launch_unpack(d, links_dev, canonical_dev, st)) != cudaSuccess) return cuda_fail(e);
   e = cudaMemcpyAsync(canonical_host, canonical_dev, cbytes, cudaMemcpyDeviceToHost, st);
   if (e != cudaSuccess) return cuda_fail(e);
@@ -495,32 +526,33 @@ int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, do
 }
 
 // Run-time autotuner (the paper's selection of the fastest kernel set-up per GPU at run time,
-// P:L89 (d)): times every result-equivalent sweep mapping built for this storage format
-// on the caller's field and makes the fastest one the process-wide choice.
-int culgt_autotune_sweep(const culgt_lattice* lat, void* links, double omega, int sweeps_per_trial,
-                         int* best_variant, float* best_us_per_half_sweep, void* stream) {
+// P:L89 (d)): times every result-equivalent sweep schedule built for this storage format
+// on the caller's field and makes the fastest one the calling thread's choice.
+int culgt_autotune_sweep(const culgt_lattice* lat, void* links, void* workspace, double omega,
+                         int sweeps_per_trial, int* best_variant, float* best_us_per_half_sweep, void* stream) {
   LatticeDesc d;
   int rc = describe(lat, &d);
   if (rc != CULGT_OK) return rc;
-  if (!links) return CULGT_ERR_NULL;
-  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (!links || !workspace) return CULGT_ERR_NULL;
+  if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
   if (sweeps_per_trial < 1) return CULGT_ERR_ARG;
   if ((rc = check_omega(omega)) != CULGT_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   cudaEvent_t e0, e1;
-  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return cuda_fail(cudaGetLastError());
+  if (cudaEventCreate(&e0) != cudaSuccess) return cuda_fail(cudaGetLastError());
+  if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); return cuda_fail(cudaGetLastError()); }
   int best = 0;
   float best_us = -1.f;
-  for (int v = 0; v < 40; ++v) {
+  for (int v = 1; v < 64; ++v) {
+    if (!sweep_variant_known(v)) continue;
     // 11, 14, 25: all-fp32 arithmetic (different precision); 28, 32: measurement-only (no solve)
     if (v == 11 || v == 14 || v == 25 || v == 28 || v == 32) continue;
-    if (d.group == 2 && v != 0) continue;
-    cudaError_t e = cudaSuccess;
-    e = launch_or_full_sweep(d, links, omega, v, st);
-    if (e == cudaErrorInvalidValue) continue;                     // mapping not built for this format
+    if (d.group == 2 && v != 20) continue;
+    cudaError_t e = launch_or_full_sweeps(d, links, (double*)workspace, 1, omega, v, nullptr, st);
+    if (e == cudaErrorInvalidValue) { cudaGetLastError(); continue; }   // mapping not built for this format
     if (e != cudaSuccess) { rc = cuda_fail(e); break; }
     cudaEventRecord(e0, st);
-    for (int i = 0; i < sweeps_per_trial && e == cudaSuccess; ++i) e = launch_or_full_sweep(d, links, omega, v, st);
+    e = launch_or_full_sweeps(d, links, (double*)workspace, sweeps_per_trial, omega, v, nullptr, st);
     cudaEventRecord(e1, st);
     if (e == cudaSuccess) e = cudaEventSynchronize(e1);
     if (e != cudaSuccess) { rc = cuda_fail(e); break; }
@@ -538,12 +570,26 @@ int culgt_autotune_sweep(const culgt_lattice* lat, void* links, double omega, in
   return CULGT_OK;
 }
 
+int culgt_fused_schedule(int n_slices, int lag, int direction, unsigned* tasks_out) {
+  if (!tasks_out) return CULGT_ERR_NULL;
+  if (n_slices < 2 || (n_slices & 1) || n_slices > kFusedMaxSlices || (direction != 0 && direction != 1)) return CULGT_ERR_ARG;
+  fused_schedule(n_slices, lag, direction, tasks_out);
+  return CULGT_OK;
+}
+
 int culgt_set_sweep_variant(int variant) {
-  if (variant < 0 || variant > 99) return CULGT_ERR_ARG;
+  if (!sweep_variant_known(variant)) return CULGT_ERR_ARG;
   g_variant = variant;
   return CULGT_OK;
 }
 int culgt_get_sweep_variant(void) { return g_variant; }
+int culgt_measure_build(void) {
+#ifdef CULGT_MEASURE
+  return 1;
+#else
+  return 0;
+#endif
+}
 
 const char* culgt_strerror(int status) {
   switch (status) {
@@ -560,6 +606,6 @@ const char* culgt_strerror(int status) {
   }
 }
 const char* culgt_last_cuda_error(void) { return g_cuda_err; }
-int culgt_version(void) { return 100; }
+int culgt_version(void) { return 200; }
 
 }  // extern "C"

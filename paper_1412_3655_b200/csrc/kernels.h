@@ -1,6 +1,7 @@
 // kernels.h -- internal (C++) interface between the C-ABI layer (api.cu) and the kernel files.
 #pragma once
 #include <cuda_runtime.h>
+#include <stddef.h>
 #include "lattice.cuh"
 
 namespace culgt {
@@ -12,6 +13,10 @@ struct LatticeDesc {
   int params;     // 18, 12 or 4
   long long V;
 };
+
+constexpr int kMaxDevices = 64;         // per-device caches (function attributes, SM count, L2 size)
+int device_sm_count();                  // of the current device
+double device_l2_bytes();
 
 constexpr int kReduceBlock = 256;       // threads per block of the reduction kernels
 // CTAs (= partials per quantity) of the fused theta+F kernel: `half` sites of each parity per CTA
@@ -31,9 +36,55 @@ inline size_t reduce_workspace_doubles(const Geom& g) {
   return reduce_partial_doubles(g) + 2 * (size_t)g.n[3] + ((size_t)g.n[3] + 7) / 8;
 }
 
-// coulomb = true: Coulomb-gauge half-sweep (K from the spatial links; production mapping only)
+// ---- control blocks that live behind the reduction part of the caller's workspace ---------------
+// The library keeps no device state of its own: whatever a kernel needs to remember between
+// launches sits in the workspace the caller hands in, and is (re)initialised by the call that uses it.
+
+// Driver loop (culgt_landau_fix): written by the final reduction kernel of every check, read by
+// the sweep and reduction kernels enqueued behind it (they return at entry once `stop` is set).
+struct FixCtl {
+  int stop;            // 1 once a check found theta < theta_target
+  int checks_done;     // checks that ran (not skipped) so far
+  int sweeps_at_stop;  // value of `sweeps_before` of the check that set `stop`
+  int pad;
+  double theta, F;     // of the last check that ran
+};
+
+// Fused full sweep (or_sweep_fused.cu).
+constexpr int kFusedMaxSlices = 512;
+struct FusedCtl {
+  unsigned ticket;                           // next ticket of the running launch
+  unsigned exited;                           // CTAs of the running launch that have left
+  unsigned pad[30];
+  unsigned done[2][kFusedMaxSlices];         // completed site blocks per (parity, time-slice)
+  unsigned task[2][2 * kFusedMaxSlices];     // [direction][u] = parity << 31 | slice: slice-task order
+};
+
+// L2 eviction policies of the fused sweep (2 bits each: black loads, black stores, white loads, white
+// stores; 0 evict_first, 1 evict_normal, 2 evict_last), chosen by measurement
+constexpr int kFusedDefaultHints = 1 | (1 << 2) | (1 << 4) | (1 << 6);
+
+inline size_t ctl_offset_doubles(const Geom& g) { return (reduce_workspace_doubles(g) + 15) / 16 * 16; }
+inline size_t fix_ctl_offset_doubles(const Geom& g) { return ctl_offset_doubles(g); }
+inline size_t fused_ctl_offset_doubles(const Geom& g) { return ctl_offset_doubles(g) + 16; }
+inline size_t workspace_doubles(const Geom& g) { return fused_ctl_offset_doubles(g) + sizeof(FusedCtl) / 8; }
+static_assert(sizeof(FixCtl) <= 16 * 8, "FixCtl must fit its 16-double slot");
+static_assert(sizeof(FusedCtl) % 8 == 0, "FusedCtl is addressed in doubles");
+
+// ---- half-sweeps ----------------------------------------------------------------------------------
+// Product variants: 0 (= 20) production mapping; 24 no reversed odd-parity traversal; 33 no programmatic
+// dependent launch; 34 no L2 hints -- identical arithmetic, bit-identical results.  With
+// -DCULGT_MEASURE also the measured alternatives of or_sweep_measure.cu.  Others: cudaErrorInvalidValue.
+// coulomb = true: Coulomb-gauge half-sweep (K from the spatial links; production mapping only).
+// stop_flag (device, may be null): the launch does nothing if *stop_flag != 0 when it starts.
+bool sweep_variant_known(int variant);
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
-                            int variant, cudaStream_t st, bool coulomb = false);
+                            int variant, cudaStream_t st, bool coulomb = false, const int* stop_flag = nullptr);
+cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
+                                   int variant, bool coulomb, const int* stop_flag, cudaStream_t st);
+// production half-sweep restricted to the time-slices [t_lo, t_hi) (time-slab decomposition)
+cudaError_t launch_or_sweep_window(const LatticeDesc& d, void* links, int parity, double omega, int t_lo, int t_hi,
+                                   cudaStream_t st);
 struct SeriesPower;
 struct HeatBathPower;
 // simulated-annealing half-sweep (reading C-25), production mappings only
@@ -49,21 +100,40 @@ cudaError_t launch_or_sweep_series(const LatticeDesc& d, void* links, int parity
                                    cudaStream_t st);
 cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int parity, const SeriesPower& pw,
                                           cudaStream_t st);
-// One FULL sweep (black then white).  Variants 40..59 select the slab-blocked schedule of
-// or_sweep_staged.cu (40 + log2(slab slices): one stream; 50 + log2(slab slices): white windows on a
-// second stream); every other variant, and any lattice the slab schedule does not fit, is the two
-// whole half-sweeps of launch_or_sweep.
-cudaError_t launch_or_full_sweep(const LatticeDesc& d, void* links, double omega, int variant, cudaStream_t st);
-cudaError_t launch_or_sweep_staged_slabbed(const LatticeDesc& d, void* links, double omega, int slab_slices,
-                                           bool overlap, cudaStream_t st);
-cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
-                                   int variant, bool coulomb, cudaStream_t st);
+
+// ---- full sweeps ------------------------------------------------------------------------------------
+// n_sweeps FULL sweeps (black then white).  `workspace` (may be null) is the caller's reduction
+// workspace: with it, and where the lattice qualifies, the sweeps run as the fused one-kernel
+// schedule of or_sweep_fused.cu; otherwise as two half-sweep launches each.
+cudaError_t launch_or_full_sweeps(const LatticeDesc& d, void* links, double* workspace, int n_sweeps, double omega,
+                                  int variant, const int* stop_flag, cudaStream_t st);
+// the fused schedule itself: cudaErrorNotSupported when the lattice does not qualify.
+// lag <= 0: default; hints: L2 policy bits (or_sweep_fused.cu); alternate: every other sweep descending.
+cudaError_t launch_or_sweeps_fused(const LatticeDesc& d, void* links, double omega, void* ctl, int n_sweeps,
+                                   int lag, int hints, bool alternate, const int* stop_flag, cudaStream_t st);
+void fused_schedule(int n3, int lag, int dir, unsigned* out);   // host: the slice-task order (2 * n3 entries)
+#ifdef CULGT_MEASURE
+cudaError_t launch_or_sweep_measure(const LatticeDesc& d, void* links, int parity, double omega, int variant,
+                                    cudaStream_t st);
+cudaError_t launch_or_sweep_measure_slabbed(const LatticeDesc& d, void* links, double omega, int slab_slices,
+                                            cudaStream_t st);
+#endif
+
+// ---- layout, reductions, transform ----------------------------------------------------------------
 cudaError_t launch_pack(const LatticeDesc& d, const void* canonical, void* links, cudaStream_t st);
 cudaError_t launch_reunitarize(const LatticeDesc& d, void* links, cudaStream_t st);
 cudaError_t launch_unpack(const LatticeDesc& d, const void* links, void* canonical, cudaStream_t st);
-// fused theta + F; workspace holds 2 * reduce_blocks_fused(vh) partials
+// fused theta + F; workspace holds 2 * reduce_blocks_fused(vh) partials.
+// fix (may be null): driver-loop bookkeeping done by the final kernel -- see FixCtl; the pass is
+// skipped when fix->stop is already set.
+struct FixCheck {
+  FixCtl* ctl;
+  double theta_target;
+  int sweeps_before;     // sweeps completed when this check runs
+};
 cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
-                                    double* out_theta, double* out_F, cudaStream_t st);
+                                    double* out_theta, double* out_F, cudaStream_t st,
+                                    const FixCheck* fix = nullptr);
 // Coulomb gauge: per-slice theta_t, F_t (N3 doubles each)
 cudaError_t launch_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
                                             double* out_theta_t, double* out_F_t, cudaStream_t st);

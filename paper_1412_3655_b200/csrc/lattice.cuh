@@ -31,6 +31,10 @@ struct Geom {
   int32_t n[4];      // N0..N3
   int32_t nh0;       // N0/2
   int32_t vh;        // V/2 sites per parity
+  int32_t pitch;     // vectors per [parity][mu][j] plane: vh, or vh + stride[3] for a time slab that
+                     // carries a ghost slice behind its last slice (slab.cu)
+  int32_t wrap3;     // x3 = 0: index offset of the neighbour x - t_hat.  Periodic lattice:
+                     // stride[3]*(N3-1) (its own last slice); time slab: stride[3]*N3 = the ghost slice
   int32_t stride[4]; // half-index strides: 1 (unused for mu=0), N0/2, N0/2*N1, N0/2*N1*N2
   FastDiv d_nh0, d_n1, d_n2;
   // Coulomb gauge only: device array of N3 bytes, a site of time-slice t is swept iff
@@ -47,6 +51,8 @@ inline Geom make_geom(const int32_t dims[4]) {
   g.stride[2] = g.nh0 * dims[1];
   g.stride[3] = g.nh0 * dims[1] * dims[2];
   g.vh = g.stride[3] * dims[3];
+  g.pitch = g.vh;
+  g.wrap3 = g.stride[3] * (dims[3] - 1);
   g.d_nh0.init((uint32_t)g.nh0);
   g.d_n1.init((uint32_t)dims[1]);
   g.d_n2.init((uint32_t)dims[2]);
@@ -84,8 +90,8 @@ __device__ __forceinline__ int down_index(const Geom& g, int h, const SiteCoord&
   // would make the compiler copy it to local memory
   const int x = (mu == 1) ? c.x1 : (mu == 2) ? c.x2 : c.x3;
   const int st = (mu == 1) ? g.stride[1] : (mu == 2) ? g.stride[2] : g.stride[3];
-  const int n = (mu == 1) ? g.n[1] : (mu == 2) ? g.n[2] : g.n[3];
-  return x > 0 ? h - st : h + st * (n - 1);
+  const int wrap = (mu == 1) ? g.stride[1] * (g.n[1] - 1) : (mu == 2) ? g.stride[2] * (g.n[2] - 1) : g.wrap3;
+  return x > 0 ? h - st : h + wrap;
 }
 
 // Half index (other parity) of x + mu_hat, periodic.
@@ -133,34 +139,34 @@ __device__ __forceinline__ void vec_get(const double2& v, double* r) { r[0] = v.
 __device__ __forceinline__ void vec_set(float4& v, const float* r) { v = make_float4(r[0], r[1], r[2], r[3]); }
 __device__ __forceinline__ void vec_set(double2& v, const double* r) { v = make_double2(r[0], r[1]); }
 
-// Pointer to vector j=0 of link (parity, mu, h); vector j is at +j*vh.
+// Pointer to vector j=0 of link (parity, mu, h); vector j is at +j*pitch.
 template <typename S>
 __device__ __forceinline__ typename S::Vec* link_base(typename S::Vec* links, const Geom& g,
                                                       int parity, int mu, int h) {
-  return links + ((size_t)((parity * 4 + mu) * S::NV)) * (size_t)g.vh + (size_t)h;
+  return links + ((size_t)((parity * 4 + mu) * S::NV)) * (size_t)g.pitch + (size_t)h;
 }
 template <typename S>
 __device__ __forceinline__ const typename S::Vec* link_base(const typename S::Vec* links, const Geom& g,
                                                             int parity, int mu, int h) {
-  return links + ((size_t)((parity * 4 + mu) * S::NV)) * (size_t)g.vh + (size_t)h;
+  return links + ((size_t)((parity * 4 + mu) * S::NV)) * (size_t)g.pitch + (size_t)h;
 }
 
 // Load the NP stored reals of a link into r[0..NP).
 template <typename S>
-__device__ __forceinline__ void load_params(const typename S::Vec* p, int vh, typename S::Real* r) {
+__device__ __forceinline__ void load_params(const typename S::Vec* p, int pitch, typename S::Real* r) {
 #pragma unroll
   for (int j = 0; j < S::NV; ++j) {
-    typename S::Vec v = p[(size_t)j * (size_t)vh];
+    typename S::Vec v = p[(size_t)j * (size_t)pitch];
     vec_get(v, r + j * S::VL);
   }
 }
 template <typename S>
-__device__ __forceinline__ void store_params(typename S::Vec* p, int vh, const typename S::Real* r) {
+__device__ __forceinline__ void store_params(typename S::Vec* p, int pitch, const typename S::Real* r) {
 #pragma unroll
   for (int j = 0; j < S::NV; ++j) {
     typename S::Vec v;
     vec_set(v, r + j * S::VL);
-    p[(size_t)j * (size_t)vh] = v;
+    p[(size_t)j * (size_t)pitch] = v;
   }
 }
 

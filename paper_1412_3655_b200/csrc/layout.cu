@@ -46,22 +46,22 @@ layout_tiled_kernel(typename S::Real* __restrict__ canonical, typename S::Vec* _
 #pragma unroll
       for (int i = 0; i < kLinkRegs; ++i) m[i] = i < NF ? c[i] : (Real)0;   // pad reals stay 0
       if (S::NC == 3) {
-        store_params<S>(lptr, g.vh, m);              // first NP reals = first NP/6 rows (L118)
+        store_params<S>(lptr, g.pitch, m);              // first NP reals = first NP/6 rows (L118)
       } else {
         // SU(2): [[a0+i a3, a2+i a1],[..]] -> (a0,a1,a2,a3)   (C-7)
         Real a[4] = {m[0], m[3], m[2], m[1]};
-        store_params<S>(lptr, g.vh, a);
+        store_params<S>(lptr, g.pitch, a);
       }
     } else {
       if (S::NC == 3) {
         Real m[kLinkRegs];
-        load_params<S>(lptr, g.vh, m);
+        load_params<S>(lptr, g.pitch, m);
         if (S::NP == 12) reconstruct_row2(m);
 #pragma unroll
         for (int i = 0; i < 18; ++i) c[i] = m[i];
       } else {
         Real a[4];
-        load_params<S>(lptr, g.vh, a);
+        load_params<S>(lptr, g.pitch, a);
         c[0] = a[0];  c[1] = a[3];     // a0 + i a3
         c[2] = a[2];  c[3] = a[1];     // a2 + i a1
         c[4] = -a[2]; c[5] = a[1];     // -a2 + i a1
@@ -116,9 +116,9 @@ reunitarize_kernel(typename S::Vec* __restrict__ links, const Geom g) {
   if (t >= 8ll * g.vh) return;
   const int pm = (int)(t / g.vh);
   const int h = (int)(t - (long long)pm * g.vh);
-  typename S::Vec* p = links + ((size_t)pm * S::NV) * (size_t)g.vh + (size_t)h;
+  typename S::Vec* p = links + ((size_t)pm * S::NV) * (size_t)g.pitch + (size_t)h;
   Real r[kLinkRegs];
-  load_params<S>(p, g.vh, r);
+  load_params<S>(p, g.pitch, r);
   if (S::NC == 2) {
     double a[4] = {(double)r[0], (double)r[1], (double)r[2], (double)r[3]};
     const double inv = 1.0 / sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2] + a[3] * a[3]);
@@ -155,7 +155,7 @@ reunitarize_kernel(typename S::Vec* __restrict__ links, const Geom g) {
 #pragma unroll
     for (int i = 0; i < S::NP; ++i) r[i] = (Real)m[i];
   }
-  store_params<S>(p, g.vh, r);
+  store_params<S>(p, g.pitch, r);
 }
 
 template <typename S>

@@ -1,6 +1,6 @@
-// or_sweep.cu -- half-sweep dispatch (launch_or_sweep and friends), the SU(2) kernel, and the first
-// generation of SU(3) kernels that keep all links in registers (variants 1-14, the measured
-// alternatives of DESIGN.md 6.1).  The production SU(3) kernel is in or_sweep_staged.cu.
+// or_sweep.cu -- half-sweep and full-sweep dispatch (launch_or_sweep, launch_or_full_sweeps and
+// friends) and the SU(2) kernel.  The production SU(3) kernel is in or_sweep_staged.cu, the fused
+// full-sweep kernel in or_sweep_fused.cu, the measured alternatives in or_sweep_measure.cu.
 // (SURVEY.md 8(a) rows a1-a6.)
 //
 // For every site x of one parity:
@@ -8,86 +8,12 @@
 //   G from K by the SU(2) closed form / the SU(3) subgroup loop with g^omega   (L50-54)
 //   U_mu(x) <- G U_mu(x),  U_mu(x-mu) <- U_mu(x-mu) G^dagger                   (L19-21, L48)
 // Sites of one parity are independent (L54), so there is no synchronisation inside a launch.
-//
-// Thread-to-site mapping (the paper's 1 / 4 / 8 threads per site, L62-72, L122) is the template
-// parameter TPS: each of the TPS cooperating lanes owns 8/TPS links, the partial K are summed by
-// xor-shuffles (the warp-level analogue of the paper's shared-memory exchange) and every lane
-// then holds the same K and computes the same G.  Which TPS each storage uses is chosen by
-// measurement (profiles/).
 #include "lattice.cuh"
 #include "su_math.cuh"
 #include "su2_power.cuh"
 #include "kernels.h"
 
 namespace culgt {
-
-template <typename T>
-__device__ __forceinline__ T shfl_xor_t(T v, int mask);
-template <>
-__device__ __forceinline__ float shfl_xor_t<float>(float v, int mask) { return __shfl_xor_sync(0xffffffffu, v, mask); }
-template <>
-__device__ __forceinline__ double shfl_xor_t<double>(double v, int mask) { return __shfl_xor_sync(0xffffffffu, v, mask); }
-
-// ---------------------------------------------------------------------------------------------
-// SU(3).  S = storage traits, Acc = type of K and of the subgroup solve, TPS threads per site.
-// ---------------------------------------------------------------------------------------------
-template <typename S, typename Acc, int TPS, int BLOCK>
-__global__ void __launch_bounds__(BLOCK)
-or_sweep_su3_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity, const Acc omega) {
-  typedef typename S::Real Real;
-  constexpr int LPT = 8 / TPS;   // links per thread
-  const int tid = blockIdx.x * BLOCK + threadIdx.x;
-  int h = tid / TPS;
-  const int q = tid % TPS;
-  const bool active = h < g.vh;
-  if (!active) h = g.vh - 1;     // keep the lane alive for the shuffles; it stores nothing
-  const SiteCoord sc = decode_site(g, h, parity);
-
-  Real U[LPT][kLinkRegs];
-  typename S::Vec* ptr[LPT];
-#pragma unroll
-  for (int l = 0; l < LPT; ++l) {
-    const int slot = q * LPT + l;          // slot = 2*mu + (0: U_mu(x), 1: U_mu(x-mu))
-    const int mu = slot >> 1;
-    const bool dn = slot & 1;
-    const int idx = dn ? down_index(g, h, sc, mu) : h;
-    ptr[l] = link_base<S>(links, g, dn ? 1 - parity : parity, mu, idx);
-  }
-#pragma unroll
-  for (int l = 0; l < LPT; ++l) load_params<S>(ptr[l], g.vh, U[l]);
-  if (S::NP == 12) {
-#pragma unroll
-    for (int l = 0; l < LPT; ++l) reconstruct_row2(U[l]);
-  }
-
-  Acc K[18];
-#pragma unroll
-  for (int i = 0; i < 18; ++i) K[i] = 0;
-#pragma unroll
-  for (int l = 0; l < LPT; ++l) accumulate(K, U[l], ((q * LPT + l) & 1) != 0);
-#pragma unroll
-  for (int m = 1; m < TPS; m <<= 1) {
-#pragma unroll
-    for (int i = 0; i < 18; ++i) K[i] += shfl_xor_t<Acc>(K[i], m);
-  }
-
-  Acc Ga[18];
-  su3_site_G(K, Ga, omega);
-  Real G[18];
-#pragma unroll
-  for (int i = 0; i < 18; ++i) G[i] = (Real)Ga[i];
-
-  if (!active) return;
-  constexpr int NR = (S::NP == 12) ? 2 : 3;   // rows that are stored
-#pragma unroll
-  for (int l = 0; l < LPT; ++l) {
-    Real R[kLinkRegs];
-    R[18] = 0; R[19] = 0;
-    if (((q * LPT + l) & 1) == 0) mul_ab<NR>(G, U[l], R);
-    else mul_abd<NR>(U[l], G, R);
-    store_params<S>(ptr[l], g.vh, R);
-  }
-}
 
 // ---------------------------------------------------------------------------------------------
 // SU(2), 4-parameter storage, one thread per site.  8 links = 32 (fp32) / 64 (fp64) registers, so
@@ -99,13 +25,12 @@ or_sweep_su3_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
 template <typename S, int BLOCK, bool COULOMB, typename Power>
 __global__ void __launch_bounds__(BLOCK)
 or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int parity,
-                    const Power omega, const int reverse) {
+                    const Power omega, const int reverse, const int* __restrict__ stop_flag) {
   typedef typename S::Real Real;
   const int blk = reverse ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x;
   const int h = blk * BLOCK + threadIdx.x;
   if (h >= g.vh) return;
   const SiteCoord sc = decode_site(g, h, parity);
-  if (COULOMB && g.slice_active != nullptr && g.slice_active[sc.x3] == 0) return;   // frozen slice
   Real U[8][4];
   typename S::Vec* ptr[8];
 #pragma unroll
@@ -114,8 +39,10 @@ or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
     ptr[2 * mu + 1] = link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu));
   }
   pdl_prologue_done();    // lattice.cuh: the next half-sweep may be scheduled; the previous one is complete
+  if (stop_flag != nullptr && *stop_flag != 0) return;                               // driver loop has stopped
+  if (COULOMB && g.slice_active != nullptr && g.slice_active[sc.x3] == 0) return;   // frozen slice
 #pragma unroll
-  for (int l = 0; l < 8; ++l) load_params<S>(ptr[l], g.vh, U[l]);
+  for (int l = 0; l < 8; ++l) load_params<S>(ptr[l], g.pitch, U[l]);
   // K = k0 + i k.sigma = sum_mu u_up + conj(u_dn)
   double k[4] = {0, 0, 0, 0};
 #pragma unroll
@@ -135,32 +62,30 @@ or_sweep_su2_kernel(typename S::Vec* __restrict__ links, const Geom g, const int
     Real R[4];
     if ((l & 1) == 0) quat_mul(G, U[l], R);
     else quat_mul_dag(U[l], G, R);
-    store_params<S>(ptr[l], g.vh, R);
+    store_params<S>(ptr[l], g.pitch, R);
   }
 }
 
 // ---------------------------------------------------------------------------------------------
 // host-side launchers
 // ---------------------------------------------------------------------------------------------
-template <typename S, typename Acc, int TPS>
-static cudaError_t launch_su3(void* links, const Geom& g, int parity, double omega, cudaStream_t st) {
-  constexpr int BLOCK = 128;
-  const long long threads = (long long)g.vh * TPS;
-  const unsigned grid = (unsigned)((threads + BLOCK - 1) / BLOCK);
-  or_sweep_su3_kernel<S, Acc, TPS, BLOCK><<<grid, BLOCK, 0, st>>>(
-      (typename S::Vec*)links, g, parity, (Acc)omega);
-  return cudaGetLastError();
-}
-
 template <typename S, typename Power>
-static cudaError_t launch_su2(void* links, const Geom& g, int parity, Power omega, bool coulomb, cudaStream_t st) {
+static cudaError_t launch_su2(void* links, const Geom& g, int parity, Power omega, bool coulomb, const int* stop_flag,
+                              cudaStream_t st) {
   constexpr int BLOCK = 128;
   const unsigned grid = (unsigned)((g.vh + BLOCK - 1) / BLOCK);
   if (coulomb)
     return launch_pdl(or_sweep_su2_kernel<S, BLOCK, true, Power>, dim3(grid), dim3(BLOCK), 0, st,
-                      (typename S::Vec*)links, g, parity, omega, parity);
+                      (typename S::Vec*)links, g, parity, omega, parity, stop_flag);
   return launch_pdl(or_sweep_su2_kernel<S, BLOCK, false, Power>, dim3(grid), dim3(BLOCK), 0, st,
-                    (typename S::Vec*)links, g, parity, omega, parity);
+                    (typename S::Vec*)links, g, parity, omega, parity, stop_flag);
+}
+
+template <typename Power>
+static cudaError_t launch_su2_any(const LatticeDesc& d, void* links, int parity, const Power& pw, bool coulomb,
+                                  const int* stop_flag, cudaStream_t st) {
+  if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, d.geom, parity, pw, coulomb, stop_flag, st);
+  return launch_su2<Storage<double, 2, 4> >(links, d.geom, parity, pw, coulomb, stop_flag, st);
 }
 
 // Truncated-series overrelaxation (reading C-24): b_n = binom(omega, n) by the recurrence
@@ -172,10 +97,7 @@ cudaError_t launch_or_sweep_series(const LatticeDesc& d, void* links, int parity
   pw.order = order;
   pw.b[0] = 1.0;
   for (int n = 1; n <= kMaxSeriesOrder; ++n) pw.b[n] = n <= order ? pw.b[n - 1] * ((omega - (double)(n - 1)) / (double)n) : 0.0;
-  if (d.group == 2) {
-    if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, d.geom, parity, pw, false, st);
-    return launch_su2<Storage<double, 2, 4> >(links, d.geom, parity, pw, false, st);
-  }
+  if (d.group == 2) return launch_su2_any(d, links, parity, pw, false, nullptr, st);
   return launch_or_sweep_staged_series(d, links, parity, pw, st);
 }
 
@@ -187,82 +109,96 @@ cudaError_t launch_sa_sweep(const LatticeDesc& d, void* links, int parity, doubl
   pw.seed_lo = (uint32_t)seed;
   pw.seed_hi = (uint32_t)(seed >> 32);
   pw.counter = counter;
-  if (d.group == 2) {
-    if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, d.geom, parity, pw, false, st);
-    return launch_su2<Storage<double, 2, 4> >(links, d.geom, parity, pw, false, st);
-  }
+  if (d.group == 2) return launch_su2_any(d, links, parity, pw, false, nullptr, st);
   return launch_or_sweep_staged_heatbath(d, links, parity, pw, st);
 }
 
 // Microcanonical half-sweep (reading C-26); production mappings only.
 cudaError_t launch_micro_sweep(const LatticeDesc& d, void* links, int parity, cudaStream_t st) {
-  if (d.group == 2) {
-    if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, d.geom, parity, MicroPower{0}, false, st);
-    return launch_su2<Storage<double, 2, 4> >(links, d.geom, parity, MicroPower{0}, false, st);
-  }
+  if (d.group == 2) return launch_su2_any(d, links, parity, MicroPower{0}, false, nullptr, st);
   return launch_or_sweep_staged_micro(d, links, parity, st);
 }
 
-cudaError_t launch_or_full_sweep(const LatticeDesc& d, void* links, double omega, int variant, cudaStream_t st) {
-  if (variant >= 40 && variant < 60) {
-    const cudaError_t e = launch_or_sweep_staged_slabbed(d, links, omega, 1 << (variant % 10), variant >= 50, st);
-    if (e != cudaErrorNotSupported) return e;
-    variant = 0;                                         // lattice does not fit the slab schedule
+// Variant numbers (culgt_set_sweep_variant):
+//   product:  0 production (20 is its explicit name), 24 / 33 / 34 the same kernel without the reversed
+//             traversal / programmatic dependent launch / L2 hints, 60 the fused full sweep forced on,
+//             61 the fused full sweep forced off (two launches per sweep);
+//   -DCULGT_MEASURE only: 1-14, 21-32 (or_sweep_measure.cu), 41-44 launch-level slab schedules,
+//             >= 100000 fused-sweep parameter sweeps (100000 + 50000*alternate + 1000*lag + hints code).
+bool sweep_variant_known(int variant) {
+  switch (variant) {
+    case 0: case 20: case 24: case 33: case 34: case 60: case 61: return true;
+    default: break;
   }
-  for (int parity = 0; parity < 2; ++parity) {
-    const cudaError_t e = launch_or_sweep(d, links, parity, omega, variant, st);
-    if (e != cudaSuccess) return e;
-  }
-  return cudaSuccess;
+#ifdef CULGT_MEASURE
+  if ((variant >= 1 && variant <= 14) || (variant >= 21 && variant <= 32) || (variant >= 41 && variant <= 44) ||
+      (variant >= 100000 && variant < 200000))
+    return true;
+#endif
+  return false;
 }
 
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
-                            int variant, cudaStream_t st, bool coulomb) {
-  const Geom& g = d.geom;
-  if (variant >= 40 && variant < 60) variant = 0;       // slab schedules exist for full sweeps only
-  if (d.group == 2) {
-    if (d.precision == 32) return launch_su2<Storage<float, 2, 4> >(links, g, parity, omega, coulomb, st);
-    return launch_su2<Storage<double, 2, 4> >(links, g, parity, omega, coulomb, st);
+                            int variant, cudaStream_t st, bool coulomb, const int* stop_flag) {
+  if (d.group == 2) return launch_su2_any(d, links, parity, omega, coulomb, stop_flag, st);
+  // full-sweep schedules (fused, slab-blocked) have no half-sweep form: the production mapping
+  if (variant == 0 || variant >= 40) variant = 20;
+  if (variant == 20 || variant == 24 || variant == 33 || variant == 34)
+    return launch_or_sweep_staged(d, links, parity, omega, variant, coulomb, stop_flag, st);
+#ifdef CULGT_MEASURE
+  if (!coulomb && stop_flag == nullptr) return launch_or_sweep_measure(d, links, parity, omega, variant, st);
+#endif
+  return cudaErrorInvalidValue;
+}
+
+// Whether variant 0 takes the fused schedule: where one launch per full sweep wins by measurement
+// (DESIGN.md 6.1): SU(3) fields between 0.87 and 2.5 L2 sizes (32^4 fp32-12: 201 MB on a 126 MB L2).
+static bool fused_by_default(const LatticeDesc& d) {
+  if (d.group != 3) return false;
+  const double link_bytes = (d.precision == 32 && d.params == 18) ? 80.0 : (double)d.params * (d.precision / 8);
+  const double field = 4.0 * (double)d.V * link_bytes;
+  const double l2 = device_l2_bytes();
+  return field > 0.87 * l2 && field < 2.5 * l2;
+}
+
+cudaError_t launch_or_full_sweeps(const LatticeDesc& d, void* links, double* workspace, int n_sweeps, double omega,
+                                  int variant, const int* stop_flag, cudaStream_t st) {
+  if (n_sweeps <= 0) return cudaSuccess;
+  bool fused = workspace != nullptr && (variant == 60 || (variant == 0 && fused_by_default(d)));
+  int lag = 0, hints = kFusedDefaultHints;
+  bool alternate = true;
+#ifdef CULGT_MEASURE
+  if (variant >= 100000 && workspace != nullptr) {
+    const int v = variant - 100000;
+    fused = true;
+    alternate = v >= 50000;
+    lag = (v % 50000) / 1000;
+    int code = v % 1000, h = 0;              // base-3 digits: black load, black store, white load, white store
+    for (int i = 0; i < 4; ++i) { h |= (code % 3) << (2 * i); code /= 3; }
+    hints = h;
   }
-  // variant 0 = the production mapping (or_sweep_staged.cu); 20+ select staged mappings
-  if (variant == 0) {
-    const int best = 20;   // the production mapping of each storage format (or_sweep_staged.cu)
-    return launch_or_sweep_staged(d, links, parity, omega, best, coulomb, st);
-  }
-  if (coulomb) return cudaErrorInvalidValue;   // Coulomb gauge: production mapping (variant 0) only
-  if (variant >= 20) return launch_or_sweep_staged(d, links, parity, omega, variant, false, st);
-  if (d.precision == 32) {
-    // fp32 storage: K and the subgroup solve in fp64 (reading C-15); variants 10+ are
-    // all-fp32 arithmetic, kept for the precision/throughput comparison in profiles/.
-    if (d.params == 12) {
-      switch (variant) {
-        case 1: return launch_su3<Storage<float, 3, 12>, double, 1>(links, g, parity, omega, st);
-        case 2: return launch_su3<Storage<float, 3, 12>, double, 2>(links, g, parity, omega, st);
-        case 4: return launch_su3<Storage<float, 3, 12>, double, 4>(links, g, parity, omega, st);
-        case 11: return launch_su3<Storage<float, 3, 12>, float, 1>(links, g, parity, omega, st);
-        case 14: return launch_su3<Storage<float, 3, 12>, float, 4>(links, g, parity, omega, st);
-        default: return cudaErrorInvalidValue;
-      }
+  if (variant >= 41 && variant <= 44) {
+    bool fits = true;                          // cudaErrorNotSupported depends on the lattice only: first call
+    for (int i = 0; i < n_sweeps && fits; ++i) {
+      const cudaError_t e = launch_or_sweep_measure_slabbed(d, links, omega, 1 << (variant - 40), st);
+      if (e == cudaErrorNotSupported) fits = false;
+      else if (e != cudaSuccess) return e;
     }
-    switch (variant) {
-      case 2: return launch_su3<Storage<float, 3, 18>, double, 2>(links, g, parity, omega, st);
-      case 4: return launch_su3<Storage<float, 3, 18>, double, 4>(links, g, parity, omega, st);
-      default: return cudaErrorInvalidValue;
+    if (fits) return cudaSuccess;
+  }
+#endif
+  if (fused) {
+    void* ctl = workspace + fused_ctl_offset_doubles(d.geom);
+    const cudaError_t e = launch_or_sweeps_fused(d, links, omega, ctl, n_sweeps, lag, hints, alternate, stop_flag, st);
+    if (e != cudaErrorNotSupported) return e;     // lattice does not fit the fused schedule: two launches
+  }
+  const int half_variant = (variant >= 40) ? 0 : variant;
+  for (int i = 0; i < n_sweeps; ++i)
+    for (int parity = 0; parity < 2; ++parity) {
+      const cudaError_t e = launch_or_sweep(d, links, parity, omega, half_variant, st, false, stop_flag);
+      if (e != cudaSuccess) return e;
     }
-  }
-  if (d.params == 12) {
-    switch (variant) {
-      case 4: return launch_su3<Storage<double, 3, 12>, double, 4>(links, g, parity, omega, st);
-      case 2: return launch_su3<Storage<double, 3, 12>, double, 2>(links, g, parity, omega, st);
-      case 8: return launch_su3<Storage<double, 3, 12>, double, 8>(links, g, parity, omega, st);
-      default: return cudaErrorInvalidValue;
-    }
-  }
-  switch (variant) {
-    case 4: return launch_su3<Storage<double, 3, 18>, double, 4>(links, g, parity, omega, st);
-    case 8: return launch_su3<Storage<double, 3, 18>, double, 8>(links, g, parity, omega, st);
-    default: return cudaErrorInvalidValue;
-  }
+  return cudaSuccess;
 }
 
 }  // namespace culgt

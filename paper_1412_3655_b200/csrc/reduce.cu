@@ -77,8 +77,10 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 template <typename S, int BLOCK, bool COULOMB, bool STAGED>
 __global__ void __launch_bounds__(BLOCK, STAGED ? 512 / BLOCK : 0)
 theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
-                        double* __restrict__ partial_theta, double* __restrict__ partial_F) {
+                        double* __restrict__ partial_theta, double* __restrict__ partial_F,
+                        const int* __restrict__ stop_flag) {
   typedef typename S::Real Real;
+  if (stop_flag != nullptr && *stop_flag != 0) return;   // driver loop: this check is no longer wanted
   constexpr int HALF = BLOCK / 2;
   constexpr int ND = COULOMB ? 3 : 4;
   const int parity = threadIdx.x >= HALF;
@@ -102,8 +104,8 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
           const Vec* dn = link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu));
 #pragma unroll
           for (int j = 0; j < S::NV; ++j) {
-            cp_async16(sm + ((2 * mu) * S::NV + j) * BLOCK, up + (size_t)j * (size_t)g.vh);
-            cp_async16(sm + ((2 * mu + 1) * S::NV + j) * BLOCK, dn + (size_t)j * (size_t)g.vh);
+            cp_async16(sm + ((2 * mu) * S::NV + j) * BLOCK, up + (size_t)j * (size_t)g.pitch);
+            cp_async16(sm + ((2 * mu + 1) * S::NV + j) * BLOCK, dn + (size_t)j * (size_t)g.pitch);
           }
           asm volatile("cp.async.commit_group;" ::: "memory");   // one group per direction
         }
@@ -135,8 +137,8 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
 #pragma unroll
         for (int b = 0; b < MU_BATCH; ++b)
           if (mu0 + b < ND) {
-            load_params<S>(link_base<S>(links, g, parity, mu0 + b, h), g.vh, U[2 * b]);
-            load_params<S>(link_base<S>(links, g, 1 - parity, mu0 + b, down_index(g, h, sc, mu0 + b)), g.vh,
+            load_params<S>(link_base<S>(links, g, parity, mu0 + b, h), g.pitch, U[2 * b]);
+            load_params<S>(link_base<S>(links, g, 1 - parity, mu0 + b, down_index(g, h, sc, mu0 + b)), g.pitch,
                            U[2 * b + 1]);
           }
 #pragma unroll
@@ -161,8 +163,8 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
 #pragma unroll
       for (int mu = 0; mu < ND; ++mu) {
         Real u[4], w[4];
-        load_params<S>(link_base<S>(links, g, parity, mu, h), g.vh, u);
-        load_params<S>(link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu)), g.vh, w);
+        load_params<S>(link_base<S>(links, g, parity, mu, h), g.pitch, u);
+        load_params<S>(link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu)), g.pitch, w);
         f += 2.0 * (double)u[0];
 #pragma unroll
         for (int i = 0; i < 3; ++i) d[i] += (double)u[i + 1] - (double)w[i + 1];
@@ -180,8 +182,8 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
   }
 }
 
-// Final pass: block (group, quantity) sums the n partials of that group in a fixed order and
-// scales.  partial = [quantity][group][n]; quantity 0 = theta, 1 = F; group = time-slice for the
+// Final pass of the per-slice (Coulomb) sums: block (group, quantity) sums the n partials of that group
+// in a fixed order and scales.  partial = [quantity][group][n]; quantity 0 = theta, 1 = F; group = time-slice for the
 // Coulomb sums, a single group for the Landau sums.
 template <int BLOCK>
 __global__ void __launch_bounds__(BLOCK)
@@ -197,18 +199,56 @@ final_sum_kernel(const double* __restrict__ partial, int n, double scale0, doubl
   }
 }
 
+// Landau gauge: ONE block sums the theta partials, then the F partials, each in a fixed order, scales,
+// writes both scalars and -- when a driver loop is attached (FixCtl, kernels.h) -- does the loop's
+// bookkeeping on the device: records theta and F, and raises `stop` once theta < theta_target, after
+// which every sweep and check enqueued behind this one returns at entry ("iterated until the
+// discrete gauge condition (1) is satisfied up to a given numerical precision").  A NaN theta never
+// satisfies the test, so a non-finite field runs to max_sweeps.
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK)
+final_sum_landau_kernel(const double* __restrict__ partial, int n, double scale_theta, double scale_F,
+                        double* __restrict__ out_theta, double* __restrict__ out_F, FixCtl* __restrict__ ctl,
+                        double theta_target, int sweeps_before) {
+  if (ctl != nullptr && ctl->stop != 0) return;
+  double acc = 0;
+  for (int i = threadIdx.x; i < n; i += BLOCK) acc += partial[i];
+  const double st = block_sum<BLOCK>(acc);
+  __syncthreads();
+  acc = 0;
+  for (int i = threadIdx.x; i < n; i += BLOCK) acc += partial[(size_t)n + i];
+  const double sf = block_sum<BLOCK>(acc);
+  if (threadIdx.x == 0) {
+    const double theta = st * scale_theta, F = sf * scale_F;
+    *out_theta = theta;
+    *out_F = F;
+    if (ctl != nullptr) {
+      ctl->theta = theta;
+      ctl->F = F;
+      ctl->checks_done += 1;
+      if (theta < theta_target) {
+        ctl->sweeps_at_stop = sweeps_before;
+        ctl->stop = 1;
+      }
+    }
+  }
+}
+
 template <typename S, int BLOCK, bool COULOMB>
 static cudaError_t launch_theta_staged(dim3 grid, const void* links, const Geom& g, double* p_theta, double* p_F,
-                                       cudaStream_t st) {
+                                       const int* stop_flag, cudaStream_t st) {
   auto kern = theta_functional_kernel<S, BLOCK, COULOMB, true>;
   constexpr size_t smem = (size_t)8 * S::NV * BLOCK * sizeof(typename S::Vec);
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  static bool configured[kMaxDevices] = {false};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices || !configured[dev]) {
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = true;
+    if (dev >= 0 && dev < kMaxDevices) configured[dev] = true;
   }
-  kern<<<grid, BLOCK, smem, st>>>((const typename S::Vec*)links, g, p_theta, p_F);
+  kern<<<grid, BLOCK, smem, st>>>((const typename S::Vec*)links, g, p_theta, p_F, stop_flag);
   return cudaGetLastError();
 }
 
@@ -223,27 +263,30 @@ static constexpr bool theta_is_staged() { return S::NC == 3 && S::NP == 12 && si
 // the partials of quantity 1 start at p_theta + ny * blocks
 template <typename S, bool COULOMB>
 static cudaError_t launch_theta_pass(int group_size, int ny, const void* links, const Geom& g, double* p_theta,
-                                     cudaStream_t st, int* blocks_out) {
+                                     const int* stop_flag, cudaStream_t st, int* blocks_out) {
   const int nb = reduce_blocks_fused(group_size, theta_is_staged<S>() ? 64 : 128);
   *blocks_out = nb;
   double* p_F = p_theta + (size_t)ny * nb;
   const dim3 grid(nb, ny);
   if constexpr (theta_is_staged<S>()) {
-    return launch_theta_staged<S, 128, COULOMB>(grid, links, g, p_theta, p_F, st);
+    return launch_theta_staged<S, 128, COULOMB>(grid, links, g, p_theta, p_F, stop_flag, st);
   } else {
-    theta_functional_kernel<S, 256, COULOMB, false><<<grid, 256, 0, st>>>((const typename S::Vec*)links, g, p_theta, p_F);
+    theta_functional_kernel<S, 256, COULOMB, false><<<grid, 256, 0, st>>>((const typename S::Vec*)links, g, p_theta, p_F,
+                                                                          stop_flag);
     return cudaGetLastError();
   }
 }
 
 template <typename S>
 static cudaError_t run_theta_functional(const LatticeDesc& d, const void* links, double* ws, double* out_theta,
-                                        double* out_F, cudaStream_t st) {
+                                        double* out_F, cudaStream_t st, const FixCheck* fix) {
   int nblk = 0;
-  cudaError_t e = launch_theta_pass<S, false>(d.geom.vh, 1, links, d.geom, ws, st, &nblk);
+  FixCtl* ctl = fix ? fix->ctl : nullptr;
+  cudaError_t e = launch_theta_pass<S, false>(d.geom.vh, 1, links, d.geom, ws, ctl ? &ctl->stop : nullptr, st, &nblk);
   if (e != cudaSuccess) return e;
-  final_sum_kernel<kReduceBlock><<<dim3(1, 2), kReduceBlock, 0, st>>>(
-      ws, nblk, 1.0 / ((double)S::NC * (double)d.V), 1.0 / (4.0 * S::NC * (double)d.V), out_theta, out_F);
+  final_sum_landau_kernel<kReduceBlock><<<1, kReduceBlock, 0, st>>>(
+      ws, nblk, 1.0 / ((double)S::NC * (double)d.V), 1.0 / (4.0 * S::NC * (double)d.V), out_theta, out_F, ctl,
+      fix ? fix->theta_target : 0.0, fix ? fix->sweeps_before : 0);
   return cudaGetLastError();
 }
 
@@ -253,7 +296,7 @@ static cudaError_t run_coulomb_theta_functional(const LatticeDesc& d, const void
                                                 double* out_theta_t, double* out_F_t, cudaStream_t st) {
   const int n3 = d.geom.n[3];
   int nbx = 0;
-  cudaError_t e = launch_theta_pass<S, true>(d.geom.stride[3], n3, links, d.geom, ws, st, &nbx);
+  cudaError_t e = launch_theta_pass<S, true>(d.geom.stride[3], n3, links, d.geom, ws, nullptr, st, &nbx);
   if (e != cudaSuccess) return e;
   const double vs = (double)d.V / (double)n3;
   final_sum_kernel<kReduceBlock><<<dim3(n3, 2), kReduceBlock, 0, st>>>(
@@ -274,8 +317,8 @@ static cudaError_t run_coulomb_theta_functional(const LatticeDesc& d, const void
   return FN<Storage<double, 3, 18> >(__VA_ARGS__);
 
 cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
-                                    double* out_theta, double* out_F, cudaStream_t st) {
-  CULGT_DISPATCH(run_theta_functional, d, links, workspace, out_theta, out_F, st)
+                                    double* out_theta, double* out_F, cudaStream_t st, const FixCheck* fix) {
+  CULGT_DISPATCH(run_theta_functional, d, links, workspace, out_theta, out_F, st, fix)
 }
 
 cudaError_t launch_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* workspace,

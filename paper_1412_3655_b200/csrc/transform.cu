@@ -54,12 +54,12 @@ gauge_transform_kernel(typename S::Vec* __restrict__ links, const typename S::Re
       R[18] = 0; R[19] = 0;
       load_g3(gf, su, gu);
       typename S::Vec* p = link_base<S>(links, g, parity, mu, h);
-      load_params<S>(p, g.vh, U);
+      load_params<S>(p, g.pitch, U);
       if (S::NP == 12) reconstruct_row2(U);
       mul_ab<3>(gx, U, T);
       constexpr int NR = (S::NP == 12) ? 2 : 3;
       mul_abd<NR>(T, gu, R);
-      store_params<S>(p, g.vh, R);
+      store_params<S>(p, g.pitch, R);
     }
   } else {
     // SU(2): canonical 2x2 -> quaternion (a0,a1,a2,a3) = (Re g00, Im g01, Re g01, Im g00)
@@ -71,10 +71,10 @@ gauge_transform_kernel(typename S::Vec* __restrict__ links, const typename S::Re
       Real gu[4] = {gf[su * 8 + 0], gf[su * 8 + 3], gf[su * 8 + 2], gf[su * 8 + 1]};
       Real U[4], T[4], R[4];
       typename S::Vec* p = link_base<S>(links, g, parity, mu, h);
-      load_params<S>(p, g.vh, U);
+      load_params<S>(p, g.pitch, U);
       quat_mul(gx, U, T);
       quat_mul_dag(T, gu, R);
-      store_params<S>(p, g.vh, R);
+      store_params<S>(p, g.pitch, R);
     }
   }
 }

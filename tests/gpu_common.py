@@ -59,6 +59,10 @@ class GpuField:
     def sweep(self, omega, n=1):
         culgt.culgt_or_sweeps(self.lat, self.links, n, omega)
 
+    def sweep_ws(self, omega, n=1):
+        """full sweeps through the workspace entry point (fused one-kernel schedule where it applies)"""
+        culgt.culgt_or_sweeps_ws(self.lat, self.links, self.ws, n, omega)
+
     def theta(self):
         culgt.culgt_gauge_precision(self.lat, self.links, self.ws, self.scal[0:1])
         return float(self.scal[0].item())

@@ -46,8 +46,15 @@ def test_sizes():
     # the fused theta+F pass keeps two partials per 64 sites of a parity (the staged fp32 12-parameter
     # kernel; the other formats use every other slot's worth, 128 sites per partial), plus the 2 scalars
     # + 2 * N3 result slots (theta_t, F_t of the Coulomb driver; the Landau scalars use two) + N3 mask bytes
-    assert culgt.culgt_workspace_bytes(culgt.Lattice((64,) * 4, 3, 64, 18)) == (2 * (64 ** 4 // 2 // 64) + 2 * 64 + 8) * 8
-    assert culgt.culgt_workspace_bytes(culgt.Lattice((4,) * 4, 3, 64, 18)) == (4096 + 2 * 4 + 1) * 8
+    # ... rounded up to 16 doubles, + the driver loop's control block (16 doubles) + the fused sweep's
+    # (32 words of counters, 2 x 512 slice counters, 2 x 1024 slice-task words)
+    ctl = 16 * 8 + (32 + 2 * 512 + 2 * 1024) * 4
+
+    def ws_bytes(partials, n3):
+        red = partials + 2 * n3 + (n3 + 7) // 8
+        return (red + 15) // 16 * 16 * 8 + ctl
+    assert culgt.culgt_workspace_bytes(culgt.Lattice((64,) * 4, 3, 64, 18)) == ws_bytes(2 * (64 ** 4 // 2 // 64), 64)
+    assert culgt.culgt_workspace_bytes(culgt.Lattice((4,) * 4, 3, 64, 18)) == ws_bytes(4096, 4)
 
 
 @pytest.mark.parametrize("lat,code", [
@@ -89,6 +96,9 @@ def test_argument_errors_by_return_code():
     assert lib.culgt_landau_fix(ref, ok_ptr, ok_ptr, 1.7, 1e-10, 10, 0, None, None, None, None) == E["CULGT_ERR_ARG"]
     assert lib.culgt_fix_host(ref, None, ok_ptr, ok_ptr, ok_ptr, 1, 1.7, None, None, None) == E["CULGT_ERR_NULL"]
     assert lib.culgt_set_sweep_variant(-3) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_or_sweeps_ws(ref, ok_ptr, None, 1, 1.7, None) == E["CULGT_ERR_NULL"]
+    assert lib.culgt_or_sweeps_ws(ref, ok_ptr, ok_ptr, -1, 1.7, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_or_sweeps_ws(ref, ok_ptr, ok_ptr, 1, 2.0, None) == E["CULGT_ERR_OMEGA"]
     # the widened entry points (Coulomb gauge, series power, annealing, re-unitarisation, autotuner)
     assert lib.culgt_or_sweep_coulomb(ref, None, 0, 1.7, None) == E["CULGT_ERR_NULL"]
     assert lib.culgt_or_sweep_coulomb(ref, ok_ptr, 3, 1.7, None) == E["CULGT_ERR_PARITY"]
@@ -105,11 +115,64 @@ def test_argument_errors_by_return_code():
     assert lib.culgt_micro_sweeps(ref, None, 1, None) == E["CULGT_ERR_NULL"]
     assert lib.culgt_sa_anneal_micro(ref, ok_ptr, 1.0, 0.1, 5, -1, 1, None) == E["CULGT_ERR_ARG"]
     assert lib.culgt_reunitarize(ref, None, None) == E["CULGT_ERR_NULL"]
-    assert lib.culgt_autotune_sweep(ref, ok_ptr, 1.7, 0, None, None, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_autotune_sweep(ref, ok_ptr, ok_ptr, 1.7, 0, None, None, None) == E["CULGT_ERR_ARG"]
+    assert lib.culgt_autotune_sweep(ref, ok_ptr, None, 1.7, 1, None, None, None) == E["CULGT_ERR_NULL"]
     assert lib.culgt_gauge_precision_functional(ref, ok_ptr, ok_ptr, ok_ptr, None, None) == E["CULGT_ERR_NULL"]
     for code in E.values():
         assert culgt.culgt_strerror(code) != "unknown status"
     assert culgt.culgt_strerror(-99) == "unknown status"
+
+
+def test_product_build_rejects_measurement_variants():
+    """The product library accepts only schedules that compute the method, bit-identically: the
+    all-fp32 kernels (11, 14, 25), the G = 1 / no-solve measurement kernels (28, 32) and the rejected
+    mappings exist only in a -DCULGT_MEASURE build (include/culgt_b200.h, culgt_set_sweep_variant)."""
+    lib = culgt.lib()
+    E = culgt.ERRORS
+    assert culgt.culgt_measure_build() is False, "the committed build step must produce the product library"
+    for v in (0, 20, 24, 33, 34, 60, 61):
+        assert lib.culgt_set_sweep_variant(v) == culgt.CULGT_OK
+        assert culgt.culgt_get_sweep_variant() == v
+    lib.culgt_set_sweep_variant(0)
+    for v in (11, 14, 25, 28, 32, 1, 2, 4, 8, 21, 22, 23, 26, 27, 29, 30, 31, 41, 44, 51, 54, 99, 100, 100000, 150123):
+        assert lib.culgt_set_sweep_variant(v) == E["CULGT_ERR_ARG"], v
+        assert culgt.culgt_get_sweep_variant() == 0
+
+
+def test_sweep_variant_is_per_thread():
+    """The selection is a per-host-thread setting (no process-global mutable state)."""
+    import threading
+    lib = culgt.lib()
+    assert lib.culgt_set_sweep_variant(33) == culgt.CULGT_OK
+    seen = []
+    t = threading.Thread(target=lambda: seen.append(culgt.culgt_get_sweep_variant()))
+    t.start()
+    t.join()
+    assert seen == [0] and culgt.culgt_get_sweep_variant() == 33
+    lib.culgt_set_sweep_variant(0)
+
+
+def test_fused_schedule_order_and_dependencies():
+    """The slice-task order of the fused full sweep (csrc/or_sweep_fused.cu): every slice of both
+    parities exactly once, and every white slice t after the black slices t-1, t, t+1 (periodic) --
+    the property that makes the ticket scheme deadlock-free."""
+    import ctypes as C
+    lib = culgt.lib()
+    for n3 in (2, 4, 6, 8, 12, 32, 96, 512):
+        for lag in (0, 1, 2, 5, 40, 1000):
+            for direction in (0, 1):
+                buf = (C.c_uint * (2 * n3))()
+                lib.culgt_fused_schedule(n3, lag, direction, buf)
+                tasks = [(w >> 31, w & 0x7fffffff) for w in buf]
+                assert sorted(tasks) == sorted((p, t) for p in (0, 1) for t in range(n3))
+                pos = {task: i for i, task in enumerate(tasks)}
+                for t in range(n3):
+                    for nb in ((t - 1) % n3, t, (t + 1) % n3):
+                        assert pos[(0, nb)] < pos[(1, t)], (n3, lag, direction, t, nb)
+                if direction == 0:
+                    assert tasks[0] == (0, 0)
+                else:
+                    assert tasks[0] == (0, n3 - 1)
 
 
 def test_no_cpu_fallback():

@@ -42,6 +42,25 @@ def field_and_ref(name):
     return c, f, ref
 
 
+def require_host_memory(name, copies=6):
+    """The largest configurations must not be able to drop out of a green run: a host too small for
+    the full-size oracle field FAILS the test instead of skipping it."""
+    import psutil
+    c = li.CONFIGS[name]
+    need = copies * li.volume(c["dims"]) * 4 * 18 * 8      # fp64 canonical copies on the host
+    have = psutil.virtual_memory().available
+    if have < need:
+        pytest.fail(f"{name}: host has {have >> 30} GiB free, the full-size oracle comparison needs {need >> 30} GiB")
+
+
+def max_abs_diff(got, ref_real, step=1 << 20):
+    """max |got - ref| over all links, in slabs (no third full-size copy)."""
+    err = 0.0
+    for lo in range(0, got.shape[0], step):
+        err = max(err, float(np.abs(got[lo:lo + step] - li.from_real(ref_real[lo:lo + step])).max()))
+    return err
+
+
 def test_cfg0_su3_4x4_fp64_full_run():
     """configs[0]: omega = 1.7 until theta < 1e-20, theta every sweep; link parity after sweep 1,
     (F, theta) after every sweep, same stopping sweep (+-1)."""
@@ -149,11 +168,7 @@ def test_cfg4_large_volume_links_theta_F(name):
     offsets, asymmetric extents, plane sizes that are not powers of two) in the launch
     configuration bench.py times: theta and F of the input, ALL 4V links after the first sweep,
     theta and F after it -- the oracle needs ~2 s per sweep at this size, so one sweep."""
-    import psutil
-    c = li.CONFIGS[name]
-    need = 6 * li.volume(c["dims"]) * 4 * 18 * 8           # ~6 fp64 canonical copies on the host
-    if psutil.virtual_memory().available < need:
-        pytest.skip(f"host has less than {need >> 30} GiB free for the full-size oracle field")
+    require_host_memory(name)
     _INPUTS.clear()
     c, f, ref = field_and_ref(name)
     _INPUTS.clear()
@@ -166,12 +181,7 @@ def test_cfg4_large_volume_links_theta_F(name):
         assert abs(th - th_o) <= 1e-9 * th_o and abs(F - F_o) <= 1e-10
     oracle.full_sweep(dims, ref, om)
     f.sweep(om)
-    got = f.download()
-    err = 0.0
-    step = 1 << 20                                          # compare in slabs: no third full copy
-    for lo in range(0, got.shape[0], step):
-        err = max(err, float(np.abs(got[lo:lo + step] - li.from_real(ref[lo:lo + step])).max()))
-    del got
+    err = max_abs_diff(f.download(), ref)                   # in slabs: no third full copy
     assert err < TOL_LINK[prec], err
     th, F = f.theta_functional()
     th_o, F_o = oracle.gauge_precision(dims, ref), oracle.functional(dims, ref)
@@ -179,3 +189,111 @@ def test_cfg4_large_volume_links_theta_F(name):
         assert theta_close(th, th_o) and abs(F - F_o) <= 1e-10 * abs(F_o) + 1e-15
     else:
         assert abs(th - th_o) <= 1e-3 * th_o and abs(F - F_o) <= 2e-6
+
+
+@pytest.mark.parametrize("name", ["cfg3_fp32", "cfg3_fp64", "cfg4_fp32", "cfg4_fp64"])
+def test_gauge_transform_and_reunitarize_at_full_size(name):
+    """a9 culgt_gauge_transform and culgt_reunitarize (C-23) at the sizes DESIGN.md
+    quotes timings for -- 32^4 in both headline storages, 48^3 x 96 fp32-12, 64^4 fp64-18 (64-bit
+    byte offsets into g and the links, tens of thousands of CTAs): ALL 4V links against the oracle."""
+    require_host_memory(name, copies=5)
+    _INPUTS.clear()
+    c, f, ref = field_and_ref(name)
+    _INPUTS.clear()
+    dims, prec, params = c["dims"], c["precision"], c["params"]
+    g = li.haar_su3(li.volume(dims), c["seed"] + 500)
+    if prec == 32:
+        g = li.round_to_fp32(g)
+    oracle.gauge_transform(dims, ref, li.to_real(g))
+    f.transform(g)
+    del g
+    got = f.download()
+    err = max_abs_diff(got, ref)
+    assert err < (1e-13 if prec == 64 else 2e-6), err
+    # re-unitarisation of what the storage now holds (fp32: the products' rounding has moved the rows
+    # off SU(3) by ~1e-7; a deliberate 1e-3 drift is added on top, slab by slab, and re-uploaded)
+    rng = np.random.default_rng(c["seed"] + 501)
+    step = 1 << 20
+    for lo in range(0, got.shape[0], step):
+        blk = got[lo:lo + step]
+        blk += 1e-3 * (rng.standard_normal(blk.shape) + 1j * rng.standard_normal(blk.shape))
+    f.upload(got)
+    del got, ref
+    stored = f.download()                       # rounded to the storage precision, row 2 rebuilt for 12 parameters
+    ref2 = li.to_real(stored)
+    del stored
+    oracle.reunitarize(ref2)
+    culgt.culgt_reunitarize(f.lat, f.links)
+    got = f.download()
+    err = max_abs_diff(got, ref2)
+    assert err < (1e-14 if prec == 64 else 3e-7), err
+    for lo in range(0, got.shape[0], step):
+        blk = got[lo:lo + step]
+        assert np.abs(blk @ np.conj(np.swapaxes(blk, -1, -2)) - np.eye(3)).max() < (1e-14 if prec == 64 else 5e-7)
+
+
+@pytest.mark.parametrize("name", ["su2_32_fp64", "su2_32_fp32"])
+def test_su2_32x4_links_theta_F_transform(name):
+    """The SU(2) 4-parameter path at the headline volume 32^4 (the size DESIGN.md 6.2 quotes a timing
+    for; cfg1's 8^4 is a single wave): theta and F of the hot input, all 4V links after one sweep at
+    omega = 1.5, theta and F after it, the first sweeps of the trajectory, and the gauge transform."""
+    c, f, ref = field_and_ref(name)
+    _INPUTS.clear()
+    dims, om, prec = c["dims"], c["omega"], c["precision"]
+
+    def check_scalars(sweep):
+        th, F = f.theta_functional()
+        th_o, F_o = oracle.gauge_precision(dims, ref), oracle.functional(dims, ref)
+        if prec == 64:
+            assert theta_close(th, th_o), (sweep, th, th_o)
+            assert abs(F - F_o) <= 1e-10 * abs(F_o) + 1e-15, sweep
+        elif sweep == 0:        # identical stored values, fp64 reduction arithmetic
+            assert abs(th - th_o) <= 1e-9 * th_o and abs(F - F_o) <= 1e-10
+        else:
+            assert abs(th - th_o) <= 1e-3 * th_o and abs(F - F_o) <= 2e-6, sweep
+
+    check_scalars(0)
+    oracle.full_sweep(dims, ref, om)
+    f.sweep(om)
+    err = max_abs_diff(f.download(), ref)
+    assert err < TOL_LINK[prec], err
+    check_scalars(1)
+    for s in range(2, 6):
+        oracle.full_sweep(dims, ref, om)
+        f.sweep(om)
+        check_scalars(s)
+    # gauge transform of the stored field
+    stored = f.download()
+    ref = li.to_real(stored)
+    g = li.haar_su2(li.volume(dims), c["seed"] + 500)
+    if prec == 32:
+        g = li.round_to_fp32(g)
+    oracle.gauge_transform(dims, ref, li.to_real(g))
+    f.transform(g)
+    err = max_abs_diff(f.download(), ref)
+    assert err < (1e-13 if prec == 64 else 2e-6), err
+
+
+@pytest.mark.parametrize("name", ["cfg3_fp32", "cfg3_fp64", "cfg3_fp32_18", "cfg3_fp64_12"])
+def test_cfg3_fused_sweep_bit_identical_and_matches_oracle(name):
+    """The fused one-kernel full sweep (culgt_or_sweeps_ws, csrc/or_sweep_fused.cu) at the headline
+    volume, where its dependency counters and the lag between the black and the white front are really
+    exercised (thousands of tickets per resident CTA): all 4V links after sweep 1 against the oracle,
+    and bit-identical to the two-launch schedule after 6 sweeps (ascending and descending passes)."""
+    c, f, ref = field_and_ref(name)
+    dims, om, prec = c["dims"], c["omega"], c["precision"]
+    u = named_input(name)
+    oracle.full_sweep(dims, ref, om)
+    culgt.culgt_set_sweep_variant(60)
+    try:
+        f.sweep_ws(om, 1)
+        err = max_abs_diff(f.download(), ref)
+        assert err < TOL_LINK[prec], err
+        f.sweep_ws(om, 5)
+        fused = f.links.clone()
+    finally:
+        culgt.culgt_set_sweep_variant(0)
+    f.upload(u)
+    f.sweep(om, 6)
+    torch.cuda.synchronize()
+    assert torch.equal(fused, f.links)

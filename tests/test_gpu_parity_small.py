@@ -45,18 +45,25 @@ def test_pack_unpack_round_trip_su2(dims, precision):
     assert np.array_equal(f.download(), want)
 
 
+PRODUCT_VARIANTS = [0, 24, 33, 34]
+
+
 def variants_for(precision, params):
-    """0 = production mapping (= staged variant 20); 1..8 = direct register kernels with that
-    many threads per site; 20+ = shared-memory staged mappings (table in or_sweep_staged.cu):
-    flat / persistent grids, 1-2 stages, 1/2/4 threads per site, prefetch, chunked, stream stores,
-    33 = the production mapping without programmatic dependent launch, 34 = without L2 eviction hints."""
+    """Product build: 0 = the production mapping; 24 / 33 / 34 = the same kernel without the reversed
+    odd-parity traversal / programmatic dependent launch / L2 eviction hints.  A library built with
+    -DCULGT_MEASURE (culgt_measure_build()) also carries the measured alternatives of
+    csrc/or_sweep_measure.cu that compute the same update: 1..8 = direct register kernels with that
+    many threads per site; 21+ = staged mappings (flat / persistent grids, 1-2 stages, 1/2/4 threads
+    per site, prefetch, chunked, stream stores)."""
+    if not culgt.culgt_measure_build():
+        return list(PRODUCT_VARIANTS)
     if precision == 32 and params == 12:
-        return [0, 1, 2, 4, 21, 22, 23, 24, 26, 27, 29, 30, 31, 33, 34]
+        return PRODUCT_VARIANTS + [1, 2, 4, 21, 22, 23, 26, 27, 29, 30, 31]
     if precision == 32:
-        return [0, 2, 4, 21, 22, 23, 24]
+        return PRODUCT_VARIANTS + [2, 4, 21, 22, 23, 30]
     if params == 12:
-        return [0, 2, 4, 8, 21, 22, 23, 24]
-    return [0, 4, 8, 21, 22, 23, 24, 26, 27, 30, 31, 32, 33, 34]
+        return PRODUCT_VARIANTS + [2, 4, 8, 21, 22, 23, 30]
+    return PRODUCT_VARIANTS + [4, 8, 21, 22, 23, 26, 27, 30, 31, 32]
 
 
 @pytest.mark.parametrize("dims", DIMS)
@@ -188,46 +195,74 @@ def test_sweep_is_asynchronous():
 
 
 def test_autotuner_picks_a_result_equivalent_mapping():
-    """culgt_autotune_sweep (PAPER.md L89 (d), L134): returns one of the built mappings with a
+    """culgt_autotune_sweep (PAPER.md L89 (d), L134): returns one of the built schedules with a
     positive time, leaves it selected, and sweeps with it still match the oracle."""
     dims = (8, 8, 8, 8)
     u = make(dims, 3, 47)
     for precision, params in SU3_STORES:
         scratch = GpuField(dims, 3, precision, params, u)
         try:
-            v, us = culgt.culgt_autotune_sweep(scratch.lat, scratch.links, 1.7, 2)
-            assert v in variants_for(precision, params) + [20] and us > 0
+            v, us = culgt.culgt_autotune_sweep(scratch.lat, scratch.links, scratch.ws, 1.7, 2)
+            assert v in variants_for(precision, params) + [20, 60, 61] and us > 0
             assert culgt.culgt_get_sweep_variant() == v
             ref = storage_input(u, precision, params)
             oracle.full_sweep(dims, ref, 1.7)
             f = GpuField(dims, 3, precision, params, u)
-            f.sweep(1.7)
+            f.sweep_ws(1.7)
             assert np.abs(f.download() - li.from_real(ref)).max() < TOL_LINK[precision]
         finally:
             culgt.culgt_set_sweep_variant(0)
 
 
-@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (8, 8, 8, 12), (16, 8, 8, 6), (4, 6, 2, 8)])
+FUSED_DIMS = [(8, 8, 8, 8), (8, 8, 8, 12), (16, 8, 8, 6), (8, 8, 4, 2), (8, 8, 8, 4), (8, 4, 8, 16), (4, 6, 2, 8)]
+
+
+@pytest.mark.parametrize("dims", FUSED_DIMS)
 @pytest.mark.parametrize("precision,params", SU3_STORES)
-def test_slab_blocked_full_sweep_is_the_same_sweep(dims, precision, params):
-    """Variants 41-43 / 51-53 (black and white half-sweeps interleaved slab by slab
-    along t, on one or two streams) reorder launches only: three sweeps must agree with the oracle
-    and be bit-identical to the default schedule; (4,6,2,8) does not split into whole site blocks per
-    slice and takes the fallback."""
+def test_fused_full_sweep_is_the_same_sweep(dims, precision, params):
+    """culgt_or_sweeps_ws with variant 60 (csrc/or_sweep_fused.cu: black and white half-sweeps
+    interleaved slice by slice inside ONE persistent kernel, tickets + per-slice completion counters,
+    every other sweep descending) only reorders independent site updates: one sweep must agree with
+    the oracle, and three more must be bit-identical to the two-launch schedule (variant 61).  Covers
+    N3 = 2 (both black slices first), N3 = 4 (lag clamped), long time extents, and (4,6,2,8), which
+    does not hold whole site blocks per slice and takes the two-launch fallback.  With -DCULGT_MEASURE
+    also the launch-level slab schedules 41-43."""
     u = make(dims, 3, 46)
     ref = storage_input(u, precision, params)
     oracle.full_sweep(dims, ref, 1.7)
     outs = {}
-    for variant in (0, 41, 42, 43, 51, 52, 53):
+    for variant in [61, 60, 0] + ([41, 42, 43] if culgt.culgt_measure_build() else []):
         culgt.culgt_set_sweep_variant(variant)
         try:
             f = GpuField(dims, 3, precision, params, u)
-            f.sweep(1.7, 1)
+            f.sweep_ws(1.7, 1)
             assert np.abs(f.download() - li.from_real(ref)).max() < TOL_LINK[precision], variant
-            f.sweep(1.7, 2)
+            f.sweep_ws(1.7, 3)
+            f.sweep_ws(1.7, 2)          # a second call: the control block is set up again
             torch.cuda.synchronize()
             outs[variant] = f.download()
         finally:
             culgt.culgt_set_sweep_variant(0)
     for variant, out in outs.items():
-        assert np.array_equal(out, outs[0]), variant
+        assert np.array_equal(out, outs[61]), variant
+
+
+def test_fused_sweep_in_the_driver_loop_and_host_call():
+    """culgt_landau_fix and culgt_fix_host hand their workspace to the sweeps: with the fused schedule
+    forced on they must stop at the same sweep with the same theta and F, bit for bit."""
+    dims = (8, 8, 8, 8)
+    u = make(dims, 3, 49)
+    res = {}
+    for variant in (61, 60):
+        culgt.culgt_set_sweep_variant(variant)
+        try:
+            f = GpuField(dims, 3, 64, 18, u)
+            res[variant] = culgt.culgt_landau_fix(f.lat, f.links, f.ws, 1.7, 1e-12, 400, 3)
+            host = torch.from_numpy(li.to_real(u)).pin_memory()
+            can = torch.empty_like(host, device="cuda")
+            res[variant] += culgt.culgt_fix_host(f.lat, host, can, f.links, f.ws, 5, 1.7)
+            res[variant] += (host.numpy().tobytes(),)
+        finally:
+            culgt.culgt_set_sweep_variant(0)
+    assert res[60] == res[61]
+    assert res[60][1] < 1e-12 and res[60][0] % 3 == 0
