@@ -10,7 +10,7 @@
  *   - The library keeps NO state between calls except, per device, lazily-set kernel attributes and
  *     cached device properties, and, per HOST THREAD, the sweep-variant selection
  *     (culgt_set_sweep_variant) and the text of the last CUDA error.  Whatever a kernel must remember
- *     between launches (the driver loop's stop word, the fused sweep's ticket counters) lives in the
+ *     between launches (the driver loop's stop word) lives in the
  *     caller's `workspace` and is re-initialised by the call that uses it; a workspace must therefore
  *     not be shared by calls that run concurrently.  One process may drive several devices: every call
  *     acts on the CURRENT device (cudaSetDevice), to which its pointers and stream must belong.
@@ -74,7 +74,7 @@ size_t culgt_canonical_bytes(const culgt_lattice* lat);  /* V*4*Nc*Nc*2*sizeof(r
 size_t culgt_gfield_bytes(const culgt_lattice* lat);     /* V*Nc*Nc*2*sizeof(real)                  */
 size_t culgt_workspace_bytes(const culgt_lattice* lat);  /* reductions: block partials + result slots
                                                             (V/64 doubles), plus ~12 KB of control
-                                                            blocks (driver loop, fused sweep)        */
+                                                            blocks (driver loop)                     */
 
 /* Validate a descriptor: CULGT_OK, CULGT_ERR_NULL, CULGT_ERR_DIMS or CULGT_ERR_DESC. */
 int culgt_validate(const culgt_lattice* lat);
@@ -102,19 +102,8 @@ int culgt_reunitarize(const culgt_lattice* lat, void* links, void* stream);
  * link products in fp32; K accumulation and the subgroup solve in fp64 (C-15). */
 int culgt_or_sweep(const culgt_lattice* lat, void* links, int parity, double omega, void* stream);
 
-/* n_sweeps full sweeps (black then white half-sweep each; C-12), enqueued back to back as two
- * launches per sweep. */
+/* n_sweeps full sweeps (black then white half-sweep each; C-12), enqueued back to back. */
 int culgt_or_sweeps(const culgt_lattice* lat, void* links, int n_sweeps, double omega, void* stream);
-
-/* The same n_sweeps full sweeps, bit-identical links, given a workspace (>= culgt_workspace_bytes,
- * device pointer, used exclusively by this call while it runs): where the field is about one to two
- * L2 sizes (SU(3) 32^4 fp32-12 on B200) each sweep runs as ONE persistent kernel that interleaves
- * the black and the white half-sweep time-slice by time-slice, so that white sites find the links
- * their black neighbours have just written in the L2 and the field crosses HBM about once per sweep
- * instead of twice (sites of one parity are independent, so the order inside a parity is
- * free); elsewhere exactly culgt_or_sweeps.  Asynchronous on `stream`. */
-int culgt_or_sweeps_ws(const culgt_lattice* lat, void* links, void* workspace, int n_sweeps, double omega,
-                       void* stream);
 
 /* a8: theta = 1/(Nc V) sum_x tr[Delta(x) Delta(x)^dagger],  Delta = sum_mu A_mu(x) - A_mu(x-mu),
  * A_mu = [(U_mu - U_mu^dagger)/(2i)]_traceless with a*g = 1 (eq. (1); C-4, C-5).
@@ -217,25 +206,15 @@ int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, do
                       double theta_target, int max_sweeps, int check_every, int* sweeps_done,
                       double* theta_t_out, double* F_t_out, void* stream);
 
-/* Host-only query (no CUDA call): the order in which the fused full sweep of culgt_or_sweeps_ws hands
- * out its 2*n_slices slice-tasks, tasks_out[u] = parity << 31 | time-slice, for a lattice of n_slices
- * (even, 2..512) time-slices, a lag of `lag` slices between the black and the white front (clamped to
- * [1, n_slices-2]; <= 0: 1) and direction 0 (ascending) or 1 (descending).  Every white slice t comes
- * after the black slices t-1, t, t+1 (periodic), which is what makes the schedule deadlock-free.
- * tasks_out: HOST array of 2*n_slices words. */
-int culgt_fused_schedule(int n_slices, int lag, int direction, unsigned* tasks_out);
-
 /* Sweep-schedule selection of the CALLING HOST THREAD.  Every value the product
  * library accepts computes the same update, bit for bit:
  *    0  the default chosen by measurement (20 is its explicit name for the half-sweep kernel);
  *   24 / 33 / 34  the production kernel without the reversed odd-parity traversal / without
- *       programmatic dependent launch / without L2 eviction hints;
- *   60 / 61  the fused one-kernel full sweep of culgt_or_sweeps_ws forced on (where the lattice
- *       qualifies) / off.
+ *       programmatic dependent launch / without L2 eviction hints.
  * Anything else returns CULGT_ERR_ARG.  (A library built with -DCULGT_MEASURE -- python -m
  * paper_1412_3655_b200.build --measure; culgt_measure_build() == 1 -- additionally accepts the
- * measured alternatives of csrc/or_sweep_measure.cu, some of which deliberately do NOT compute the
- * method; they are never part of the product build.) */
+ * measured alternatives of csrc/or_sweep_measure.cu and csrc/or_sweep_fused.cu, some of which
+ * deliberately do NOT compute the method; they are never part of the product build.) */
 int culgt_set_sweep_variant(int variant);
 int culgt_get_sweep_variant(void);
 int culgt_measure_build(void);
@@ -243,7 +222,7 @@ int culgt_measure_build(void);
 /* Run-time autotuner (the paper's per-GPU selection of the fastest set-up, P:L89 (d)):
  * times every result-equivalent sweep schedule with `sweeps_per_trial` REAL full sweeps each on
  * `links` (the field is gauge-fixed further by them), makes the fastest the calling thread's
- * variant and reports it.  workspace as for culgt_or_sweeps_ws.  SYNCHRONISES.  best_variant,
+ * variant and reports it.  workspace: device pointer, >= culgt_workspace_bytes.  SYNCHRONISES.  best_variant,
  * best_us_per_half_sweep: host pointers, may be NULL. */
 int culgt_autotune_sweep(const culgt_lattice* lat, void* links, void* workspace, double omega,
                          int sweeps_per_trial, int* best_variant, float* best_us_per_half_sweep, void* stream);

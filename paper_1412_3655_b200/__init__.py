@@ -66,7 +66,8 @@ def lib() -> ctypes.CDLL:
     L.culgt_reunitarize.argtypes = [latp, vp, vp]
     L.culgt_or_sweep.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_or_sweeps.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
-    L.culgt_or_sweeps_ws.argtypes = [latp, vp, vp, ctypes.c_int, ctypes.c_double, vp]
+    if hasattr(L, "culgt_or_sweeps_ws"):       # measurement library only (csrc/measure_api.h)
+        L.culgt_or_sweeps_ws.argtypes = [latp, vp, vp, ctypes.c_int, ctypes.c_double, vp]
     L.culgt_gauge_precision.argtypes = [latp, vp, vp, vp, vp]
     L.culgt_functional.argtypes = [latp, vp, vp, vp, vp]
     L.culgt_gauge_precision_functional.argtypes = [latp, vp, vp, vp, vp, vp]
@@ -223,6 +224,7 @@ def culgt_or_sweeps(lat: Lattice, links, n_sweeps: int, omega: float, stream=Non
 
 
 def culgt_or_sweeps_ws(lat: Lattice, links, workspace, n_sweeps: int, omega: float, stream=None) -> None:
+    """Measurement library only (CULGT_MEASURE=1): full sweeps with a workspace, variant 60 = fused kernel."""
     _require_cuda()
     _check(lib().culgt_or_sweeps_ws(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace), int(n_sweeps),
                                     float(omega), _stream(stream)), "culgt_or_sweeps_ws")
@@ -393,7 +395,8 @@ def culgt_get_sweep_variant() -> int:
 
 
 def culgt_fused_schedule(n_slices: int, lag: int, direction: int):
-    """[(parity, slice), ...] in the order the fused full sweep hands out its slice-tasks (host only)."""
+    """Measurement library only: [(parity, slice), ...] in the order the fused full sweep hands out
+    its slice-tasks (host only)."""
     buf = (ctypes.c_uint * (2 * int(n_slices)))()
     _check(lib().culgt_fused_schedule(int(n_slices), int(lag), int(direction), buf), "culgt_fused_schedule")
     return [(w >> 31, w & 0x7FFFFFFF) for w in buf]

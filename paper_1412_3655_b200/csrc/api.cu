@@ -7,6 +7,7 @@
 #include <vector>
 #include "../../include/culgt_b200.h"
 #include "kernels.h"
+#include "measure_api.h"
 
 using namespace culgt;
 
@@ -138,20 +139,6 @@ int culgt_or_sweeps(const culgt_lattice* lat, void* links, int n_sweeps, double 
   if (n_sweeps < 0) return CULGT_ERR_ARG;
   if ((rc = check_omega(omega)) != CULGT_OK) return rc;
   cudaError_t e = launch_or_full_sweeps(d, links, nullptr, n_sweeps, omega, g_variant, nullptr, (cudaStream_t)stream);
-  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
-}
-
-int culgt_or_sweeps_ws(const culgt_lattice* lat, void* links, void* workspace, int n_sweeps, double omega,
-                       void* stream) {
-  LatticeDesc d;
-  int rc = describe(lat, &d);
-  if (rc != CULGT_OK) return rc;
-  if (!links || !workspace) return CULGT_ERR_NULL;
-  if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
-  if (n_sweeps < 0) return CULGT_ERR_ARG;
-  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
-  cudaError_t e = launch_or_full_sweeps(d, links, (double*)workspace, n_sweeps, omega, g_variant, nullptr,
-                                        (cudaStream_t)stream);
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
@@ -544,7 +531,7 @@ int culgt_autotune_sweep(const culgt_lattice* lat, void* links, void* workspace,
   int best = 0;
   float best_us = -1.f;
   for (int v = 1; v < 64; ++v) {
-    if (!sweep_variant_known(v)) continue;
+    if (!sweep_variant_known(v) || v == 20) continue;            // 20 is variant 0's other name: timed once, below
     // 11, 14, 25: all-fp32 arithmetic (different precision); 28, 32: measurement-only (no solve)
     if (v == 11 || v == 14 || v == 25 || v == 28 || v == 32) continue;
     if (d.group == 2 && v != 20) continue;
@@ -570,13 +557,6 @@ int culgt_autotune_sweep(const culgt_lattice* lat, void* links, void* workspace,
   return CULGT_OK;
 }
 
-int culgt_fused_schedule(int n_slices, int lag, int direction, unsigned* tasks_out) {
-  if (!tasks_out) return CULGT_ERR_NULL;
-  if (n_slices < 2 || (n_slices & 1) || n_slices > kFusedMaxSlices || (direction != 0 && direction != 1)) return CULGT_ERR_ARG;
-  fused_schedule(n_slices, lag, direction, tasks_out);
-  return CULGT_OK;
-}
-
 int culgt_set_sweep_variant(int variant) {
   if (!sweep_variant_known(variant)) return CULGT_ERR_ARG;
   g_variant = variant;
@@ -590,6 +570,31 @@ int culgt_measure_build(void) {
   return 0;
 #endif
 }
+
+#ifdef CULGT_MEASURE
+// ---- entry points of the measurement build only (csrc/measure_api.h) -----------------------------------
+int culgt_or_sweeps_ws(const culgt_lattice* lat, void* links, void* workspace, int n_sweeps, double omega,
+                       void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !workspace) return CULGT_ERR_NULL;
+  if (misaligned(links) || misaligned(workspace)) return CULGT_ERR_ALIGN;
+  if (n_sweeps < 0) return CULGT_ERR_ARG;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  cudaError_t e = launch_or_full_sweeps(d, links, (double*)workspace, n_sweeps, omega, g_variant, nullptr,
+                                        (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_fused_schedule(int n_slices, int lag, int direction, unsigned* tasks_out) {
+  if (!tasks_out) return CULGT_ERR_NULL;
+  if (n_slices < 2 || (n_slices & 1) || n_slices > kFusedMaxSlices || (direction != 0 && direction != 1)) return CULGT_ERR_ARG;
+  fused_schedule(n_slices, lag, direction, tasks_out);
+  return CULGT_OK;
+}
+
+#endif
 
 const char* culgt_strerror(int status) {
   switch (status) {

@@ -50,7 +50,8 @@ struct FixCtl {
   double theta, F;     // of the last check that ran
 };
 
-// Fused full sweep (or_sweep_fused.cu).
+// Fused full sweep (or_sweep_fused.cu; -DCULGT_MEASURE builds only -- the struct is declared
+// unconditionally so that both builds lay the workspace out the same way).
 constexpr int kFusedMaxSlices = 512;
 struct FusedCtl {
   unsigned ticket;                           // next ticket of the running launch
@@ -102,17 +103,17 @@ cudaError_t launch_or_sweep_staged_series(const LatticeDesc& d, void* links, int
                                           cudaStream_t st);
 
 // ---- full sweeps ------------------------------------------------------------------------------------
-// n_sweeps FULL sweeps (black then white).  `workspace` (may be null) is the caller's reduction
-// workspace: with it, and where the lattice qualifies, the sweeps run as the fused one-kernel
-// schedule of or_sweep_fused.cu; otherwise as two half-sweep launches each.
+// n_sweeps FULL sweeps (black then white), two half-sweep launches each.  `workspace` (may be null)
+// is the caller's reduction workspace; only the -DCULGT_MEASURE build uses it here (variant 60: the
+// fused one-kernel schedule of or_sweep_fused.cu).
 cudaError_t launch_or_full_sweeps(const LatticeDesc& d, void* links, double* workspace, int n_sweeps, double omega,
                                   int variant, const int* stop_flag, cudaStream_t st);
+#ifdef CULGT_MEASURE
 // the fused schedule itself: cudaErrorNotSupported when the lattice does not qualify.
 // lag <= 0: default; hints: L2 policy bits (or_sweep_fused.cu); alternate: every other sweep descending.
 cudaError_t launch_or_sweeps_fused(const LatticeDesc& d, void* links, double omega, void* ctl, int n_sweeps,
                                    int lag, int hints, bool alternate, const int* stop_flag, cudaStream_t st);
 void fused_schedule(int n3, int lag, int dir, unsigned* out);   // host: the slice-task order (2 * n3 entries)
-#ifdef CULGT_MEASURE
 cudaError_t launch_or_sweep_measure(const LatticeDesc& d, void* links, int parity, double omega, int variant,
                                     cudaStream_t st);
 cudaError_t launch_or_sweep_measure_slabbed(const LatticeDesc& d, void* links, double omega, int slab_slices,

@@ -121,18 +121,18 @@ cudaError_t launch_micro_sweep(const LatticeDesc& d, void* links, int parity, cu
 
 // Variant numbers (culgt_set_sweep_variant):
 //   product:  0 production (20 is its explicit name), 24 / 33 / 34 the same kernel without the reversed
-//             traversal / programmatic dependent launch / L2 hints, 60 the fused full sweep forced on,
-//             61 the fused full sweep forced off (two launches per sweep);
-//   -DCULGT_MEASURE only: 1-14, 21-32 (or_sweep_measure.cu), 41-44 launch-level slab schedules,
-//             >= 100000 fused-sweep parameter sweeps (100000 + 50000*alternate + 1000*lag + hints code).
+//             traversal / programmatic dependent launch / L2 hints;
+//   -DCULGT_MEASURE only: 1-14, 21-32 (or_sweep_measure.cu), 41-44 launch-level slab schedules, 60 the
+//             fused one-kernel full sweep (or_sweep_fused.cu; needs a workspace), >= 100000 its parameter
+//             sweeps (100000 + 50000*alternate + 1000*lag + hints code).
 bool sweep_variant_known(int variant) {
   switch (variant) {
-    case 0: case 20: case 24: case 33: case 34: case 60: case 61: return true;
+    case 0: case 20: case 24: case 33: case 34: return true;
     default: break;
   }
 #ifdef CULGT_MEASURE
   if ((variant >= 1 && variant <= 14) || (variant >= 21 && variant <= 32) || (variant >= 41 && variant <= 44) ||
-      (variant >= 100000 && variant < 200000))
+      variant == 60 || (variant >= 100000 && variant < 200000))
     return true;
 #endif
   return false;
@@ -151,31 +151,24 @@ cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, doubl
   return cudaErrorInvalidValue;
 }
 
-// Whether variant 0 takes the fused schedule: where one launch per full sweep wins by measurement
-// (DESIGN.md 6.1): SU(3) fields between 0.87 and 2.5 L2 sizes (32^4 fp32-12: 201 MB on a 126 MB L2).
-static bool fused_by_default(const LatticeDesc& d) {
-  if (d.group != 3) return false;
-  const double link_bytes = (d.precision == 32 && d.params == 18) ? 80.0 : (double)d.params * (d.precision / 8);
-  const double field = 4.0 * (double)d.V * link_bytes;
-  const double l2 = device_l2_bytes();
-  return field > 0.87 * l2 && field < 2.5 * l2;
-}
-
 cudaError_t launch_or_full_sweeps(const LatticeDesc& d, void* links, double* workspace, int n_sweeps, double omega,
                                   int variant, const int* stop_flag, cudaStream_t st) {
   if (n_sweeps <= 0) return cudaSuccess;
-  bool fused = workspace != nullptr && (variant == 60 || (variant == 0 && fused_by_default(d)));
-  int lag = 0, hints = kFusedDefaultHints;
-  bool alternate = true;
 #ifdef CULGT_MEASURE
-  if (variant >= 100000 && workspace != nullptr) {
-    const int v = variant - 100000;
-    fused = true;
-    alternate = v >= 50000;
-    lag = (v % 50000) / 1000;
-    int code = v % 1000, h = 0;              // base-3 digits: black load, black store, white load, white store
-    for (int i = 0; i < 4; ++i) { h |= (code % 3) << (2 * i); code /= 3; }
-    hints = h;
+  if ((variant == 60 || variant >= 100000) && workspace != nullptr) {
+    int lag = 0, hints = kFusedDefaultHints;
+    bool alternate = true;
+    if (variant >= 100000) {
+      const int v = variant - 100000;
+      alternate = v >= 50000;
+      lag = (v % 50000) / 1000;
+      int code = v % 1000;                     // base-3 digits: black load, black store, white load, white store
+      hints = 0;
+      for (int i = 0; i < 4; ++i) { hints |= (code % 3) << (2 * i); code /= 3; }
+    }
+    void* ctl = workspace + fused_ctl_offset_doubles(d.geom);
+    const cudaError_t e = launch_or_sweeps_fused(d, links, omega, ctl, n_sweeps, lag, hints, alternate, stop_flag, st);
+    if (e != cudaErrorNotSupported) return e;     // lattice does not fit the fused schedule: two launches
   }
   if (variant >= 41 && variant <= 44) {
     bool fits = true;                          // cudaErrorNotSupported depends on the lattice only: first call
@@ -186,12 +179,9 @@ cudaError_t launch_or_full_sweeps(const LatticeDesc& d, void* links, double* wor
     }
     if (fits) return cudaSuccess;
   }
+#else
+  (void)workspace;
 #endif
-  if (fused) {
-    void* ctl = workspace + fused_ctl_offset_doubles(d.geom);
-    const cudaError_t e = launch_or_sweeps_fused(d, links, omega, ctl, n_sweeps, lag, hints, alternate, stop_flag, st);
-    if (e != cudaErrorNotSupported) return e;     // lattice does not fit the fused schedule: two launches
-  }
   const int half_variant = (variant >= 40) ? 0 : variant;
   for (int i = 0; i < n_sweeps; ++i)
     for (int parity = 0; parity < 2; ++parity) {

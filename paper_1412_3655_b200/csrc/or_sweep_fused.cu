@@ -19,6 +19,13 @@
 // holds a ticket only while it is running.
 // The lag L keeps the white front far enough behind the black front that in the steady state no
 // CTA ever waits.  The last CTA to leave resets the control block for the next launch.
+//
+// MEASURED AND REJECTED (profiles/r2_fused_sweep.md): at 32^4 fp32-12 the schedule does what it was
+// built for -- DRAM traffic per full sweep falls from 691 MB to 542 MB, L2 hit rate from 19 % to 66 % --
+// but the sweep takes 127-136 us against 111 us for two launches, because the half-sweep is not
+// bound by DRAM: the same kernel on an L2-RESIDENT 24^4 field runs at the same 6.9 TB/s per site
+// update as on the 32^4 field streamed from HBM.  Compiled only with -DCULGT_MEASURE.
+#ifdef CULGT_MEASURE
 #include "staged.cuh"
 #include "kernels.h"
 
@@ -210,3 +217,4 @@ cudaError_t launch_or_sweeps_fused(const LatticeDesc& d, void* links, double ome
 }
 
 }  // namespace culgt
+#endif  // CULGT_MEASURE

@@ -96,9 +96,6 @@ def test_argument_errors_by_return_code():
     assert lib.culgt_landau_fix(ref, ok_ptr, ok_ptr, 1.7, 1e-10, 10, 0, None, None, None, None) == E["CULGT_ERR_ARG"]
     assert lib.culgt_fix_host(ref, None, ok_ptr, ok_ptr, ok_ptr, 1, 1.7, None, None, None) == E["CULGT_ERR_NULL"]
     assert lib.culgt_set_sweep_variant(-3) == E["CULGT_ERR_ARG"]
-    assert lib.culgt_or_sweeps_ws(ref, ok_ptr, None, 1, 1.7, None) == E["CULGT_ERR_NULL"]
-    assert lib.culgt_or_sweeps_ws(ref, ok_ptr, ok_ptr, -1, 1.7, None) == E["CULGT_ERR_ARG"]
-    assert lib.culgt_or_sweeps_ws(ref, ok_ptr, ok_ptr, 1, 2.0, None) == E["CULGT_ERR_OMEGA"]
     # the widened entry points (Coulomb gauge, series power, annealing, re-unitarisation, autotuner)
     assert lib.culgt_or_sweep_coulomb(ref, None, 0, 1.7, None) == E["CULGT_ERR_NULL"]
     assert lib.culgt_or_sweep_coulomb(ref, ok_ptr, 3, 1.7, None) == E["CULGT_ERR_PARITY"]
@@ -130,11 +127,12 @@ def test_product_build_rejects_measurement_variants():
     lib = culgt.lib()
     E = culgt.ERRORS
     assert culgt.culgt_measure_build() is False, "the committed build step must produce the product library"
-    for v in (0, 20, 24, 33, 34, 60, 61):
+    assert not hasattr(lib, "culgt_or_sweeps_ws") and not hasattr(lib, "culgt_fused_schedule")
+    for v in (0, 20, 24, 33, 34):
         assert lib.culgt_set_sweep_variant(v) == culgt.CULGT_OK
         assert culgt.culgt_get_sweep_variant() == v
     lib.culgt_set_sweep_variant(0)
-    for v in (11, 14, 25, 28, 32, 1, 2, 4, 8, 21, 22, 23, 26, 27, 29, 30, 31, 41, 44, 51, 54, 99, 100, 100000, 150123):
+    for v in (11, 14, 25, 28, 32, 1, 2, 4, 8, 21, 22, 23, 26, 27, 29, 30, 31, 41, 44, 51, 54, 60, 61, 99, 100, 100000, 150123):
         assert lib.culgt_set_sweep_variant(v) == E["CULGT_ERR_ARG"], v
         assert culgt.culgt_get_sweep_variant() == 0
 
@@ -150,29 +148,6 @@ def test_sweep_variant_is_per_thread():
     t.join()
     assert seen == [0] and culgt.culgt_get_sweep_variant() == 33
     lib.culgt_set_sweep_variant(0)
-
-
-def test_fused_schedule_order_and_dependencies():
-    """The slice-task order of the fused full sweep (csrc/or_sweep_fused.cu): every slice of both
-    parities exactly once, and every white slice t after the black slices t-1, t, t+1 (periodic) --
-    the property that makes the ticket scheme deadlock-free."""
-    import ctypes as C
-    lib = culgt.lib()
-    for n3 in (2, 4, 6, 8, 12, 32, 96, 512):
-        for lag in (0, 1, 2, 5, 40, 1000):
-            for direction in (0, 1):
-                buf = (C.c_uint * (2 * n3))()
-                lib.culgt_fused_schedule(n3, lag, direction, buf)
-                tasks = [(w >> 31, w & 0x7fffffff) for w in buf]
-                assert sorted(tasks) == sorted((p, t) for p in (0, 1) for t in range(n3))
-                pos = {task: i for i, task in enumerate(tasks)}
-                for t in range(n3):
-                    for nb in ((t - 1) % n3, t, (t + 1) % n3):
-                        assert pos[(0, nb)] < pos[(1, t)], (n3, lag, direction, t, nb)
-                if direction == 0:
-                    assert tasks[0] == (0, 0)
-                else:
-                    assert tasks[0] == (0, n3 - 1)
 
 
 def test_no_cpu_fallback():

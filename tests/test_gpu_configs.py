@@ -272,28 +272,3 @@ def test_su2_32x4_links_theta_F_transform(name):
     f.transform(g)
     err = max_abs_diff(f.download(), ref)
     assert err < (1e-13 if prec == 64 else 2e-6), err
-
-
-@pytest.mark.parametrize("name", ["cfg3_fp32", "cfg3_fp64", "cfg3_fp32_18", "cfg3_fp64_12"])
-def test_cfg3_fused_sweep_bit_identical_and_matches_oracle(name):
-    """The fused one-kernel full sweep (culgt_or_sweeps_ws, csrc/or_sweep_fused.cu) at the headline
-    volume, where its dependency counters and the lag between the black and the white front are really
-    exercised (thousands of tickets per resident CTA): all 4V links after sweep 1 against the oracle,
-    and bit-identical to the two-launch schedule after 6 sweeps (ascending and descending passes)."""
-    c, f, ref = field_and_ref(name)
-    dims, om, prec = c["dims"], c["omega"], c["precision"]
-    u = named_input(name)
-    oracle.full_sweep(dims, ref, om)
-    culgt.culgt_set_sweep_variant(60)
-    try:
-        f.sweep_ws(om, 1)
-        err = max_abs_diff(f.download(), ref)
-        assert err < TOL_LINK[prec], err
-        f.sweep_ws(om, 5)
-        fused = f.links.clone()
-    finally:
-        culgt.culgt_set_sweep_variant(0)
-    f.upload(u)
-    f.sweep(om, 6)
-    torch.cuda.synchronize()
-    assert torch.equal(fused, f.links)

@@ -203,66 +203,12 @@ def test_autotuner_picks_a_result_equivalent_mapping():
         scratch = GpuField(dims, 3, precision, params, u)
         try:
             v, us = culgt.culgt_autotune_sweep(scratch.lat, scratch.links, scratch.ws, 1.7, 2)
-            assert v in variants_for(precision, params) + [20, 60, 61] and us > 0
+            assert v in variants_for(precision, params) and us > 0
             assert culgt.culgt_get_sweep_variant() == v
             ref = storage_input(u, precision, params)
             oracle.full_sweep(dims, ref, 1.7)
             f = GpuField(dims, 3, precision, params, u)
-            f.sweep_ws(1.7)
+            f.sweep(1.7)
             assert np.abs(f.download() - li.from_real(ref)).max() < TOL_LINK[precision]
         finally:
             culgt.culgt_set_sweep_variant(0)
-
-
-FUSED_DIMS = [(8, 8, 8, 8), (8, 8, 8, 12), (16, 8, 8, 6), (8, 8, 4, 2), (8, 8, 8, 4), (8, 4, 8, 16), (4, 6, 2, 8)]
-
-
-@pytest.mark.parametrize("dims", FUSED_DIMS)
-@pytest.mark.parametrize("precision,params", SU3_STORES)
-def test_fused_full_sweep_is_the_same_sweep(dims, precision, params):
-    """culgt_or_sweeps_ws with variant 60 (csrc/or_sweep_fused.cu: black and white half-sweeps
-    interleaved slice by slice inside ONE persistent kernel, tickets + per-slice completion counters,
-    every other sweep descending) only reorders independent site updates: one sweep must agree with
-    the oracle, and three more must be bit-identical to the two-launch schedule (variant 61).  Covers
-    N3 = 2 (both black slices first), N3 = 4 (lag clamped), long time extents, and (4,6,2,8), which
-    does not hold whole site blocks per slice and takes the two-launch fallback.  With -DCULGT_MEASURE
-    also the launch-level slab schedules 41-43."""
-    u = make(dims, 3, 46)
-    ref = storage_input(u, precision, params)
-    oracle.full_sweep(dims, ref, 1.7)
-    outs = {}
-    for variant in [61, 60, 0] + ([41, 42, 43] if culgt.culgt_measure_build() else []):
-        culgt.culgt_set_sweep_variant(variant)
-        try:
-            f = GpuField(dims, 3, precision, params, u)
-            f.sweep_ws(1.7, 1)
-            assert np.abs(f.download() - li.from_real(ref)).max() < TOL_LINK[precision], variant
-            f.sweep_ws(1.7, 3)
-            f.sweep_ws(1.7, 2)          # a second call: the control block is set up again
-            torch.cuda.synchronize()
-            outs[variant] = f.download()
-        finally:
-            culgt.culgt_set_sweep_variant(0)
-    for variant, out in outs.items():
-        assert np.array_equal(out, outs[61]), variant
-
-
-def test_fused_sweep_in_the_driver_loop_and_host_call():
-    """culgt_landau_fix and culgt_fix_host hand their workspace to the sweeps: with the fused schedule
-    forced on they must stop at the same sweep with the same theta and F, bit for bit."""
-    dims = (8, 8, 8, 8)
-    u = make(dims, 3, 49)
-    res = {}
-    for variant in (61, 60):
-        culgt.culgt_set_sweep_variant(variant)
-        try:
-            f = GpuField(dims, 3, 64, 18, u)
-            res[variant] = culgt.culgt_landau_fix(f.lat, f.links, f.ws, 1.7, 1e-12, 400, 3)
-            host = torch.from_numpy(li.to_real(u)).pin_memory()
-            can = torch.empty_like(host, device="cuda")
-            res[variant] += culgt.culgt_fix_host(f.lat, host, can, f.links, f.ws, 5, 1.7)
-            res[variant] += (host.numpy().tobytes(),)
-        finally:
-            culgt.culgt_set_sweep_variant(0)
-    assert res[60] == res[61]
-    assert res[60][1] < 1e-12 and res[60][0] % 3 == 0
