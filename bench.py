@@ -14,9 +14,17 @@ value       site-updates/s over all ranks, inputs resident in HBM, CUDA events, 
 e2e         the same through culgt_fix_host: pinned HOST canonical field -> H2D -> pack -> K
             sweeps -> theta, F -> unpack -> D2H, all inside the timed region (one job of K steps;
             the byte counts are per step = job bytes / K).
-roofline    dominant kernel = the half-sweep; algorithmic bytes per launch = 2 * field bytes
-            (every link read once and written once) / the average
-            launch duration measured live with CUDA events on the launching stream.
+roofline    dominant kernel = the half-sweep; `achieved` = ALGORITHMIC bytes per launch (2 * field
+            bytes: every link read once and written once) / the average
+            launch duration measured live with CUDA events on the launching stream.  Part of
+            those bytes is served by the L2 (the white half-sweep walks the lattice backwards):
+            `dram_achieved` = the DRAM bytes per launch of the committed steady-state ncu capture
+            (profiles/roofline_traffic.csv, stamped with the kernel it was taken on) / the same
+            duration is what HBM itself moves.
+kernels     the other kernels of the path at the same workload: theta+F, pack, unpack, gauge transform.
+extra_workloads   the second half of BASELINE.json configs[3] (fp64 18-parameter) and configs[4]
+            (48^3 x 96 fp32-12, 64^4 fp64-18), a few steps each, and the driver loop
+            (culgt_landau_fix) on the latency-bound configs[0..2].
 cpu_baseline the oracle (oracle/, as it stands) timed on this host's cores on a bounded sample.
 --impl reference  times the oracle itself (rank 0 only), same metric / config / unit.
 
@@ -64,6 +72,12 @@ def parse_args():
                     help="> 0: time simulated-annealing sweeps at this temperature instead of overrelaxation (DESIGN.md C-25)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extra", action="store_true",
+                    help="skip the extra_workloads / kernels blocks (they only run for the default workload, N = 1)")
+    ap.add_argument("--extra-steps", type=int, default=10, help="timed sweeps of each extra workload")
+    ap.add_argument("--extra-workloads", default=None,
+                    help="comma-separated workloads for the extra_workloads block (default: cfg3_fp64,cfg4_fp32,"
+                         "cfg4_fp64 when the main workload is cfg3_fp32, none otherwise)")
     return ap.parse_args()
 
 
@@ -76,18 +90,25 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def committed_traffic(workload: str, capture: str = "ncu_set_full_cold_cache"):
-    """dram bytes (read + write) per half-sweep launch from the committed ncu captures
-    (profiles/roofline_traffic.csv), or None."""
+def committed_traffic(workload: str, capture: str, kernel: str):
+    """DRAM bytes (read + write) per half-sweep launch from the committed ncu captures
+    (profiles/roofline_traffic.csv: workload, capture, read, write, commit, kernel, source).  They
+    cannot be measured live without ncu attached, so every row names the commit and the kernel
+    (culgt_sweep_kernel_name) it was captured on; a row taken on another kernel than the one this
+    run launches is reported as stale instead of being used.  Returns (bytes or None, info dict)."""
     try:
         with open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) as f:
             for line in f:
-                p = line.strip().split(",")
-                if len(p) >= 4 and p[0] == workload and p[1] == capture:
-                    return int(p[2]) + int(p[3])
-    except Exception:
-        pass
-    return None
+                p = [x.strip() for x in line.strip().split(";")]
+                if len(p) >= 7 and p[0] == workload and p[1] == capture:
+                    info = {"commit": p[4], "kernel": p[5], "source": p[6]}
+                    if p[5] != kernel:
+                        info["stale"] = f"captured on another kernel than this run's ({kernel})"
+                        return None, info
+                    return int(p[2]) + int(p[3]), info
+    except Exception as e:      # pragma: no cover
+        return None, {"stale": f"profiles/roofline_traffic.csv unreadable: {e}"}
+    return None, {"stale": "no capture committed for this workload"}
 
 
 class ClockSampler:
@@ -97,6 +118,7 @@ class ClockSampler:
 
     def __init__(self, index: int):
         self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.t0 = None
         self._stop = threading.Event()
         self._thread = None
         try:
@@ -122,6 +144,7 @@ class ClockSampler:
             time.sleep(0.004)
 
     def start(self):
+        self.t0 = time.perf_counter()
         if self.nv is not None:
             self._thread = threading.Thread(target=self._run, daemon=True)
             self._thread.start()
@@ -132,7 +155,8 @@ class ClockSampler:
             self._thread.join()
         med = float(np.median(self.samples)) if self.samples else None
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(self.samples)}
+                "samples": len(self.samples),
+                "window_ms": 1e3 * (time.perf_counter() - self.t0) if self.t0 else None}
 
 
 def time_oracle(dims, group, ur, omega, max_sweeps, budget_s, threads, gauge="landau"):
@@ -231,10 +255,165 @@ def workload_config(args, cfg):
                     f"{cfg['kind']} eps={cfg['eps']} scramble={cfg['scramble']} seed={cfg['seed']}",
         "step": "one full sweep (black+white half-sweep) = V site updates; theta and F every "
                 f"{args.check_every} steps inside the timed region",
-        "l2": "no flush: the field is larger than the 126 MB L2 for the 32^4 and larger workloads "
-              "and every half-sweep streams all of it",
+        "l2": "no flush between steps: the field (201 MB ... 9.7 GB at 32^4 and above) is larger than the "
+              "126 MB L2; the white half-sweep walks the lattice backwards, so the L2 carries the last "
+              "lines of one half-sweep into the next (15 % of the traffic at 32^4 fp32-12, "
+              "roofline.traffic_steady_state) -- part of the method's steady state, reported, not hidden",
         "parallelism": "replicas only (one independent configuration per GPU)",
     }
+
+
+class Field:
+    """One seeded configuration resident on the GPU: pinned host canonical field, device canonical
+    scratch, internal links, workspace."""
+
+    def __init__(self, culgt, torch, name, rank):
+        cfg = li.CONFIGS[name]
+        self.name, self.cfg = name, cfg
+        self.dims, self.omega = cfg["dims"], cfg["omega"]
+        self.V = li.volume(self.dims)
+        self.lat = culgt.Lattice(tuple(self.dims), cfg["group"], cfg["precision"], cfg["params"])
+        u = li.make_config(self.dims, cfg["group"], cfg["kind"], rank_seed(cfg["seed"], rank), eps=cfg["eps"],
+                           scramble=cfg["scramble"])
+        np_dt = np.float32 if cfg["precision"] == 32 else np.float64
+        self.host = torch.from_numpy(li.to_real(u, np_dt)).pin_memory()
+        del u
+        self.can_dev = torch.empty_like(self.host, device="cuda")
+        self.links = culgt.alloc_links(self.lat)
+        self.ws = culgt.alloc_workspace(self.lat)
+        self.can_dev.copy_(self.host)
+        culgt.culgt_pack(self.lat, self.can_dev, self.links)
+        torch.cuda.synchronize()
+        # algorithmic bytes: the stored parameters (fp32-18 keeps 2 pad floats per link that are not counted)
+        self.field_bytes = 4 * self.V * cfg["params"] * (cfg["precision"] // 8)
+
+
+def time_sweep_loop(torch, field, sweeps, check, steps, warmup, check_every, barrier, sampler=None, window_ms=60.0):
+    """W warm-up sweeps, then K timed sweeps with a check every check_every; CUDA events on the current
+    stream.  With a sampler: when the timed window is shorter than window_ms, untimed sweeps before and
+    after it keep the GPU under the same load until NVML has been sampled for that long, so that the
+    clocks record never rests on one sample (a 20-step run at 32^4 is 2 ms of work)."""
+    stream = torch.cuda.current_stream()
+    sweeps(max(warmup, 3))
+    check()
+    barrier()
+
+    def roll_until(t_end):
+        while time.perf_counter() < t_end:
+            sweeps(8)
+            torch.cuda.synchronize()
+
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    checks = []
+    t_start = time.perf_counter()
+    if sampler is not None:
+        sampler.start()
+        roll_until(t_start + 0.4e-3 * window_ms)
+    ev0.record(stream)
+    done = 0
+    while done < steps:
+        n = min(check_every, steps - done)
+        sweeps(n)
+        done += n
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        check()
+        b.record(stream)
+        checks.append((a, b))
+    ev1.record(stream)
+    if sampler is not None:
+        torch.cuda.synchronize()
+        roll_until(t_start + 1e-3 * window_ms)
+    barrier()
+    clocks = sampler.stop() if sampler is not None else None
+    elapsed_ms = ev0.elapsed_time(ev1)
+    check_ms = sum(a.elapsed_time(b) for a, b in checks)
+    return {"elapsed_ms": elapsed_ms, "check_ms": check_ms, "n_checks": len(checks), "clocks": clocks,
+            "launch_ms": (elapsed_ms - check_ms) / (2 * steps)}
+
+
+def time_kernel(torch, fn, reps=20, warm=3):
+    """Average device time of fn() in microseconds (CUDA events on the current stream)."""
+    stream = torch.cuda.current_stream()
+    for _ in range(warm):
+        fn()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(reps):
+        fn()
+    b.record(stream)
+    torch.cuda.synchronize()
+    return 1e3 * a.elapsed_time(b) / reps
+
+
+def other_kernels(culgt, torch, f, peak):
+    """theta+F, pack, unpack, gauge transform at the workload of `f`: us per call, algorithmic GB/s
+    (bytes the call must move once), fraction of the measured copy peak."""
+    scal = torch.zeros(2, dtype=torch.float64, device="cuda")
+    cbytes = culgt.culgt_canonical_bytes(f.lat)
+    g = li.haar_su3(f.V, f.cfg["seed"] + 500) if f.cfg["group"] == 3 else li.haar_su2(f.V, f.cfg["seed"] + 500)
+    gt = torch.from_numpy(li.to_real(g, np.float32 if f.cfg["precision"] == 32 else np.float64)).cuda()
+    del g
+    spec = {
+        "theta_F": (lambda: culgt.culgt_gauge_precision_functional(f.lat, f.links, f.ws, scal[0:1], scal[1:2]),
+                    f.field_bytes, "one read of the field"),
+        "pack": (lambda: culgt.culgt_pack(f.lat, f.can_dev, f.links), cbytes + f.field_bytes,
+                 "canonical read + internal write"),
+        "unpack": (lambda: culgt.culgt_unpack(f.lat, f.links, f.can_dev), cbytes + f.field_bytes,
+                   "internal read + canonical write"),
+        "gauge_transform": (lambda: culgt.culgt_gauge_transform(f.lat, f.links, gt),
+                            2 * f.field_bytes + gt.numel() * gt.element_size(), "links read + written, g once"),
+    }
+    out = {}
+    culgt.culgt_unpack(f.lat, f.links, f.can_dev)      # pack/unpack round-trip on the current field
+    for name, (fn, nbytes, what) in spec.items():
+        us = time_kernel(torch, fn)
+        gbs = nbytes / (us * 1e-6) / 1e9
+        out[name] = {"us": us, "bytes": nbytes, "what": what, "gbs": gbs, "frac": gbs / peak}
+    return out
+
+
+def driver_loop_times(culgt, torch, rank):
+    """The paper's driver loop on the latency-bound BASELINE.json configs[0..2]: wall time of
+    culgt_landau_fix (stopping decision on the device, one host synchronisation per batch of checks)
+    next to the same loop driven from the host with a synchronisation at every check."""
+    runs = {"cfg0": (1e-20, 5000, 1), "cfg1": (0.0, 200, 10), "cfg2": (0.0, 1000, 10)}
+    out = {}
+    for name, (target, max_sweeps, every) in runs.items():
+        f = Field(culgt, torch, name, rank)
+        scal = torch.zeros(2, dtype=torch.float64, device="cuda")
+
+        def host_loop():
+            culgt.culgt_gauge_precision_functional(f.lat, f.links, f.ws, scal[0:1], scal[1:2])
+            theta, done = float(scal[0].item()), 0
+            while not (theta < target) and done < max_sweeps:
+                n = min(every, max_sweeps - done)
+                culgt.culgt_or_sweeps(f.lat, f.links, n, f.omega)
+                done += n
+                culgt.culgt_gauge_precision_functional(f.lat, f.links, f.ws, scal[0:1], scal[1:2])
+                theta = float(scal[0].item())
+            return done, theta
+
+        res = {}
+        for label, loop in (("host_sync_every_check", host_loop),
+                            ("device_stop_flag", lambda: culgt.culgt_landau_fix(f.lat, f.links, f.ws, f.omega, target,
+                                                                                max_sweeps, every)[:2])):
+            best = None
+            for _ in range(3):
+                culgt.culgt_pack(f.lat, f.can_dev, f.links)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                done, theta = loop()
+                torch.cuda.synchronize()
+                dt = time.perf_counter() - t0
+                best = dt if best is None else min(best, dt)
+            res[label] = {"wall_ms": 1e3 * best, "sweeps": done, "theta": theta,
+                          "us_per_sweep": 1e6 * best / max(done, 1), "value": f.V * done / best}
+        res["speedup"] = res["host_sync_every_check"]["wall_ms"] / res["device_stop_flag"]["wall_ms"]
+        res["workload"] = f"{name}: {'x'.join(map(str, f.dims))} SU({f.cfg['group']}) fp{f.cfg['precision']}, " \
+                          f"theta checked every {every} sweep(s), target {target:g}, at most {max_sweeps} sweeps"
+        out[name] = res
+    return out
 
 
 def main():
@@ -256,50 +435,39 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    cfg = li.CONFIGS[args.workload]
-    dims, omega = cfg["dims"], cfg["omega"]
-    V = li.volume(dims)
-    lat = culgt.Lattice(tuple(dims), cfg["group"], cfg["precision"], cfg["params"])
-    culgt.culgt_set_sweep_variant(args.variant)
-
-    # seeded synthetic input, one independent configuration per rank
-    u = li.make_config(dims, cfg["group"], cfg["kind"], rank_seed(cfg["seed"], rank), eps=cfg["eps"],
-                       scramble=cfg["scramble"])
-    np_dt = np.float32 if cfg["precision"] == 32 else np.float64
-    host = torch.from_numpy(li.to_real(u, np_dt)).pin_memory()
-    del u
-    can_dev = torch.empty_like(host, device="cuda")
-    links = culgt.alloc_links(lat)
-    ws = culgt.alloc_workspace(lat)
-    scal = torch.zeros(2, dtype=torch.float64, device="cuda")
-    can_dev.copy_(host)
-    culgt.culgt_pack(lat, can_dev, links)
-    torch.cuda.synchronize()
-    stream = torch.cuda.current_stream()
-
     def barrier():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
+    culgt.culgt_set_sweep_variant(args.variant)
+    f = Field(culgt, torch, args.workload, rank)      # seeded synthetic input, one independent configuration per rank
+    cfg, lat, links, ws, V, omega = f.cfg, f.lat, f.links, f.ws, f.V, f.omega
+    peak, peak_src = measured_peak()
+
     coulomb = args.gauge == "coulomb"
-    n3 = int(dims[3])
+    n3 = int(f.dims[3])
+    scal = torch.zeros(2 * n3 if coulomb else 2, dtype=torch.float64, device="cuda")   # Coulomb: theta_t, F_t per slice
+    with_ws = hasattr(culgt.lib(), "culgt_or_sweeps_ws")     # measurement library: variant 60 needs the workspace
     if coulomb:
-        scal = torch.zeros(2 * n3, dtype=torch.float64, device="cuda")     # theta_t, F_t per slice
-    sweeps = culgt.culgt_or_sweeps_coulomb if coulomb else culgt.culgt_or_sweeps
+        sweeps = lambda n: culgt.culgt_or_sweeps_coulomb(lat, links, n, omega)  # noqa: E731
+    elif with_ws:
+        sweeps = lambda n: culgt.culgt_or_sweeps_ws(lat, links, ws, n, omega)  # noqa: E731
+    else:
+        sweeps = lambda n: culgt.culgt_or_sweeps(lat, links, n, omega)  # noqa: E731
     if args.sa_temperature > 0:
         if coulomb or args.series_order > 0:
             raise SystemExit("--sa-temperature applies to Landau gauge and excludes --series-order")
-        sweeps = lambda lat_, links_, n_, om_: culgt.culgt_sa_anneal(lat_, links_, args.sa_temperature, args.sa_temperature, n_, 2024)  # noqa: E731
+        sweeps = lambda n: culgt.culgt_sa_anneal(lat, links, args.sa_temperature, args.sa_temperature, n, 2024)  # noqa: E731
     if args.micro:
         if coulomb or args.series_order > 0 or args.sa_temperature > 0:
             raise SystemExit("--micro applies to Landau gauge and excludes --series-order / --sa-temperature")
-        sweeps = lambda lat_, links_, n_, om_: culgt.culgt_micro_sweeps(lat_, links_, n_)  # noqa: E731
+        sweeps = lambda n: culgt.culgt_micro_sweeps(lat, links, n)  # noqa: E731
     if args.series_order > 0:
         if coulomb:
             raise SystemExit("--series-order applies to Landau gauge")
-        sweeps = lambda lat_, links_, n_, om_: culgt.culgt_or_sweeps_series(lat_, links_, n_, om_, args.series_order)  # noqa: E731
+        sweeps = lambda n: culgt.culgt_or_sweeps_series(lat, links, n, omega, args.series_order)  # noqa: E731
 
     def check():
         if coulomb:
@@ -307,34 +475,11 @@ def main():
         else:
             culgt.culgt_gauge_precision_functional(lat, links, ws, scal[0:1], scal[1:2])
 
-    # ---- warm-up
-    sweeps(lat, links, max(args.warmup, 3), omega)
-    check()
-    barrier()
-
-    # ---- timed region: K steps, theta/F every check_every steps
-    sampler = ClockSampler(local_rank)
-    n_checks = 0
-    check_events = []
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler.start()
-    ev0.record(stream)
-    done = 0
-    while done < args.steps:
-        n = min(args.check_every, args.steps - done)
-        sweeps(lat, links, n, omega)
-        done += n
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        check()
-        b.record(stream)
-        check_events.append((a, b))
-        n_checks += 1
-    ev1.record(stream)
-    barrier()
-    clocks = sampler.stop()
-    elapsed_ms = ev0.elapsed_time(ev1)
-    check_ms = sum(a.elapsed_time(b) for a, b in check_events)
+    # ---- the timed region: K steps, theta/F every check_every steps
+    t = time_sweep_loop(torch, f, sweeps, check, args.steps, args.warmup, args.check_every, barrier,
+                        ClockSampler(local_rank))
+    elapsed_ms, check_ms, n_checks, clocks, launch_ms = (t["elapsed_ms"], t["check_ms"], t["n_checks"], t["clocks"],
+                                                         t["launch_ms"])
     res = scal.cpu()
     theta, F = (float(res[:n3].max()), float(res[n3:].mean())) if coulomb else (float(res[0]), float(res[1]))
 
@@ -343,16 +488,21 @@ def main():
 
     sweep_launches = 2 * args.steps
     gpu_launches = sweep_launches + n_checks * 2        # fused theta+F: partial + final kernel
-    launch_ms = (elapsed_ms - check_ms) / sweep_launches
-    # algorithmic bytes: the stored parameters (fp32-18 keeps 2 pad floats per link that are not counted)
-    field_bytes = 4 * V * cfg["params"] * (cfg["precision"] // 8)
-    alg_bytes_per_launch = 2 * field_bytes
+    alg_bytes_per_launch = 2 * f.field_bytes
     achieved_gbs = alg_bytes_per_launch / (launch_ms * 1e-3) / 1e9
-    peak, peak_src = measured_peak()
+    kernel_name = culgt.culgt_sweep_kernel_name(lat)
+    traffic, traffic_info = committed_traffic(args.workload, "ncu_set_full_cold_cache", kernel_name)
+    steady, steady_info = committed_traffic(args.workload, "steady_state", kernel_name)
+    plain_or = not (coulomb or args.micro or args.series_order > 0 or args.sa_temperature > 0 or args.variant != 0)
+    if not plain_or:
+        traffic = steady = None
+        traffic_info = steady_info = {"stale": "captures exist for the default overrelaxation sweep only"}
 
     # ---- end to end through the host-buffer entry point
     e2e = None
     if not args.no_e2e:
+        host, can_dev = f.host, f.can_dev
+
         def host_job(n):
             if not coulomb:
                 return culgt.culgt_fix_host(lat, host, can_dev, links, ws, n, omega)
@@ -360,7 +510,7 @@ def main():
             # unpack, D2H of the field and of the 2*N3 scalars)
             can_dev.copy_(host, non_blocking=True)
             culgt.culgt_pack(lat, can_dev, links)
-            sweeps(lat, links, n, omega)
+            sweeps(n)
             check()
             culgt.culgt_unpack(lat, links, can_dev)
             host.copy_(can_dev, non_blocking=True)
@@ -380,11 +530,44 @@ def main():
                "job": f"one {'culgt_fix_host call' if not coulomb else 'host job (pack, sweeps, theta_t/F_t, unpack)'} = H2D {cbytes} B + pack + {args.steps} sweeps + theta,F + unpack + D2H {cbytes} B",
                "theta": th_e, "F": F_e}
 
+    # ---- the other kernels of the path at this workload; the other BASELINE.json workloads; the driver loop
+    kernels = extra = loops = None
+    extra_names = (args.extra_workloads.split(",") if args.extra_workloads
+                   else ["cfg3_fp64", "cfg4_fp32", "cfg4_fp64"] if args.workload == "cfg3_fp32" else [])
+    if world == 1 and not args.no_extra and plain_or and extra_names:
+        kernels = other_kernels(culgt, torch, f, peak)
+        del f, links, ws
+        torch.cuda.empty_cache()
+        extra = []
+        for name in extra_names:
+            fx = Field(culgt, torch, name, rank)
+            sx = torch.zeros(2, dtype=torch.float64, device="cuda")
+            tx = time_sweep_loop(
+                torch, fx, lambda n: culgt.culgt_or_sweeps(fx.lat, fx.links, n, fx.omega),
+                lambda: culgt.culgt_gauge_precision_functional(fx.lat, fx.links, fx.ws, sx[0:1], sx[1:2]),
+                args.extra_steps, 3, args.extra_steps, barrier, ClockSampler(local_rank))
+            gbs = 2 * fx.field_bytes / (tx["launch_ms"] * 1e-3) / 1e9
+            chk_us = 1e3 * tx["check_ms"] / tx["n_checks"]
+            extra.append({
+                "workload": workload_config(argparse.Namespace(**{**vars(args), "workload": name}), fx.cfg)["workload"],
+                "steps": args.extra_steps, "value": fx.V * args.extra_steps / (tx["elapsed_ms"] * 1e-3), "unit": UNIT,
+                "ms_per_step": tx["elapsed_ms"] / args.extra_steps, "launch_us": 1e3 * tx["launch_ms"],
+                "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                             "bytes_per_launch": 2 * fx.field_bytes},
+                "theta_F": {"us": chk_us, "gbs": fx.field_bytes / (chk_us * 1e-6) / 1e9,
+                            "frac": fx.field_bytes / (chk_us * 1e-6) / 1e9 / peak},
+                "clocks": tx["clocks"], "final": {"theta": float(sx[0].item()), "F": float(sx[1].item())},
+            })
+            del fx, sx
+            torch.cuda.empty_cache()
+        loops = driver_loop_times(culgt, torch, rank)
+
     # ---- CPU baseline: the oracle on this host's cores (rank 0, N=1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         threads = min(oracle.max_threads(), os.cpu_count() or 1)
+        dims = cfg["dims"]
         u0 = li.make_config(dims, cfg["group"], cfg["kind"], cfg["seed"], eps=cfg["eps"], scramble=cfg["scramble"])
         if cfg["precision"] == 32:
             u0 = li.round_to_fp32(u0)
@@ -398,6 +581,18 @@ def main():
                "one_core_value": v_one}
 
     if rank == 0:
+        roofline = {"bound": "hbm", "achieved": achieved_gbs, "peak": peak, "unit": "GB/s",
+                    "frac": achieved_gbs / peak, "traffic": traffic, "traffic_steady_state": steady,
+                    "traffic_capture": traffic_info, "traffic_steady_state_capture": steady_info,
+                    "kernel": kernel_name, "bytes_per_launch": alg_bytes_per_launch,
+                    "launch_us": launch_ms * 1e3, "peak_source": peak_src,
+                    "note": "achieved / frac count ALGORITHMIC bytes (the contract); the L2 serves part of them, "
+                            "so frac can exceed 1 -- dram_achieved / dram_frac is what HBM itself moves",
+                    "algorithmic_frac_of_8TBs_nominal": achieved_gbs / 8000.0}
+        if steady is not None:
+            dram_gbs = steady / (launch_ms * 1e-3) / 1e9
+            roofline.update({"dram_achieved": dram_gbs, "dram_frac": dram_gbs / peak,
+                             "dram_frac_of_8TBs_nominal": dram_gbs / 8000.0})
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": elapsed_max_ms / args.steps,
@@ -408,16 +603,12 @@ def main():
             "algorithmic_gbs": value * 16 * (cfg["params"] * cfg["precision"] // 8) / 1e9,
             "gpu_launches": gpu_launches,
             "e2e": e2e,
-            "roofline": {"bound": "hbm", "achieved": achieved_gbs, "peak": peak, "unit": "GB/s",
-                         "frac": achieved_gbs / peak, "traffic": committed_traffic(args.workload),
-                         "traffic_steady_state": committed_traffic(args.workload, "steady_state"),
-                         "kernel": "or_sweep half-sweep", "bytes_per_launch": alg_bytes_per_launch,
-                         "launch_us": launch_ms * 1e3, "peak_source": peak_src,
-                         "frac_of_8TBs_nominal": achieved_gbs / 8000.0},
+            "roofline": roofline,
             "cpu_baseline": cpu,
             "clocks": clocks,
             "final": {"theta": theta, "F": F},
             "check_ms_total": check_ms, "variant": args.variant,
+            "kernels": kernels, "extra_workloads": extra, "driver_loop": loops,
             "context": {"paper": "470 GFlops at 80% of peak bandwidth on a GeForce GTX 580 (PAPER.md L7), context only"},
         }
         print(json.dumps(line), flush=True)

@@ -59,6 +59,7 @@ extern "C" {
 #define CULGT_ERR_ALIGN    -6  /* a device pointer is not 16-byte aligned                      */
 #define CULGT_ERR_CUDA     -7  /* CUDA runtime / launch failure (see culgt_last_cuda_error)    */
 #define CULGT_ERR_ARG      -8  /* another argument is out of range                             */
+#define CULGT_ERR_NCCL     -9  /* NCCL failure, or libnccl.so.2 not found (culgt_last_cuda_error) */
 
 typedef struct {
   int32_t dims[4];    /* N0..N3, x fastest in the canonical site index                        */
@@ -206,6 +207,81 @@ int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, do
                       double theta_target, int max_sweeps, int check_every, int* sweeps_done,
                       double* theta_t_out, double* F_t_out, void* stream);
 
+/* ---- Time-slab decomposition over several GPUs (the paper's only hook is
+ * the title of its ref. [2], "... with Multi-GPUs").  The lattice is cut along t into n_slabs
+ * slabs of T = dims[3] / n_slabs time-slices (T even >= 2).  A slab is described by the LOCAL lattice
+ * (dims[3] = T; culgt_slab_lattice) and stored as an internal field whose planes carry one extra GHOST
+ * slice (culgt_slab_links_bytes): it holds the t-links U_t(y), y in the previous slab's last slice, i.e.
+ * the links U_t(x - t_hat) that the sites x of the slab's first slice read AND write.
+ * Sites of one parity are independent: a half-sweep of parity p runs on all slabs at once with
+ * the unchanged kernels (the links come out bit-identical to the undivided sweep), followed by ONE halo
+ * message each way per boundary, culgt_slab_halo_bytes = N0*N1*N2/2 links each:
+ *     BACK    (direction 1): my ghost slice, parity 1-p  ->  the previous slab's last slice;
+ *     FORWARD (direction 0): my last slice,  parity p    ->  the next slab's ghost slice.
+ * Before the first half-sweep (and before theta/F on freshly packed slabs) both parities go FORWARD once
+ * (culgt_slab_exchange_all_*).  The slab holding time-slices [k*T, (k+1)*T) is slab k; "previous" is
+ * k-1 (mod n_slabs).  The canonical field of slab k is the contiguous part [k*V/n_slabs, (k+1)*V/n_slabs)
+ * of the global canonical field (t is the slowest coordinate).
+ *
+ * culgt_slab_halo_chunks (host only): a message is n_chunks (= vectors per link, <= 9) runs of chunk_bytes
+ *   bytes; offsets[j] = byte offset of run j from the start of the slab's links, for the ghost slice
+ *   (which = 0) or the last slice (which = 1) of the t-links of `parity`.
+ * culgt_slab_halo_peers (host only): the ranks a message of `direction` is sent to / received from
+ *   (FORWARD: to rank+1 from rank-1; BACK: to rank-1 from rank+1; periodic).
+ * culgt_slab_or_sweep / _window: the half-sweep on one slab (all of it / time-slices [t_lo, t_hi) only --
+ *   CULGT_ERR_DESC when the slab holds no whole site blocks per time-slice, or for SU(2)).  Sweeping the
+ *   boundary slices 0 and T-1 first lets both messages travel while the interior [1, T-1) is swept.
+ * culgt_slab_halo_copy: one message between two slabs of this process (same or peer devices).
+ * culgt_slab_theta_F_sums: the slab's RAW sums (sum_x tr[Delta Delta^dagger], sum_{x,mu} Re tr U) as two
+ *   doubles at sums2_dev; culgt_slab_theta_F_combine adds the n_slabs pairs at sums_dev in slab order and
+ *   normalises with the GLOBAL volume (eq. (1), (2)): bit-reproducible for a given n_slabs.
+ * culgt_slab_*_local: drivers for n_slabs slabs held by ONE process (links_slabs: host array of device
+ *   pointers, slab order): n_sweeps full sweeps with the exchanges as device copies on `stream`
+ *   (boundary_first != 0: boundary slices first, as the overlapped schedule orders them); theta and F
+ *   (sums_dev: 2*n_slabs doubles of device scratch).
+ * culgt_slab_comm_*: one slab per rank over NCCL (resolved at run time from the process, normally the
+ *   libnccl torch loaded; CULGT_ERR_NCCL if absent).  unique_id: 128 bytes of HOST memory, made on rank
+ *   0 and distributed by the caller (e.g. torch.distributed broadcast); create is collective.
+ * culgt_slab_or_sweeps_nccl: n_sweeps full sweeps of my slab with ncclSend/ncclRecv halo messages
+ *   around the ring.  comm_stream NULL or == stream: messages on `stream` after each half-sweep;
+ *   otherwise the boundary slices are swept first and the messages travel on comm_stream while the
+ *   interior is swept (the next half-sweep waits for them).
+ * culgt_slab_theta_F_nccl: every rank's raw sums are all-gathered (sums_dev: 2*n_ranks + 2 doubles of
+ *   device scratch) and combined in rank order on every rank. */
+int culgt_slab_lattice(const culgt_lattice* global, int n_slabs, culgt_lattice* local);
+size_t culgt_slab_links_bytes(const culgt_lattice* local);
+size_t culgt_slab_halo_bytes(const culgt_lattice* local);
+int culgt_slab_halo_chunks(const culgt_lattice* local, int parity, int which, size_t* offsets, size_t* chunk_bytes,
+                           int* n_chunks);
+int culgt_slab_halo_peers(int rank, int n_ranks, int direction, int* send_to, int* recv_from);
+int culgt_slab_pack(const culgt_lattice* local, const void* canonical_slab, void* links_slab, void* stream);
+int culgt_slab_unpack(const culgt_lattice* local, const void* links_slab, void* canonical_slab, void* stream);
+int culgt_slab_or_sweep(const culgt_lattice* local, void* links_slab, int parity, double omega, void* stream);
+int culgt_slab_or_sweep_window(const culgt_lattice* local, void* links_slab, int parity, double omega, int t_lo,
+                               int t_hi, void* stream);
+int culgt_slab_halo_copy(const culgt_lattice* local, const void* src_links, void* dst_links, int parity, int direction,
+                         void* stream);
+int culgt_slab_theta_F_sums(const culgt_lattice* local, const void* links_slab, void* workspace, double* sums2_dev,
+                            void* stream);
+int culgt_slab_theta_F_combine(const culgt_lattice* global, const double* sums_dev, int n_slabs, double* theta_dev,
+                               double* F_dev, void* stream);
+int culgt_slab_exchange_all_local(const culgt_lattice* local, void* const* links_slabs, int n_slabs, void* stream);
+int culgt_slab_or_sweeps_local(const culgt_lattice* local, void* const* links_slabs, int n_slabs, int n_sweeps,
+                               double omega, int boundary_first, void* stream);
+int culgt_slab_theta_F_local(const culgt_lattice* global, const culgt_lattice* local, void* const* links_slabs,
+                             int n_slabs, void* workspace, double* sums_dev, double* theta_dev, double* F_dev,
+                             void* stream);
+int culgt_slab_comm_unique_id(void* id128_host);
+int culgt_slab_comm_create(const void* id128_host, int rank, int n_ranks, void** comm_out);
+int culgt_slab_comm_destroy(void* comm);
+int culgt_slab_halo_exchange(void* comm, const culgt_lattice* local, void* links_slab, int parity, int direction,
+                             void* stream);
+int culgt_slab_exchange_all_nccl(void* comm, const culgt_lattice* local, void* links_slab, void* stream);
+int culgt_slab_or_sweeps_nccl(void* comm, const culgt_lattice* local, void* links_slab, int n_sweeps, double omega,
+                              void* comm_stream, void* stream);
+int culgt_slab_theta_F_nccl(void* comm, const culgt_lattice* global, const culgt_lattice* local, const void* links_slab,
+                            void* workspace, double* sums_dev, double* theta_dev, double* F_dev, void* stream);
+
 /* Sweep-schedule selection of the CALLING HOST THREAD.  Every value the product
  * library accepts computes the same update, bit for bit:
  *    0  the default chosen by measurement (20 is its explicit name for the half-sweep kernel);
@@ -218,6 +294,9 @@ int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, do
 int culgt_set_sweep_variant(int variant);
 int culgt_get_sweep_variant(void);
 int culgt_measure_build(void);
+/* Name of the half-sweep kernel instantiation variant 0 launches for this lattice (static string; ""
+ * for an invalid descriptor).  bench.py stamps its committed ncu captures with it. */
+const char* culgt_sweep_kernel_name(const culgt_lattice* lat);
 
 /* Run-time autotuner (the paper's per-GPU selection of the fastest set-up, P:L89 (d)):
  * times every result-equivalent sweep schedule with `sweeps_per_trial` REAL full sweeps each on

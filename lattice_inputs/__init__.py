@@ -81,6 +81,28 @@ def _chunks(n: int):
         yield c, lo, min(n, lo + _CHUNK)
 
 
+def _fill_chunks(out: np.ndarray, make_chunk, threads: bool = True) -> np.ndarray:
+    """out[lo:hi] = make_chunk(c, hi - lo) for every RNG chunk c; chunks are independent (each has its own
+    Philox key), so they may be filled by a few threads -- the array does not depend on how many.
+    (threads=False for generators made of stacked 3x3 matmuls, which run slower side by side.)"""
+    n = out.shape[0]
+
+    def job(item):
+        c, lo, hi = item
+        out[lo:hi] = make_chunk(c, hi - lo)
+
+    items = list(_chunks(n))
+    if len(items) <= 1 or not threads:
+        for item in items:
+            job(item)
+    else:
+        import os
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(max_workers=min(len(items), os.cpu_count() or 1, 16)) as ex:
+            list(ex.map(job, items))
+    return out
+
+
 def _cross_conj(a: np.ndarray, b: np.ndarray) -> np.ndarray:
     return np.conj(np.cross(a, b))
 
@@ -98,13 +120,11 @@ def _gram_schmidt_su3(a: np.ndarray, b: np.ndarray) -> np.ndarray:
 
 
 def haar_su3(n: int, seed: int, stream: int = 0) -> np.ndarray:
-    out = np.empty((n, 3, 3), dtype=np.complex128)
-    for c, lo, hi in _chunks(n):
-        z = _rng(seed, stream, c).standard_normal((hi - lo, 12))
-        a = z[:, 0:3] + 1j * z[:, 3:6]
-        b = z[:, 6:9] + 1j * z[:, 9:12]
-        out[lo:hi] = _gram_schmidt_su3(a, b)
-    return out
+    def chunk(c, m):
+        z = _rng(seed, stream, c).standard_normal((m, 12))
+        return _gram_schmidt_su3(z[:, 0:3] + 1j * z[:, 3:6], z[:, 6:9] + 1j * z[:, 9:12])
+
+    return _fill_chunks(np.empty((n, 3, 3), dtype=np.complex128), chunk)
 
 
 def su2_from_quaternion(a: np.ndarray) -> np.ndarray:
@@ -118,12 +138,12 @@ def su2_from_quaternion(a: np.ndarray) -> np.ndarray:
 
 
 def haar_su2(n: int, seed: int, stream: int = 0) -> np.ndarray:
-    out = np.empty((n, 2, 2), dtype=np.complex128)
-    for c, lo, hi in _chunks(n):
-        z = _rng(seed, stream, c).standard_normal((hi - lo, 4))
+    def chunk(c, m):
+        z = _rng(seed, stream, c).standard_normal((m, 4))
         z /= np.linalg.norm(z, axis=1, keepdims=True)
-        out[lo:hi] = su2_from_quaternion(z)
-    return out
+        return su2_from_quaternion(z)
+
+    return _fill_chunks(np.empty((n, 2, 2), dtype=np.complex128), chunk)
 
 
 def _expm_i_hermitian(h: np.ndarray) -> np.ndarray:
@@ -142,26 +162,26 @@ def _expm_i_hermitian(h: np.ndarray) -> np.ndarray:
 
 
 def near_identity_su3(n: int, eps: float, seed: int, stream: int = 0) -> np.ndarray:
-    out = np.empty((n, 3, 3), dtype=np.complex128)
-    for c, lo, hi in _chunks(n):
-        coef = _rng(seed, stream, c).standard_normal((hi - lo, 8))
+    def chunk(c, m):
+        coef = _rng(seed, stream, c).standard_normal((m, 8))
         h = np.tensordot(coef, _GM, axes=(1, 0)) * 0.5
         u = _expm_i_hermitian(eps * h)
-        out[lo:hi] = _gram_schmidt_su3(u[:, 0], u[:, 1])
-    return out
+        return _gram_schmidt_su3(u[:, 0], u[:, 1])
+
+    return _fill_chunks(np.empty((n, 3, 3), dtype=np.complex128), chunk, threads=False)
 
 
 def near_identity_su2(n: int, eps: float, seed: int, stream: int = 0) -> np.ndarray:
     """exp(i*eps*c.sigma/2), c ~ N(0,1)^3 (closed form on the 3-sphere)."""
-    out = np.empty((n, 2, 2), dtype=np.complex128)
-    for c, lo, hi in _chunks(n):
-        v = _rng(seed, stream, c).standard_normal((hi - lo, 3)) * (0.5 * eps)
+    def chunk(c, m):
+        v = _rng(seed, stream, c).standard_normal((m, 3)) * (0.5 * eps)
         r = np.linalg.norm(v, axis=1)
-        q = np.empty((hi - lo, 4))
+        q = np.empty((m, 4))
         q[:, 0] = np.cos(r)
         q[:, 1:] = v * (np.sinc(r / np.pi))[:, None]
-        out[lo:hi] = su2_from_quaternion(q)
-    return out
+        return su2_from_quaternion(q)
+
+    return _fill_chunks(np.empty((n, 2, 2), dtype=np.complex128), chunk)
 
 
 def _shift_sites(field: np.ndarray, dims, mu: int, step: int) -> np.ndarray:

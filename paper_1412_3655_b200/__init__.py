@@ -24,6 +24,7 @@ CULGT_OK = 0
 ERRORS = {
     "CULGT_ERR_NULL": -1, "CULGT_ERR_DIMS": -2, "CULGT_ERR_DESC": -3, "CULGT_ERR_PARITY": -4,
     "CULGT_ERR_OMEGA": -5, "CULGT_ERR_ALIGN": -6, "CULGT_ERR_CUDA": -7, "CULGT_ERR_ARG": -8,
+    "CULGT_ERR_NCCL": -9,
 }
 FLOPS_PER_SITE = {3: 2304, 2: 278}   # fixed algorithmic counts, DESIGN.md "Measurement"
 
@@ -32,7 +33,7 @@ class CulgtError(RuntimeError):
     def __init__(self, status: int, where: str):
         self.status = status
         msg = lib().culgt_strerror(status).decode()
-        if status == ERRORS["CULGT_ERR_CUDA"]:
+        if status in (ERRORS["CULGT_ERR_CUDA"], ERRORS["CULGT_ERR_NCCL"]):
             msg += ": " + lib().culgt_last_cuda_error().decode()
         super().__init__(f"{where}: {msg} ({status})")
 
@@ -92,6 +93,34 @@ def lib() -> ctypes.CDLL:
     L.culgt_set_sweep_variant.argtypes = [ctypes.c_int]
     L.culgt_autotune_sweep.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_int, ctypes.POINTER(ctypes.c_int),
                                        ctypes.POINTER(ctypes.c_float), vp]
+    szp = ctypes.POINTER(ctypes.c_size_t)
+    ip = ctypes.POINTER(ctypes.c_int)
+    L.culgt_slab_lattice.argtypes = [latp, ctypes.c_int, latp]
+    for name in ("culgt_slab_links_bytes", "culgt_slab_halo_bytes"):
+        getattr(L, name).argtypes = [latp]
+        getattr(L, name).restype = ctypes.c_size_t
+    L.culgt_slab_halo_chunks.argtypes = [latp, ctypes.c_int, ctypes.c_int, szp, szp, ip]
+    L.culgt_slab_halo_peers.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ip, ip]
+    L.culgt_slab_pack.argtypes = [latp, vp, vp, vp]
+    L.culgt_slab_unpack.argtypes = [latp, vp, vp, vp]
+    L.culgt_slab_or_sweep.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, vp]
+    L.culgt_slab_or_sweep_window.argtypes = [latp, vp, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.c_int, vp]
+    L.culgt_slab_halo_copy.argtypes = [latp, vp, vp, ctypes.c_int, ctypes.c_int, vp]
+    L.culgt_slab_theta_F_sums.argtypes = [latp, vp, vp, vp, vp]
+    L.culgt_slab_theta_F_combine.argtypes = [latp, vp, ctypes.c_int, vp, vp, vp]
+    vpp = ctypes.POINTER(ctypes.c_void_p)
+    L.culgt_slab_exchange_all_local.argtypes = [latp, vpp, ctypes.c_int, vp]
+    L.culgt_slab_or_sweeps_local.argtypes = [latp, vpp, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int, vp]
+    L.culgt_slab_theta_F_local.argtypes = [latp, latp, vpp, ctypes.c_int, vp, vp, vp, vp, vp]
+    L.culgt_slab_comm_unique_id.argtypes = [vp]
+    L.culgt_slab_comm_create.argtypes = [vp, ctypes.c_int, ctypes.c_int, vpp]
+    L.culgt_slab_comm_destroy.argtypes = [vp]
+    L.culgt_slab_halo_exchange.argtypes = [vp, latp, vp, ctypes.c_int, ctypes.c_int, vp]
+    L.culgt_slab_exchange_all_nccl.argtypes = [vp, latp, vp, vp]
+    L.culgt_slab_or_sweeps_nccl.argtypes = [vp, latp, vp, ctypes.c_int, ctypes.c_double, vp, vp]
+    L.culgt_slab_theta_F_nccl.argtypes = [vp, latp, latp, vp, vp, vp, vp, vp, vp]
+    L.culgt_sweep_kernel_name.argtypes = [latp]
+    L.culgt_sweep_kernel_name.restype = ctypes.c_char_p
     L.culgt_strerror.argtypes = [ctypes.c_int]
     L.culgt_strerror.restype = ctypes.c_char_p
     L.culgt_last_cuda_error.restype = ctypes.c_char_p
@@ -374,6 +403,165 @@ def culgt_coulomb_fix(lat: Lattice, links, workspace, omega: float, theta_target
     return done.value, list(th), list(F)
 
 
+# ---- time-slab decomposition over several GPUs (include/culgt_b200.h, csrc/slab.cu) -----------------
+
+def culgt_slab_lattice(lat: Lattice, n_slabs: int) -> Lattice:
+    """The local lattice (dims[3] = N3 / n_slabs) of one of n_slabs time slabs."""
+    out = culgt_lattice()
+    _check(lib().culgt_slab_lattice(ctypes.byref(lat.c()), int(n_slabs), ctypes.byref(out)), "culgt_slab_lattice")
+    return Lattice(tuple(out.dims), out.group, out.precision, out.params)
+
+
+def culgt_slab_links_bytes(local: Lattice) -> int:
+    return lib().culgt_slab_links_bytes(ctypes.byref(local.c()))
+
+
+def culgt_slab_halo_bytes(local: Lattice) -> int:
+    return lib().culgt_slab_halo_bytes(ctypes.byref(local.c()))
+
+
+def culgt_slab_halo_chunks(local: Lattice, parity: int, which: int):
+    """(byte offsets, chunk_bytes) of one halo message: which = 0 ghost slice, 1 last slice (host only)."""
+    off = (ctypes.c_size_t * 9)()
+    nbytes = ctypes.c_size_t(0)
+    n = ctypes.c_int(0)
+    _check(lib().culgt_slab_halo_chunks(ctypes.byref(local.c()), int(parity), int(which), off, ctypes.byref(nbytes),
+                                        ctypes.byref(n)), "culgt_slab_halo_chunks")
+    return [int(off[j]) for j in range(n.value)], int(nbytes.value)
+
+
+def culgt_slab_halo_peers(rank: int, n_ranks: int, direction: int):
+    """(send_to, recv_from) of one halo message (host only)."""
+    a, b = ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().culgt_slab_halo_peers(int(rank), int(n_ranks), int(direction), ctypes.byref(a), ctypes.byref(b)),
+           "culgt_slab_halo_peers")
+    return a.value, b.value
+
+
+def alloc_slab_links(local: Lattice, device="cuda"):
+    import torch
+    n = culgt_slab_links_bytes(local)
+    if n == 0:
+        _check(culgt_validate(local), "alloc_slab_links")
+    return torch.empty(n // (local.precision // 8), dtype=local.torch_dtype, device=device)
+
+
+def _ptr_array(tensors):
+    return (ctypes.c_void_p * len(tensors))(*[_ptr(t) for t in tensors])
+
+
+def culgt_slab_pack(local: Lattice, canonical_slab, links_slab, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_pack(ctypes.byref(local.c()), _ptr(canonical_slab), _ptr(links_slab), _stream(stream)),
+           "culgt_slab_pack")
+
+
+def culgt_slab_unpack(local: Lattice, links_slab, canonical_slab, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_unpack(ctypes.byref(local.c()), _ptr(links_slab), _ptr(canonical_slab), _stream(stream)),
+           "culgt_slab_unpack")
+
+
+def culgt_slab_or_sweep(local: Lattice, links_slab, parity: int, omega: float, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_or_sweep(ctypes.byref(local.c()), _ptr(links_slab), int(parity), float(omega),
+                                     _stream(stream)), "culgt_slab_or_sweep")
+
+
+def culgt_slab_or_sweep_window(local: Lattice, links_slab, parity: int, omega: float, t_lo: int, t_hi: int,
+                               stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_or_sweep_window(ctypes.byref(local.c()), _ptr(links_slab), int(parity), float(omega),
+                                            int(t_lo), int(t_hi), _stream(stream)), "culgt_slab_or_sweep_window")
+
+
+def culgt_slab_halo_copy(local: Lattice, src_links, dst_links, parity: int, direction: int, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_halo_copy(ctypes.byref(local.c()), _ptr(src_links), _ptr(dst_links), int(parity),
+                                      int(direction), _stream(stream)), "culgt_slab_halo_copy")
+
+
+def culgt_slab_theta_F_sums(local: Lattice, links_slab, workspace, sums2_dev, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_theta_F_sums(ctypes.byref(local.c()), _ptr(links_slab), _ptr(workspace), _ptr(sums2_dev),
+                                         _stream(stream)), "culgt_slab_theta_F_sums")
+
+
+def culgt_slab_theta_F_combine(lat: Lattice, sums_dev, n_slabs: int, theta_dev, F_dev, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_theta_F_combine(ctypes.byref(lat.c()), _ptr(sums_dev), int(n_slabs), _ptr(theta_dev),
+                                            _ptr(F_dev), _stream(stream)), "culgt_slab_theta_F_combine")
+
+
+def culgt_slab_exchange_all_local(local: Lattice, links_slabs, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_exchange_all_local(ctypes.byref(local.c()), _ptr_array(links_slabs), len(links_slabs),
+                                               _stream(stream)), "culgt_slab_exchange_all_local")
+
+
+def culgt_slab_or_sweeps_local(local: Lattice, links_slabs, n_sweeps: int, omega: float, boundary_first: bool = False,
+                               stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_or_sweeps_local(ctypes.byref(local.c()), _ptr_array(links_slabs), len(links_slabs),
+                                            int(n_sweeps), float(omega), int(bool(boundary_first)), _stream(stream)),
+           "culgt_slab_or_sweeps_local")
+
+
+def culgt_slab_theta_F_local(lat: Lattice, local: Lattice, links_slabs, workspace, sums_dev, theta_dev, F_dev,
+                             stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_theta_F_local(ctypes.byref(lat.c()), ctypes.byref(local.c()), _ptr_array(links_slabs),
+                                          len(links_slabs), _ptr(workspace), _ptr(sums_dev), _ptr(theta_dev),
+                                          _ptr(F_dev), _stream(stream)), "culgt_slab_theta_F_local")
+
+
+def culgt_slab_comm_unique_id() -> bytes:
+    buf = ctypes.create_string_buffer(128)
+    _check(lib().culgt_slab_comm_unique_id(buf), "culgt_slab_comm_unique_id")
+    return buf.raw
+
+
+def culgt_slab_comm_create(unique_id: bytes, rank: int, n_ranks: int) -> int:
+    """Collective over the n_ranks ranks; returns the opaque communicator handle."""
+    _require_cuda()
+    comm = ctypes.c_void_p(0)
+    _check(lib().culgt_slab_comm_create(ctypes.create_string_buffer(unique_id, 128), int(rank), int(n_ranks),
+                                        ctypes.byref(comm)), "culgt_slab_comm_create")
+    return comm.value
+
+
+def culgt_slab_comm_destroy(comm: int) -> None:
+    _check(lib().culgt_slab_comm_destroy(comm), "culgt_slab_comm_destroy")
+
+
+def culgt_slab_halo_exchange(comm: int, local: Lattice, links_slab, parity: int, direction: int, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_halo_exchange(comm, ctypes.byref(local.c()), _ptr(links_slab), int(parity), int(direction),
+                                          _stream(stream)), "culgt_slab_halo_exchange")
+
+
+def culgt_slab_exchange_all_nccl(comm: int, local: Lattice, links_slab, stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_exchange_all_nccl(comm, ctypes.byref(local.c()), _ptr(links_slab), _stream(stream)),
+           "culgt_slab_exchange_all_nccl")
+
+
+def culgt_slab_or_sweeps_nccl(comm: int, local: Lattice, links_slab, n_sweeps: int, omega: float, comm_stream=None,
+                              stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_or_sweeps_nccl(comm, ctypes.byref(local.c()), _ptr(links_slab), int(n_sweeps), float(omega),
+                                           None if comm_stream is None else _stream(comm_stream), _stream(stream)),
+           "culgt_slab_or_sweeps_nccl")
+
+
+def culgt_slab_theta_F_nccl(comm: int, lat: Lattice, local: Lattice, links_slab, workspace, sums_dev, theta_dev, F_dev,
+                            stream=None) -> None:
+    _require_cuda()
+    _check(lib().culgt_slab_theta_F_nccl(comm, ctypes.byref(lat.c()), ctypes.byref(local.c()), _ptr(links_slab),
+                                         _ptr(workspace), _ptr(sums_dev), _ptr(theta_dev), _ptr(F_dev),
+                                         _stream(stream)), "culgt_slab_theta_F_nccl")
+
+
 def culgt_set_sweep_variant(variant: int) -> None:
     _check(lib().culgt_set_sweep_variant(int(variant)), "culgt_set_sweep_variant")
 
@@ -400,6 +588,10 @@ def culgt_fused_schedule(n_slices: int, lag: int, direction: int):
     buf = (ctypes.c_uint * (2 * int(n_slices)))()
     _check(lib().culgt_fused_schedule(int(n_slices), int(lag), int(direction), buf), "culgt_fused_schedule")
     return [(w >> 31, w & 0x7FFFFFFF) for w in buf]
+
+
+def culgt_sweep_kernel_name(lat: Lattice) -> str:
+    return lib().culgt_sweep_kernel_name(ctypes.byref(lat.c())).decode()
 
 
 def culgt_measure_build() -> bool:

@@ -19,6 +19,11 @@ namespace {
 thread_local char g_cuda_err[256] = "";
 thread_local int g_variant = 0;
 
+int nccl_fail(int code) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "NCCL: %s", slab_nccl_error(code));
+  return CULGT_ERR_NCCL;
+}
+
 int cuda_fail(cudaError_t e) {
   snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
   return CULGT_ERR_CUDA;
@@ -48,6 +53,15 @@ int describe(const culgt_lattice* lat, LatticeDesc* d) {
 }
 
 bool misaligned(const void* p) { return ((uintptr_t)p & 15u) != 0; }
+
+// descriptor of one time slab: the local lattice with a ghost slice behind every plane (slab.cu)
+int describe_slab(const culgt_lattice* local, LatticeDesc* d) {
+  const int rc = describe(local, d);
+  if (rc != CULGT_OK) return rc;
+  if ((long long)d->geom.vh + d->geom.stride[3] >= (1ll << 30)) return CULGT_ERR_DIMS;
+  make_slab_geom(&d->geom);
+  return CULGT_OK;
+}
 
 }  // namespace
 
@@ -512,6 +526,331 @@ int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, do
   return CULGT_OK;
 }
 
+
+// ---- time-slab decomposition over several GPUs (csrc/slab.cu) -------------
+
+int culgt_slab_lattice(const culgt_lattice* global, int n_slabs, culgt_lattice* local) {
+  LatticeDesc d;
+  int rc = describe(global, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!local) return CULGT_ERR_NULL;
+  if (n_slabs < 1 || global->dims[3] % n_slabs != 0) return CULGT_ERR_ARG;
+  const int t = global->dims[3] / n_slabs;
+  if (t < 2 || (t & 1)) return CULGT_ERR_ARG;          // an odd slab would flip the parity of its sites
+  *local = *global;
+  local->dims[3] = t;
+  return CULGT_OK;
+}
+
+size_t culgt_slab_links_bytes(const culgt_lattice* local) {
+  LatticeDesc d;
+  if (describe_slab(local, &d) != CULGT_OK) return 0;
+  return (size_t)8 * (size_t)slab_vectors_per_link(d) * (size_t)d.geom.pitch * 16;
+}
+
+size_t culgt_slab_halo_bytes(const culgt_lattice* local) {
+  LatticeDesc d;
+  if (describe_slab(local, &d) != CULGT_OK) return 0;
+  return (size_t)slab_vectors_per_link(d) * (size_t)d.geom.stride[3] * 16;
+}
+
+int culgt_slab_halo_chunks(const culgt_lattice* local, int parity, int which, size_t* offsets, size_t* chunk_bytes,
+                           int* n_chunks) {
+  LatticeDesc d;
+  int rc = describe_slab(local, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!offsets || !chunk_bytes || !n_chunks) return CULGT_ERR_NULL;
+  if (parity != 0 && parity != 1) return CULGT_ERR_PARITY;
+  if (which != 0 && which != 1) return CULGT_ERR_ARG;
+  slab_halo_chunks(d, parity, which, offsets, chunk_bytes, n_chunks);
+  return CULGT_OK;
+}
+
+int culgt_slab_halo_peers(int rank, int n_ranks, int direction, int* send_to, int* recv_from) {
+  if (!send_to || !recv_from) return CULGT_ERR_NULL;
+  if (n_ranks < 1 || rank < 0 || rank >= n_ranks || (direction != 0 && direction != 1)) return CULGT_ERR_ARG;
+  slab_halo_peers(rank, n_ranks, direction, send_to, recv_from);
+  return CULGT_OK;
+}
+
+int culgt_slab_pack(const culgt_lattice* local, const void* canonical_slab, void* links_slab, void* stream) {
+  LatticeDesc d;
+  int rc = describe_slab(local, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!canonical_slab || !links_slab) return CULGT_ERR_NULL;
+  if (misaligned(canonical_slab) || misaligned(links_slab)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_pack(d, canonical_slab, links_slab, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_slab_unpack(const culgt_lattice* local, const void* links_slab, void* canonical_slab, void* stream) {
+  LatticeDesc d;
+  int rc = describe_slab(local, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!canonical_slab || !links_slab) return CULGT_ERR_NULL;
+  if (misaligned(canonical_slab) || misaligned(links_slab)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_unpack(d, links_slab, canonical_slab, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+static int check_slab_sweep(const culgt_lattice* local, const void* links, int parity, double omega, LatticeDesc* d) {
+  int rc = describe_slab(local, d);
+  if (rc != CULGT_OK) return rc;
+  if (!links) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if (parity != 0 && parity != 1) return CULGT_ERR_PARITY;
+  return check_omega(omega);
+}
+
+int culgt_slab_or_sweep(const culgt_lattice* local, void* links_slab, int parity, double omega, void* stream) {
+  LatticeDesc d;
+  int rc = check_slab_sweep(local, links_slab, parity, omega, &d);
+  if (rc != CULGT_OK) return rc;
+  cudaError_t e = launch_or_sweep(d, links_slab, parity, omega, g_variant, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_slab_or_sweep_window(const culgt_lattice* local, void* links_slab, int parity, double omega, int t_lo,
+                               int t_hi, void* stream) {
+  LatticeDesc d;
+  int rc = check_slab_sweep(local, links_slab, parity, omega, &d);
+  if (rc != CULGT_OK) return rc;
+  if (t_lo < 0 || t_hi > local->dims[3] || t_lo > t_hi) return CULGT_ERR_ARG;
+  cudaError_t e = launch_or_sweep_window(d, links_slab, parity, omega, t_lo, t_hi, (cudaStream_t)stream);
+  if (e == cudaErrorNotSupported) return CULGT_ERR_DESC;      // SU(2), or no whole site blocks per time-slice
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_slab_halo_copy(const culgt_lattice* local, const void* src_links, void* dst_links, int parity, int direction,
+                         void* stream) {
+  LatticeDesc d;
+  int rc = describe_slab(local, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!src_links || !dst_links) return CULGT_ERR_NULL;
+  if (misaligned(src_links) || misaligned(dst_links)) return CULGT_ERR_ALIGN;
+  if (parity != 0 && parity != 1) return CULGT_ERR_PARITY;
+  if (direction != 0 && direction != 1) return CULGT_ERR_ARG;
+  cudaError_t e = slab_halo_copy(d, src_links, dst_links, parity, direction, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_slab_theta_F_sums(const culgt_lattice* local, const void* links_slab, void* workspace, double* sums2_dev,
+                            void* stream) {
+  LatticeDesc d;
+  int rc = describe_slab(local, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links_slab || !workspace || !sums2_dev) return CULGT_ERR_NULL;
+  if (misaligned(links_slab) || misaligned(workspace)) return CULGT_ERR_ALIGN;
+  cudaError_t e = launch_theta_functional_sums(d, links_slab, (double*)workspace, sums2_dev, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_slab_theta_F_combine(const culgt_lattice* global, const double* sums_dev, int n_slabs, double* theta_dev,
+                               double* F_dev, void* stream) {
+  LatticeDesc d;
+  int rc = describe(global, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!sums_dev || !theta_dev || !F_dev) return CULGT_ERR_NULL;
+  if (n_slabs < 1) return CULGT_ERR_ARG;
+  cudaError_t e = slab_theta_F_combine(d, sums_dev, n_slabs, theta_dev, F_dev, (cudaStream_t)stream);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+// One half-sweep of parity p on one slab, boundary slices first when `boundary_first` (the schedule that
+// lets the halo messages travel while the interior is swept): slice 0 writes the ghost slice of parity
+// 1-p, slice T-1 the slab's own t-links of parity p in its last slice; the interior touches neither.
+static cudaError_t slab_half_sweep(const LatticeDesc& d, void* links, int parity, double omega, bool boundary_first,
+                                   cudaStream_t st, cudaEvent_t boundary_done) {
+  const int T = d.geom.n[3];
+  cudaError_t e = cudaErrorNotSupported;
+  if (boundary_first) {
+    e = launch_or_sweep_window(d, links, parity, omega, 0, 1, st);
+    if (e == cudaSuccess) e = launch_or_sweep_window(d, links, parity, omega, T - 1, T, st);
+    if (e == cudaSuccess && boundary_done) e = cudaEventRecord(boundary_done, st);
+    if (e == cudaSuccess) e = launch_or_sweep_window(d, links, parity, omega, 1, T - 1, st);
+  }
+  if (e == cudaErrorNotSupported) {             // no whole site blocks per slice (or SU(2)): one launch
+    e = launch_or_sweep(d, links, parity, omega, g_variant, st);
+    if (e == cudaSuccess && boundary_done) e = cudaEventRecord(boundary_done, st);
+  }
+  return e;
+}
+
+int culgt_slab_exchange_all_local(const culgt_lattice* local, void* const* links_slabs, int n_slabs, void* stream) {
+  LatticeDesc d;
+  int rc = describe_slab(local, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links_slabs) return CULGT_ERR_NULL;
+  if (n_slabs < 1) return CULGT_ERR_ARG;
+  for (int k = 0; k < n_slabs; ++k)
+    if (!links_slabs[k]) return CULGT_ERR_NULL;
+  for (int k = 0; k < n_slabs; ++k)
+    for (int parity = 0; parity < 2; ++parity) {
+      cudaError_t e = slab_halo_copy(d, links_slabs[k], links_slabs[(k + 1) % n_slabs], parity, 0, (cudaStream_t)stream);
+      if (e != cudaSuccess) return cuda_fail(e);
+    }
+  return CULGT_OK;
+}
+
+int culgt_slab_or_sweeps_local(const culgt_lattice* local, void* const* links_slabs, int n_slabs, int n_sweeps,
+                               double omega, int boundary_first, void* stream) {
+  LatticeDesc d;
+  int rc = describe_slab(local, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links_slabs) return CULGT_ERR_NULL;
+  if (n_slabs < 1 || n_sweeps < 0) return CULGT_ERR_ARG;
+  for (int k = 0; k < n_slabs; ++k) {
+    if (!links_slabs[k]) return CULGT_ERR_NULL;
+    if (misaligned(links_slabs[k])) return CULGT_ERR_ALIGN;
+  }
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e;
+  for (int i = 0; i < n_sweeps; ++i)
+    for (int p = 0; p < 2; ++p) {
+      for (int k = 0; k < n_slabs; ++k)
+        if ((e = slab_half_sweep(d, links_slabs[k], p, omega, boundary_first != 0, st, nullptr)) != cudaSuccess) return cuda_fail(e);
+      for (int k = 0; k < n_slabs; ++k) {
+        const int prev = (k + n_slabs - 1) % n_slabs, next = (k + 1) % n_slabs;
+        // the updated U_t(x - t_hat) of slab k's first slice go BACK to their owner ...
+        if ((e = slab_halo_copy(d, links_slabs[k], links_slabs[prev], 1 - p, 1, st)) != cudaSuccess) return cuda_fail(e);
+        // ... and slab k's own updated t-links of its last slice go FORWARD for the other parity's half-sweep
+        if ((e = slab_halo_copy(d, links_slabs[k], links_slabs[next], p, 0, st)) != cudaSuccess) return cuda_fail(e);
+      }
+    }
+  return CULGT_OK;
+}
+
+int culgt_slab_theta_F_local(const culgt_lattice* global, const culgt_lattice* local, void* const* links_slabs,
+                             int n_slabs, void* workspace, double* sums_dev, double* theta_dev, double* F_dev,
+                             void* stream) {
+  LatticeDesc dg, d;
+  int rc = describe(global, &dg);
+  if (rc != CULGT_OK) return rc;
+  if ((rc = describe_slab(local, &d)) != CULGT_OK) return rc;
+  if (!links_slabs || !workspace || !sums_dev || !theta_dev || !F_dev) return CULGT_ERR_NULL;
+  if (n_slabs < 1 || (long long)n_slabs * local->dims[3] != global->dims[3]) return CULGT_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  for (int k = 0; k < n_slabs; ++k) {
+    if (!links_slabs[k]) return CULGT_ERR_NULL;
+    cudaError_t e = launch_theta_functional_sums(d, links_slabs[k], (double*)workspace, sums_dev + 2 * k, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+  }
+  cudaError_t e = slab_theta_F_combine(dg, sums_dev, n_slabs, theta_dev, F_dev, st);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+// ---- one slab per rank, NCCL over NVLink ---------------------------------------------------------------------
+
+int culgt_slab_comm_unique_id(void* id128_host) {
+  if (!id128_host) return CULGT_ERR_NULL;
+  const int r = slab_comm_id(id128_host);
+  return r == 0 ? CULGT_OK : nccl_fail(r);
+}
+
+int culgt_slab_comm_create(const void* id128_host, int rank, int n_ranks, void** comm_out) {
+  if (!id128_host || !comm_out) return CULGT_ERR_NULL;
+  if (n_ranks < 1 || rank < 0 || rank >= n_ranks) return CULGT_ERR_ARG;
+  const int r = slab_comm_create(id128_host, rank, n_ranks, comm_out);
+  return r == 0 ? CULGT_OK : nccl_fail(r);
+}
+
+int culgt_slab_comm_destroy(void* comm) {
+  const int r = slab_comm_destroy(comm);
+  return r == 0 ? CULGT_OK : nccl_fail(r);
+}
+
+int culgt_slab_halo_exchange(void* comm, const culgt_lattice* local, void* links_slab, int parity, int direction,
+                             void* stream) {
+  LatticeDesc d;
+  int rc = describe_slab(local, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!comm || !links_slab) return CULGT_ERR_NULL;
+  if (misaligned(links_slab)) return CULGT_ERR_ALIGN;
+  if (parity != 0 && parity != 1) return CULGT_ERR_PARITY;
+  if (direction != 0 && direction != 1) return CULGT_ERR_ARG;
+  const int r = slab_halo_exchange(comm, d, links_slab, parity, direction, (cudaStream_t)stream);
+  return r == 0 ? CULGT_OK : nccl_fail(r);
+}
+
+int culgt_slab_or_sweeps_nccl(void* comm, const culgt_lattice* local, void* links_slab, int n_sweeps, double omega,
+                              void* comm_stream, void* stream) {
+  LatticeDesc d;
+  int rc = describe_slab(local, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!comm || !links_slab) return CULGT_ERR_NULL;
+  if (misaligned(links_slab)) return CULGT_ERR_ALIGN;
+  if (n_sweeps < 0) return CULGT_ERR_ARG;
+  if ((rc = check_omega(omega)) != CULGT_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream, cst = (cudaStream_t)comm_stream;
+  const bool overlap = comm_stream != nullptr && comm_stream != stream;
+  cudaEvent_t boundary_done = nullptr, halo_done = nullptr;
+  cudaError_t e = cudaSuccess;
+  if (overlap) {
+    if ((e = cudaEventCreateWithFlags(&boundary_done, cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaEventCreateWithFlags(&halo_done, cudaEventDisableTiming)) != cudaSuccess) {
+      cudaEventDestroy(boundary_done);
+      return cuda_fail(e);
+    }
+  }
+  int nr = 0;
+  for (int i = 0; i < n_sweeps && e == cudaSuccess && nr == 0; ++i)
+    for (int p = 0; p < 2 && e == cudaSuccess && nr == 0; ++p) {
+      if (!overlap) {
+        e = slab_half_sweep(d, links_slab, p, omega, false, st, nullptr);
+        if (e == cudaSuccess) nr = slab_halo_exchange(comm, d, links_slab, 1 - p, 1, st);
+        if (e == cudaSuccess && nr == 0) nr = slab_halo_exchange(comm, d, links_slab, p, 0, st);
+      } else {
+        // boundary slices, then the two messages on the communication stream while the interior is swept
+        e = slab_half_sweep(d, links_slab, p, omega, true, st, boundary_done);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(cst, boundary_done, 0);
+        if (e == cudaSuccess) nr = slab_halo_exchange(comm, d, links_slab, 1 - p, 1, cst);
+        if (e == cudaSuccess && nr == 0) nr = slab_halo_exchange(comm, d, links_slab, p, 0, cst);
+        if (e == cudaSuccess && nr == 0) e = cudaEventRecord(halo_done, cst);
+        if (e == cudaSuccess && nr == 0) e = cudaStreamWaitEvent(st, halo_done, 0);   // the next half-sweep needs both
+      }
+    }
+  if (overlap) {
+    cudaEventDestroy(boundary_done);
+    cudaEventDestroy(halo_done);
+  }
+  if (e != cudaSuccess) return cuda_fail(e);
+  return nr == 0 ? CULGT_OK : nccl_fail(nr);
+}
+
+int culgt_slab_theta_F_nccl(void* comm, const culgt_lattice* global, const culgt_lattice* local, const void* links_slab,
+                            void* workspace, double* sums_dev, double* theta_dev, double* F_dev, void* stream) {
+  LatticeDesc dg, d;
+  int rc = describe(global, &dg);
+  if (rc != CULGT_OK) return rc;
+  if ((rc = describe_slab(local, &d)) != CULGT_OK) return rc;
+  if (!comm || !links_slab || !workspace || !sums_dev || !theta_dev || !F_dev) return CULGT_ERR_NULL;
+  int rank = 0, n_ranks = 1;
+  slab_comm_info(comm, &rank, &n_ranks);
+  if ((long long)n_ranks * local->dims[3] != global->dims[3]) return CULGT_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  // my two raw sums behind the gathered ones, then all ranks' pairs in rank order on every rank
+  double* mine = sums_dev + 2 * n_ranks;
+  cudaError_t e = launch_theta_functional_sums(d, links_slab, (double*)workspace, mine, st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  const int r = slab_allgather_sums(comm, mine, sums_dev, st);
+  if (r != 0) return nccl_fail(r);
+  e = slab_theta_F_combine(dg, sums_dev, n_ranks, theta_dev, F_dev, st);
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
+int culgt_slab_exchange_all_nccl(void* comm, const culgt_lattice* local, void* links_slab, void* stream) {
+  LatticeDesc d;
+  int rc = describe_slab(local, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!comm || !links_slab) return CULGT_ERR_NULL;
+  for (int parity = 0; parity < 2; ++parity) {
+    const int r = slab_halo_exchange(comm, d, links_slab, parity, 0, (cudaStream_t)stream);
+    if (r != 0) return nccl_fail(r);
+  }
+  return CULGT_OK;
+}
+
 // Run-time autotuner (the paper's selection of the fastest kernel set-up per GPU at run time,
 // P:L89 (d)): times every result-equivalent sweep schedule built for this storage format
 // on the caller's field and makes the fastest one the calling thread's choice.
@@ -563,6 +902,11 @@ int culgt_set_sweep_variant(int variant) {
   return CULGT_OK;
 }
 int culgt_get_sweep_variant(void) { return g_variant; }
+const char* culgt_sweep_kernel_name(const culgt_lattice* lat) {
+  LatticeDesc d;
+  if (describe(lat, &d) != CULGT_OK) return "";
+  return sweep_kernel_name(d);
+}
 int culgt_measure_build(void) {
 #ifdef CULGT_MEASURE
   return 1;
@@ -607,6 +951,7 @@ const char* culgt_strerror(int status) {
     case CULGT_ERR_ALIGN: return "device pointer not 16-byte aligned";
     case CULGT_ERR_CUDA: return "CUDA error (see culgt_last_cuda_error)";
     case CULGT_ERR_ARG: return "argument out of range";
+    case CULGT_ERR_NCCL: return "NCCL error (see culgt_last_cuda_error)";
     default: return "unknown status";
   }
 }

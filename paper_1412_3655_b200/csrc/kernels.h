@@ -79,6 +79,7 @@ static_assert(sizeof(FusedCtl) % 8 == 0, "FusedCtl is addressed in doubles");
 // coulomb = true: Coulomb-gauge half-sweep (K from the spatial links; production mapping only).
 // stop_flag (device, may be null): the launch does nothing if *stop_flag != 0 when it starts.
 bool sweep_variant_known(int variant);
+const char* sweep_kernel_name(const LatticeDesc& d);
 cudaError_t launch_or_sweep(const LatticeDesc& d, void* links, int parity, double omega,
                             int variant, cudaStream_t st, bool coulomb = false, const int* stop_flag = nullptr);
 cudaError_t launch_or_sweep_staged(const LatticeDesc& d, void* links, int parity, double omega,
@@ -139,5 +140,25 @@ cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, dou
 cudaError_t launch_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
                                             double* out_theta_t, double* out_F_t, cudaStream_t st);
 cudaError_t launch_gauge_transform(const LatticeDesc& d, void* links, const void* g, cudaStream_t st);
+
+// ---- time-slab decomposition (slab.cu) ------------------------------------------------------------------
+void make_slab_geom(Geom* g);     // pitch and wrap3 of a slab with a ghost slice
+int slab_vectors_per_link(const LatticeDesc& d);
+void slab_halo_chunks(const LatticeDesc& d, int parity, int which, size_t* offsets, size_t* chunk_bytes, int* n_chunks);
+cudaError_t slab_halo_copy(const LatticeDesc& d, const void* src, void* dst, int parity, int direction, cudaStream_t st);
+cudaError_t slab_theta_F_combine(const LatticeDesc& global, const double* sums, int n_slabs, double* theta, double* F,
+                                 cudaStream_t st);
+// fused theta + F of one slab as RAW sums (sum_x tr[Delta Delta^dagger], sum_{x,mu} Re tr U): out2[0], out2[1]
+cudaError_t launch_theta_functional_sums(const LatticeDesc& slab, const void* links, double* workspace, double* out2,
+                                         cudaStream_t st);
+void slab_halo_peers(int rank, int n_ranks, int direction, int* send_to, int* recv_from);
+bool slab_nccl_available();
+const char* slab_nccl_error(int code);
+int slab_comm_id(void* id128);
+int slab_comm_create(const void* id128, int rank, int n_ranks, void** out);
+int slab_comm_destroy(void* comm);
+void slab_comm_info(void* comm, int* rank, int* n_ranks);
+int slab_halo_exchange(void* comm, const LatticeDesc& d, void* links, int parity, int direction, cudaStream_t st);
+int slab_allgather_sums(void* comm, const double* sums2, double* all, cudaStream_t st);
 
 }  // namespace culgt

@@ -160,6 +160,17 @@ static cudaError_t launch_format(const LatticeDesc& d, void* links, int parity, 
   return launch_staged<Storage<double, 3, 18>, 64, 3, OPT>(links, g, parity, pw, reverse_odd, stop_flag, st, win_lo, win_n, win_reverse);
 }
 
+// Name of the kernel instantiation that variant 0 launches for this lattice (what a committed ncu
+// capture must have been taken on to describe it: bench.py, profiles/roofline_traffic.csv).  The
+// numbers are the ones launch_format uses.
+const char* sweep_kernel_name(const LatticeDesc& d) {
+  if (d.group == 2) return d.precision == 32 ? "or_sweep_su2_kernel<f32-4,128,pdl>" : "or_sweep_su2_kernel<f64-4,128,pdl>";
+  if (d.precision == 32 && d.params == 12) return "or_sweep_su3_staged_kernel<f32-12,128x4,pdl+l2hint,r2>";
+  if (d.precision == 32) return "or_sweep_su3_staged_kernel<f32-18,64x5,pdl+l2hint,r2>";
+  if (d.params == 12) return "or_sweep_su3_staged_kernel<f64-12,64x4,pdl+l2hint,r2>";
+  return "or_sweep_su3_staged_kernel<f64-18,64x3,pdl+l2hint,r2>";
+}
+
 // Product variants of the SU(3) half-sweep: all the same per-site arithmetic (bit-identical
 // results), different launch options.  0 / 20 production; 24 without the reversed odd-parity
 // traversal; 33 without programmatic dependent launch; 34 without L2 hints.

@@ -321,6 +321,22 @@ cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, dou
   CULGT_DISPATCH(run_theta_functional, d, links, workspace, out_theta, out_F, st, fix)
 }
 
+// Raw sums of one time slab (scale 1): the caller combines the slabs (slab.cu).
+template <typename S>
+static cudaError_t run_theta_functional_sums(const LatticeDesc& d, const void* links, double* ws, double* out2,
+                                             cudaStream_t st) {
+  int nblk = 0;
+  cudaError_t e = launch_theta_pass<S, false>(d.geom.vh, 1, links, d.geom, ws, nullptr, st, &nblk);
+  if (e != cudaSuccess) return e;
+  final_sum_landau_kernel<kReduceBlock><<<1, kReduceBlock, 0, st>>>(ws, nblk, 1.0, 1.0, out2, out2 + 1, nullptr, 0.0, 0);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_theta_functional_sums(const LatticeDesc& d, const void* links, double* workspace, double* out2,
+                                         cudaStream_t st) {
+  CULGT_DISPATCH(run_theta_functional_sums, d, links, workspace, out2, st)
+}
+
 cudaError_t launch_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
                                             double* out_theta_t, double* out_F_t, cudaStream_t st) {
   CULGT_DISPATCH(run_coulomb_theta_functional, d, links, workspace, out_theta_t, out_F_t, st)

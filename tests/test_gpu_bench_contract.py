@@ -21,7 +21,8 @@ def run(*args):
 
 
 def test_our_arm_json_line():
-    d = run("--steps", "6", "--warmup", "3", "--check-every", "3", "--workload", "cfg2")
+    d = run("--steps", "6", "--warmup", "3", "--check-every", "3", "--workload", "cfg2", "--extra-workloads", "cfg1",
+            "--extra-steps", "4")
     assert d["metric"] == "su3_landau_or_site_updates_per_s" and d["unit"] == "site-updates/s"
     assert d["n_gpus"] == 1 and d["steps"] == 6 and d["warmup"] >= 3 and d["higher_is_better"] is True
     assert d["scaling"] == "weak" and d["vs_baseline"] is None and d["dtype"] == "f32" and d["data"] == "synthetic"
@@ -38,6 +39,21 @@ def test_our_arm_json_line():
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["unit"] == d["unit"] and c["sample"]
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    assert d["clocks"]["samples"] >= 3 and d["clocks"]["window_ms"] >= 50     # never a single NVML sample
+    # the DRAM-side figures come from a committed ncu capture stamped with the kernel it was taken on
+    assert r["kernel"].startswith("or_sweep_su3_staged_kernel<f32-12") and "traffic_capture" in r
+    assert r["traffic"] is None and "stale" in r["traffic_capture"]           # no capture exists for cfg2
+    # the other kernels of the path, the other workloads and the driver loop ride on the same line
+    for k in ("theta_F", "pack", "unpack", "gauge_transform"):
+        assert d["kernels"][k]["us"] > 0 and 0 < d["kernels"][k]["frac"] < 2
+    (x,) = d["extra_workloads"]
+    assert x["workload"].startswith("cfg1") and x["value"] > 0 and x["launch_us"] > 0 and x["steps"] == 4
+    assert x["roofline"]["frac"] == x["roofline"]["achieved"] / x["roofline"]["peak"] and "clocks" in x
+    for name in ("cfg0", "cfg1", "cfg2"):
+        loop = d["driver_loop"][name]
+        a, b = loop["host_sync_every_check"], loop["device_stop_flag"]
+        assert a["sweeps"] == b["sweeps"] and a["wall_ms"] > 0 and b["wall_ms"] > 0
+        assert b["theta"] == a["theta"]                                       # the same loop, bit for bit
     assert d["value"] > 20 * c["value"]               # the GPU path, not a CPU fallback
 
 

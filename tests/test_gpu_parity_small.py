@@ -203,7 +203,7 @@ def test_autotuner_picks_a_result_equivalent_mapping():
         scratch = GpuField(dims, 3, precision, params, u)
         try:
             v, us = culgt.culgt_autotune_sweep(scratch.lat, scratch.links, scratch.ws, 1.7, 2)
-            assert v in variants_for(precision, params) and us > 0
+            assert v in variants_for(precision, params) + ([41, 42, 43, 44, 60] if culgt.culgt_measure_build() else []) and us > 0
             assert culgt.culgt_get_sweep_variant() == v
             ref = storage_input(u, precision, params)
             oracle.full_sweep(dims, ref, 1.7)
