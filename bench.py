@@ -28,8 +28,11 @@ extra_workloads   the second half of BASELINE.json configs[3] (fp64 18-parameter
 cpu_baseline the oracle (oracle/, as it stands) timed on this host's cores on a bounded sample.
 --impl reference  times the oracle itself (rank 0 only), same metric / config / unit.
 
-Multi-GPU: the path has no exchange step ("replicas only"): each rank fixes its own
+Multi-GPU: by default replicas only (BASELINE.json north_star): each rank fixes its own
 independent configuration; value = total site-updates / max-over-ranks time; scaling "weak".
+--sharded instead cuts ONE lattice (default cfg4_fp64, 64^4 fp64-18, 9.7 GB) into --gpus time slabs,
+one per rank, with one halo message each way per boundary and half-sweep over NCCL and theta/F from
+all-gathered per-slab sums; value = V * steps / max-over-ranks time; scaling "strong".
 """
 from __future__ import annotations
 
@@ -59,7 +62,11 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=500)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg3_fp32", choices=sorted(li.CONFIGS))
+    ap.add_argument("--workload", default=None, choices=sorted(li.CONFIGS),
+                    help="default: cfg3_fp32 (BASELINE.json configs[3], the headline); with --sharded: cfg4_fp64")
+    ap.add_argument("--sharded", action="store_true",
+                    help="strong scaling: ONE lattice cut into --gpus time slabs, one per rank, halo messages over "
+                         "NCCL (include/culgt_b200.h 'Time-slab decomposition'); default is replicas (north_star)")
     ap.add_argument("--check-every", type=int, default=50)
     ap.add_argument("--variant", type=int, default=0, help="sweep kernel variant (0 = default)")
     ap.add_argument("--gauge", default="landau", choices=["landau", "coulomb"],
@@ -78,7 +85,10 @@ def parse_args():
     ap.add_argument("--extra-workloads", default=None,
                     help="comma-separated workloads for the extra_workloads block (default: cfg3_fp64,cfg4_fp32,"
                          "cfg4_fp64 when the main workload is cfg3_fp32, none otherwise)")
-    return ap.parse_args()
+    args = ap.parse_args()
+    if args.workload is None:
+        args.workload = "cfg4_fp64" if args.sharded else "cfg3_fp32"
+    return args
 
 
 def measured_peak():
@@ -416,10 +426,124 @@ def driver_loop_times(culgt, torch, rank):
     return out
 
 
+def run_sharded(args):
+    """--sharded: the time-slab decomposition, one slab per rank (csrc/slab.cu)."""
+    import torch
+    import torch.distributed as dist
+    import paper_1412_3655_b200 as culgt
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = li.CONFIGS[args.workload]
+    dims, omega = cfg["dims"], cfg["omega"]
+    V = li.volume(dims)
+    lat = culgt.Lattice(tuple(dims), cfg["group"], cfg["precision"], cfg["params"])
+    local = culgt.culgt_slab_lattice(lat, world)          # raises unless N3 / world is an even number of slices
+    T = local.dims[3]
+    # my slab of the ONE seeded configuration, made without making the rest
+    u = li.make_config(dims, cfg["group"], cfg["kind"], cfg["seed"], eps=cfg["eps"], scramble=cfg["scramble"],
+                       t_range=(rank * T, (rank + 1) * T))
+    np_dt = np.float32 if cfg["precision"] == 32 else np.float64
+    host = torch.from_numpy(li.to_real(u, np_dt)).pin_memory()
+    del u
+    can_dev = torch.empty_like(host, device="cuda")
+    links = culgt.alloc_slab_links(local)
+    ws = culgt.alloc_workspace(local)
+    sums = torch.zeros(2 * world + 2, dtype=torch.float64, device="cuda")
+    scal = torch.zeros(2, dtype=torch.float64, device="cuda")
+    uid = [culgt.culgt_slab_comm_unique_id() if rank == 0 else None]
+    if world > 1:
+        dist.broadcast_object_list(uid, src=0)
+    comm = culgt.culgt_slab_comm_create(uid[0], rank, world)
+    comm_stream = torch.cuda.Stream()                     # halo messages travel here while the interior is swept
+
+    def load():
+        can_dev.copy_(host, non_blocking=True)
+        culgt.culgt_slab_pack(local, can_dev, links)
+        culgt.culgt_slab_exchange_all_nccl(comm, local, links)
+
+    def sweeps(n):
+        culgt.culgt_slab_or_sweeps_nccl(comm, local, links, n, omega, comm_stream)
+
+    def check():
+        culgt.culgt_slab_theta_F_nccl(comm, lat, local, links, ws, sums, scal[0:1], scal[1:2])
+
+    load()
+    t = time_sweep_loop(torch, None, sweeps, check, args.steps, args.warmup, args.check_every, barrier,
+                        ClockSampler(local_rank))
+    theta, F = (float(x) for x in scal.cpu())
+    elapsed_max_ms = max_over_ranks(t["elapsed_ms"], world, "cuda")
+    value = V * args.steps / (elapsed_max_ms * 1e-3)
+    slab_bytes = 4 * (V // world) * cfg["params"] * (cfg["precision"] // 8)
+    halo = culgt.culgt_slab_halo_bytes(local)
+    peak, peak_src = measured_peak()
+    gbs = 2 * slab_bytes / (t["launch_ms"] * 1e-3) / 1e9
+
+    e2e = None
+    if not args.no_e2e:
+        def host_job(n):
+            load()
+            sweeps(n)
+            check()
+            culgt.culgt_slab_unpack(local, links, can_dev)
+            host.copy_(can_dev, non_blocking=True)
+            return tuple(float(x) for x in scal.cpu())
+        host_job(2)
+        barrier()
+        t0 = time.perf_counter()
+        th_e, F_e = host_job(args.steps)
+        torch.cuda.synchronize()
+        dt_max = max_over_ranks(time.perf_counter() - t0, world, "cuda")
+        cbytes = host.numel() * host.element_size()
+        e2e = {"value": V * args.steps / dt_max, "unit": UNIT, "h2d_bytes_per_step": world * cbytes / args.steps,
+               "d2h_bytes_per_step": world * (cbytes + 16) / args.steps,
+               "job": f"every rank: H2D of its slab ({cbytes} B) + pack + halo exchange + {args.steps} sweeps + "
+                      f"theta,F + unpack + D2H", "theta": th_e, "F": F_e}
+    culgt.culgt_slab_comm_destroy(comm)
+    if rank == 0:
+        conf = workload_config(args, cfg)
+        conf["parallelism"] = (f"time-slab split: {world} slab(s) of {T} time-slices, one per GPU; per half-sweep one "
+                               f"ncclSend/ncclRecv halo message of {halo} B each way per boundary, boundary slices swept "
+                               f"first; theta/F from all-gathered per-slab sums")
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": elapsed_max_ms / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f32" if cfg["precision"] == 32 else "f64",
+            "data": "synthetic", "config": conf, "gflops": value * flops_per_site(cfg) / 1e9,
+            "algorithmic_gbs": value * 16 * (cfg["params"] * cfg["precision"] // 8) / 1e9,
+            "gpu_launches": 2 * args.steps * (3 if T > 2 else 2) + 3 * t["n_checks"],
+            "halo_bytes_per_step_per_rank": 4 * halo, "e2e": e2e,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                         "traffic": None, "kernel": culgt.culgt_sweep_kernel_name(lat) + " on one slab (windowed)",
+                         "bytes_per_launch": 2 * slab_bytes, "launch_us": 1e3 * t["launch_ms"], "peak_source": peak_src,
+                         "note": "per rank: a half-sweep of ONE slab (its three window launches), algorithmic bytes"},
+            "cpu_baseline": None, "clocks": t["clocks"], "final": {"theta": theta, "F": F},
+            "check_ms_total": t["check_ms"],
+        }), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.sharded:
+        run_sharded(args)
         return
 
     import torch

@@ -81,17 +81,20 @@ def _chunks(n: int):
         yield c, lo, min(n, lo + _CHUNK)
 
 
-def _fill_chunks(out: np.ndarray, make_chunk, threads: bool = True) -> np.ndarray:
-    """out[lo:hi] = make_chunk(c, hi - lo) for every RNG chunk c; chunks are independent (each has its own
-    Philox key), so they may be filled by a few threads -- the array does not depend on how many.
-    (threads=False for generators made of stacked 3x3 matmuls, which run slower side by side.)"""
-    n = out.shape[0]
+def _fill_chunks(out: np.ndarray, make_chunk, threads: bool = True, first: int = 0) -> np.ndarray:
+    """out = elements [first, first + len(out)) of the sequence whose RNG chunk c makes elements
+    [c*_CHUNK, (c+1)*_CHUNK): out[...] = make_chunk(c, m)[...] for every chunk that overlaps the range
+    (m = how many leading elements of the chunk are needed; a generator's first m elements do not depend
+    on how many more are drawn).  Chunks are independent (each has its own Philox key), so they may be
+    filled by a few threads -- the array does not depend on how many.  (threads=False for generators
+    made of stacked 3x3 matmuls, which run slower side by side.)"""
+    last = first + out.shape[0]
 
-    def job(item):
-        c, lo, hi = item
-        out[lo:hi] = make_chunk(c, hi - lo)
+    def job(c):
+        lo, hi = max(first, c * _CHUNK), min(last, (c + 1) * _CHUNK)
+        out[lo - first:hi - first] = make_chunk(c, hi - c * _CHUNK)[lo - c * _CHUNK:]
 
-    items = list(_chunks(n))
+    items = list(range(first // _CHUNK, (last + _CHUNK - 1) // _CHUNK)) if last > first else []
     if len(items) <= 1 or not threads:
         for item in items:
             job(item)
@@ -119,12 +122,13 @@ def _gram_schmidt_su3(a: np.ndarray, b: np.ndarray) -> np.ndarray:
     return out
 
 
-def haar_su3(n: int, seed: int, stream: int = 0) -> np.ndarray:
+def haar_su3(n: int, seed: int, stream: int = 0, first: int = 0) -> np.ndarray:
+    """n Haar SU(3) matrices: elements [first, first + n) of the (seed, stream) sequence."""
     def chunk(c, m):
         z = _rng(seed, stream, c).standard_normal((m, 12))
         return _gram_schmidt_su3(z[:, 0:3] + 1j * z[:, 3:6], z[:, 6:9] + 1j * z[:, 9:12])
 
-    return _fill_chunks(np.empty((n, 3, 3), dtype=np.complex128), chunk)
+    return _fill_chunks(np.empty((n, 3, 3), dtype=np.complex128), chunk, first=first)
 
 
 def su2_from_quaternion(a: np.ndarray) -> np.ndarray:
@@ -137,13 +141,13 @@ def su2_from_quaternion(a: np.ndarray) -> np.ndarray:
     return out
 
 
-def haar_su2(n: int, seed: int, stream: int = 0) -> np.ndarray:
+def haar_su2(n: int, seed: int, stream: int = 0, first: int = 0) -> np.ndarray:
     def chunk(c, m):
         z = _rng(seed, stream, c).standard_normal((m, 4))
         z /= np.linalg.norm(z, axis=1, keepdims=True)
         return su2_from_quaternion(z)
 
-    return _fill_chunks(np.empty((n, 2, 2), dtype=np.complex128), chunk)
+    return _fill_chunks(np.empty((n, 2, 2), dtype=np.complex128), chunk, first=first)
 
 
 def _expm_i_hermitian(h: np.ndarray) -> np.ndarray:
@@ -161,17 +165,17 @@ def _expm_i_hermitian(h: np.ndarray) -> np.ndarray:
     return acc
 
 
-def near_identity_su3(n: int, eps: float, seed: int, stream: int = 0) -> np.ndarray:
+def near_identity_su3(n: int, eps: float, seed: int, stream: int = 0, first: int = 0) -> np.ndarray:
     def chunk(c, m):
         coef = _rng(seed, stream, c).standard_normal((m, 8))
         h = np.tensordot(coef, _GM, axes=(1, 0)) * 0.5
         u = _expm_i_hermitian(eps * h)
         return _gram_schmidt_su3(u[:, 0], u[:, 1])
 
-    return _fill_chunks(np.empty((n, 3, 3), dtype=np.complex128), chunk, threads=False)
+    return _fill_chunks(np.empty((n, 3, 3), dtype=np.complex128), chunk, threads=False, first=first)
 
 
-def near_identity_su2(n: int, eps: float, seed: int, stream: int = 0) -> np.ndarray:
+def near_identity_su2(n: int, eps: float, seed: int, stream: int = 0, first: int = 0) -> np.ndarray:
     """exp(i*eps*c.sigma/2), c ~ N(0,1)^3 (closed form on the 3-sphere)."""
     def chunk(c, m):
         v = _rng(seed, stream, c).standard_normal((m, 3)) * (0.5 * eps)
@@ -181,7 +185,7 @@ def near_identity_su2(n: int, eps: float, seed: int, stream: int = 0) -> np.ndar
         q[:, 1:] = v * (np.sinc(r / np.pi))[:, None]
         return su2_from_quaternion(q)
 
-    return _fill_chunks(np.empty((n, 2, 2), dtype=np.complex128), chunk)
+    return _fill_chunks(np.empty((n, 2, 2), dtype=np.complex128), chunk, first=first)
 
 
 def _shift_sites(field: np.ndarray, dims, mu: int, step: int) -> np.ndarray:
@@ -212,30 +216,68 @@ def pure_gauge(g: np.ndarray, dims) -> np.ndarray:
 
 
 def make_config(dims, group: int, kind: str, seed: int, eps: float = 0.0,
-                scramble: bool = False) -> np.ndarray:
+                scramble: bool = False, t_range=None) -> np.ndarray:
     """Complex128 canonical field U[V,4,nc,nc].
 
     kind: "near_identity" (needs eps), "haar" (hot), "unit", "pure_gauge".
     scramble: apply a Haar random gauge transformation g(x) (stream 1 of the same seed).
+    t_range = (t_lo, t_hi): only the sites of the time-slices [t_lo, t_hi) -- exactly the rows
+    [t_lo*Vs, t_hi*Vs) of the full field (Vs = N0*N1*N2; t is the slowest coordinate), made without
+    making the rest (one time slab per rank, bench.py --sharded).
     """
-    v = volume(dims)
     if group not in (2, 3):
         raise ValueError("group must be 2 or 3")
+    n0, n1, n2, n3 = (int(d) for d in dims)
+    vs = n0 * n1 * n2
+    t_lo, t_hi = (0, n3) if t_range is None else (int(t_range[0]), int(t_range[1]))
+    if not 0 <= t_lo < t_hi <= n3:
+        raise ValueError("t_range outside the lattice")
+    v = vs * (t_hi - t_lo)
     haar = haar_su3 if group == 3 else haar_su2
+
+    def g_field():
+        """g(x) on the slices [t_lo, t_hi] (the slice behind the range is needed for g(x + t_hat); periodic)"""
+        g = np.empty((v + vs, group, group), dtype=np.complex128)
+        g[:v] = haar(v, seed, 1, first=vs * t_lo)
+        g[v:] = haar(vs, seed, 1, first=vs * (t_hi % n3))
+        return g
+
     if kind == "near_identity":
         near = near_identity_su3 if group == 3 else near_identity_su2
-        u = near(4 * v, eps, seed, 0).reshape(v, 4, group, group)
+        u = near(4 * v, eps, seed, 0, first=4 * vs * t_lo).reshape(v, 4, group, group)
     elif kind == "haar":
-        u = haar(4 * v, seed, 0).reshape(v, 4, group, group)
+        u = haar(4 * v, seed, 0, first=4 * vs * t_lo).reshape(v, 4, group, group)
     elif kind == "unit":
         u = np.broadcast_to(np.eye(group, dtype=np.complex128), (v, 4, group, group)).copy()
     elif kind == "pure_gauge":
-        return pure_gauge(haar(v, seed, 1), dims)
+        if t_range is None:
+            return pure_gauge(haar(v, seed, 1), dims)
+        u = np.broadcast_to(np.eye(group, dtype=np.complex128), (v, 4, group, group)).copy()
+        return _scramble_slices(u, g_field(), (n0, n1, n2, t_hi - t_lo))
     else:
         raise ValueError(f"unknown kind {kind!r}")
     if scramble:
-        u = gauge_scramble(u, haar(v, seed, 1), dims)
+        if t_range is None:
+            u = gauge_scramble(u, haar(v, seed, 1), dims)
+        else:
+            u = _scramble_slices(u, g_field(), (n0, n1, n2, t_hi - t_lo))
     return u
+
+
+def _scramble_slices(u: np.ndarray, g: np.ndarray, dims_loc) -> np.ndarray:
+    """gauge_scramble on a range of time-slices: g carries one extra slice (the one behind the range),
+    spatial shifts are periodic inside a slice, the t shift reads the next slice of g."""
+    n0, n1, n2, nt = dims_loc
+    vs = n0 * n1 * n2
+    v = vs * nt
+    out = np.empty_like(u)
+    gs = g[:v]
+    for mu in range(3):
+        gf = _shift_sites(gs, dims_loc, mu, +1)
+        out[:, mu] = np.matmul(np.matmul(gs, u[:, mu]), np.conj(np.swapaxes(gf, 1, 2)))
+    gf = g[vs:v + vs]                                   # g(x + t_hat): the same site one slice later
+    out[:, 3] = np.matmul(np.matmul(gs, u[:, 3]), np.conj(np.swapaxes(gf, 1, 2)))
+    return out
 
 
 def to_real(uc: np.ndarray, dtype=np.float64) -> np.ndarray:

@@ -26,7 +26,7 @@ inline int reduce_blocks_fused(int vh, int half = 64) { return (vh + half - 1) /
 // slice/128; never below 4096) followed by 2 * N3 result slots that the *_host / *_fix paths
 // read back (Landau uses the first two).
 inline size_t reduce_partial_doubles(const Geom& g) {
-  size_t n = 2 * (size_t)reduce_blocks_fused(g.vh);
+  size_t n = 2 * (size_t)reduce_blocks_fused(g.vh) + 8;      // + 8: the 4-threads-per-site kernel rounds per parity
   const size_t c = 2 * (size_t)g.n[3] * (size_t)reduce_blocks_fused(g.stride[3]);
   if (c > n) n = c;
   return n > 4096 ? n : 4096;

@@ -53,7 +53,7 @@ def test_sizes():
     def ws_bytes(partials, n3):
         red = partials + 2 * n3 + (n3 + 7) // 8
         return (red + 15) // 16 * 16 * 8 + ctl
-    assert culgt.culgt_workspace_bytes(culgt.Lattice((64,) * 4, 3, 64, 18)) == ws_bytes(2 * (64 ** 4 // 2 // 64), 64)
+    assert culgt.culgt_workspace_bytes(culgt.Lattice((64,) * 4, 3, 64, 18)) == ws_bytes(2 * (64 ** 4 // 2 // 64) + 8, 64)
     assert culgt.culgt_workspace_bytes(culgt.Lattice((4,) * 4, 3, 64, 18)) == ws_bytes(4096, 4)
 
 

@@ -62,3 +62,15 @@ def test_reference_arm_json_line():
     assert d["impl"] == "reference" and d["metric"] == "su3_landau_or_site_updates_per_s"
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"]
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+
+
+def test_sharded_arm_json_line():
+    """`bench.py --sharded` (time-slab decomposition, one slab per rank over NCCL) with one rank: the
+    contract keys, strong scaling, and the same theta/F as the replica arm's field would give."""
+    d = run("--sharded", "--steps", "6", "--warmup", "3", "--check-every", "3", "--workload", "cfg2")
+    assert d["metric"] == "su3_landau_or_site_updates_per_s" and d["n_gpus"] == 1 and d["scaling"] == "strong"
+    assert d["value"] > 0 and d["e2e"]["value"] > 0 and d["e2e"]["h2d_bytes_per_step"] > 0
+    assert "time-slab split: 1 slab(s) of 16 time-slices" in d["config"]["parallelism"]
+    assert d["halo_bytes_per_step_per_rank"] == 4 * (16 ** 3 // 2) * 48
+    assert d["roofline"]["frac"] == d["roofline"]["achieved"] / d["roofline"]["peak"]
+    assert 0 < d["final"]["F"] < 1 and d["final"]["theta"] > 0

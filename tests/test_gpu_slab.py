@@ -143,3 +143,42 @@ def test_single_halo_messages_and_windows():
         culgt.culgt_slab_or_sweep_window(a.local, a.slabs[0], 0, 1.7, 2, 1)
     with pytest.raises(culgt.CulgtError):
         culgt.culgt_slab_or_sweep_window(a.local, a.slabs[0], 0, 1.7, 0, T + 1)
+
+
+@pytest.mark.parametrize("overlap", [False, True])
+@pytest.mark.parametrize("precision,params", [(64, 18), (32, 12)])
+def test_nccl_transport_with_one_rank(precision, params, overlap):
+    """The one-slab-per-rank drivers (ncclSend / ncclRecv halo messages, all-gathered theta/F sums) with
+    a communicator of ONE rank: every message is a send to self matched by a receive from self, i.e.
+    the periodic lattice talking to itself through its ghost slice over the real NCCL code path.
+    Three sweeps must be bit-identical to the undivided sweep, without and with the boundary-first
+    schedule whose messages travel on a second stream.  (More ranks need more GPUs than this box has;
+    the rank bookkeeping is covered by tests/test_slab_bookkeeping.py.)"""
+    dims = (8, 8, 8, 8)
+    u = li.make_config(dims, 3, "near_identity", 79, eps=0.5, scramble=True)
+    lat = culgt.Lattice(dims, 3, precision, params)
+    local = culgt.culgt_slab_lattice(lat, 1)
+    comm = culgt.culgt_slab_comm_create(culgt.culgt_slab_comm_unique_id(), 0, 1)
+    try:
+        can = torch.from_numpy(li.to_real(np.ascontiguousarray(u), np_dtype(precision))).cuda()
+        links = culgt.alloc_slab_links(local)
+        links.fill_(float("nan"))
+        culgt.culgt_slab_pack(local, can, links)
+        culgt.culgt_slab_exchange_all_nccl(comm, local, links)
+        ws = culgt.alloc_workspace(local)
+        sums = torch.zeros(4, dtype=torch.float64, device="cuda")
+        scal = torch.zeros(2, dtype=torch.float64, device="cuda")
+        side = torch.cuda.Stream() if overlap else None
+        culgt.culgt_slab_or_sweeps_nccl(comm, local, links, 3, 1.7, side)
+        culgt.culgt_slab_theta_F_nccl(comm, lat, local, links, ws, sums, scal[0:1], scal[1:2])
+        culgt.culgt_slab_unpack(local, links, can)
+        torch.cuda.synchronize()
+        got = li.from_real(can.cpu().numpy())
+        th, F = scal.cpu().tolist()
+    finally:
+        culgt.culgt_slab_comm_destroy(comm)
+    whole = GpuField(dims, 3, precision, params, u)
+    whole.sweep(1.7, 3)
+    assert np.array_equal(got, whole.download())
+    th_w, F_w = whole.theta_functional()
+    assert abs(th - th_w) <= 1e-12 * th_w and abs(F - F_w) <= 1e-13 * abs(F_w)
