@@ -29,24 +29,44 @@ __device__ __forceinline__ double block_sum(double v) {
   return t;   // valid in thread 0
 }
 
-// sum_ab |Delta_ab|^2 with Delta = [(K - K^dagger)/(2i)]_traceless (reading C-11):
-// D_ab = (K_ab - conj(K_ba))/(2i);  re(D_ab) = (im K_ab + im K_ba)/2, im(D_ab) = -(re K_ab - re K_ba)/2.
-__device__ __forceinline__ double theta_from_K(const double* K) {
-  double dre[3];
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+
+
+// What theta and F need of one link (reading C-11: Delta = [(K - K^dagger)/(2i)]_traceless depends only
+// on the anti-Hermitian part of K, to which U_mu(x) and U_mu(x-mu)^dagger contribute with opposite signs):
+//   a[0..2] = Im U_aa;   a[3], a[4] = Im U_01 + Im U_10, Re U_01 - Re U_10;   a[5], a[6]: (0,2);   a[7], a[8]: (1,2)
+// and Re tr U.  acc += sign * a.  The stored rows are widened first; the third row of 12-parameter
+// storage is rebuilt in fp64.
+template <typename S>
+__device__ __forceinline__ double add_antihermitian_parts(const typename S::Real* U, double sign, double* acc) {
+  double m[18];
 #pragma unroll
-  for (int a = 0; a < 3; ++a) dre[a] = K[CULGT_IM(a, a)];
-  const double tr = (dre[0] + dre[1] + dre[2]) * (1.0 / 3.0);
+  for (int i = 0; i < S::NP; ++i) m[i] = (double)U[i];
+  if (S::NP == 12) reconstruct_row2(m);
+  acc[0] = fma(sign, m[CULGT_IM(0, 0)], acc[0]);
+  acc[1] = fma(sign, m[CULGT_IM(1, 1)], acc[1]);
+  acc[2] = fma(sign, m[CULGT_IM(2, 2)], acc[2]);
+  acc[3] = fma(sign, m[CULGT_IM(0, 1)] + m[CULGT_IM(1, 0)], acc[3]);
+  acc[4] = fma(sign, m[CULGT_RE(0, 1)] - m[CULGT_RE(1, 0)], acc[4]);
+  acc[5] = fma(sign, m[CULGT_IM(0, 2)] + m[CULGT_IM(2, 0)], acc[5]);
+  acc[6] = fma(sign, m[CULGT_RE(0, 2)] - m[CULGT_RE(2, 0)], acc[6]);
+  acc[7] = fma(sign, m[CULGT_IM(1, 2)] + m[CULGT_IM(2, 1)], acc[7]);
+  acc[8] = fma(sign, m[CULGT_RE(1, 2)] - m[CULGT_RE(2, 1)], acc[8]);
+  return m[CULGT_RE(0, 0)] + m[CULGT_RE(1, 1)] + m[CULGT_RE(2, 2)];
+}
+
+// tr[Delta Delta^dagger] from the accumulated parts: the diagonal with its trace removed, and
+// |D_ab|^2 + |D_ba|^2 = (s^2 + r^2)/2 for D_ab = (s - i r)/2.
+__device__ __forceinline__ double theta_from_parts(const double* a) {
+  const double tr = (a[0] + a[1] + a[2]) * (1.0 / 3.0);
   double sum = 0;
 #pragma unroll
-  for (int a = 0; a < 3; ++a) sum += (dre[a] - tr) * (dre[a] - tr);
+  for (int c = 0; c < 3; ++c) sum += (a[c] - tr) * (a[c] - tr);
 #pragma unroll
-  for (int a = 0; a < 3; ++a)
-#pragma unroll
-    for (int b = a + 1; b < 3; ++b) {
-      const double re = 0.5 * (K[CULGT_IM(a, b)] + K[CULGT_IM(b, a)]);
-      const double im = -0.5 * (K[CULGT_RE(a, b)] - K[CULGT_RE(b, a)]);
-      sum += 2.0 * (re * re + im * im);     // |D_ab|^2 + |D_ba|^2, D Hermitian
-    }
+  for (int c = 3; c < 9; ++c) sum = fma(0.5 * a[c], a[c], sum);
   return sum;
 }
 
@@ -69,11 +89,10 @@ __device__ __forceinline__ double theta_from_K(const double* K) {
 // as its direction lands: every load of the site is in flight at once without holding registers (the
 // half-sweep's staging), and the conversions of direction mu overlap the loads of the
 // later ones.  No __syncthreads: cp.async.wait_group orders a thread against its own copies.
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
-}
-
+// Measured and rejected: four threads per site with the parts exchanged through shared
+// memory (commit 7e9a7e2: 72 us against 59 at 32^4 fp32-12 -- a third of the bytes in flight per SM),
+// part of the fp32 -> fp64 conversions moved from the XU to the integer pipe (no change: the kernel is
+// not bound by a pipe), staging through the L1 with cp.async.ca (82 us).
 template <typename S, int BLOCK, bool COULOMB, bool STAGED>
 __global__ void __launch_bounds__(BLOCK, STAGED ? 512 / BLOCK : 0)
 theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
@@ -91,9 +110,9 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
   if (in_group < group_size) {
     const SiteCoord sc = decode_site(g, h, parity);
     if (S::NC == 3) {
-      double K[18];
+      double a[9];
 #pragma unroll
-      for (int i = 0; i < 18; ++i) K[i] = 0;
+      for (int i = 0; i < 9; ++i) a[i] = 0;
       if constexpr (STAGED) {
         typedef typename S::Vec Vec;
         extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -120,12 +139,8 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
           Real U[kLinkRegs];
 #pragma unroll
           for (int j = 0; j < S::NV; ++j) vec_get(sm[(l * S::NV + j) * BLOCK], U + j * S::VL);
-          double Ud[18];                     // widened first: the third row is rebuilt in fp64
-#pragma unroll
-          for (int i = 0; i < S::NP; ++i) Ud[i] = (double)U[i];
-          if (S::NP == 12) reconstruct_row2(Ud);
-          if ((l & 1) == 0) f += Ud[CULGT_RE(0, 0)] + Ud[CULGT_RE(1, 1)] + Ud[CULGT_RE(2, 2)];
-          accumulate(K, Ud, (l & 1) != 0);
+          const double tr = add_antihermitian_parts<S>(U, (l & 1) ? -1.0 : 1.0, a);
+          if ((l & 1) == 0) f += tr;
         }
       } else {
       // the loads of a batch of directions are issued before any of them is used (memory-level
@@ -144,20 +159,12 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
 #pragma unroll
         for (int b = 0; b < MU_BATCH; ++b)
           if (mu0 + b < ND) {
-            double Ud[18];                   // widened first: the third row is rebuilt in fp64
-#pragma unroll
-            for (int i = 0; i < S::NP; ++i) Ud[i] = (double)U[2 * b][i];
-            if (S::NP == 12) reconstruct_row2(Ud);
-            f += Ud[CULGT_RE(0, 0)] + Ud[CULGT_RE(1, 1)] + Ud[CULGT_RE(2, 2)];
-            accumulate(K, Ud, false);
-#pragma unroll
-            for (int i = 0; i < S::NP; ++i) Ud[i] = (double)U[2 * b + 1][i];
-            if (S::NP == 12) reconstruct_row2(Ud);
-            accumulate(K, Ud, true);
+            f += add_antihermitian_parts<S>(U[2 * b], 1.0, a);
+            add_antihermitian_parts<S>(U[2 * b + 1], -1.0, a);
           }
       }
       }
-      th = theta_from_K(K);
+      th = theta_from_parts(a);
     } else {
       double d[3] = {0, 0, 0};
 #pragma unroll
@@ -182,112 +189,6 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
   }
 }
 
-
-// ---------------------------------------------------------------------------------------------------
-// SU(3), Landau gauge, fp32 storage: FOUR THREADS PER SITE, one direction each.
-//
-// The one-thread-per-site kernel above widens and rebuilds all 8 links of a site in one long
-// dependent sequence; at 16 warps per SM (its registers and its 48 KB of staged links allow no more)
-// the XU pipe (fp32 -> fp64 conversions), the FP64 pipe (third row, sums) and the issue slots each
-// sit at 40-47 % and nothing hides the rest (profiles/r1_ncu_full_theta_cfg3_fp32.md).  Here a CTA is
-// 4 warps = 4 directions x 32 consecutive sites of one parity: a thread loads only U_mu(x) and
-// U_mu(x-mu) (6 coalesced 16-byte loads, all in flight at once, no staging), and since theta needs
-// only the anti-Hermitian part of K (reading C-11),
-//     Delta = [(K - K^dagger)/(2i)]_traceless,   K - K^dagger = sum_mu (U_mu(x) - U_mu(x)^dagger) - (same of U_mu(x-mu)),
-// it reduces each link to 9 reals -- d_a = Im U_aa and, for a < b, s_ab = Im U_ab + Im U_ba,
-// r_ab = Re U_ab - Re U_ba -- and keeps up minus down.  The four directions of a site meet in shared
-// memory ([component][direction][site], 9 KB, double-buffered: one barrier per tile); thread (mu, site)
-// then sums the four contributions of component group mu (mu = 0: the diagonal, where the trace is
-// removed; mu = 1, 2, 3: the pairs (0,1), (0,2), (1,2)) and adds its share
-//     sum_a (d_a - tr/3)^2        or        (s_ab^2 + r_ab^2)/2        of  tr[Delta Delta^dagger].
-// F is the sum of Re tr over the up links, one per thread.  A CTA walks TILES consecutive 32-site
-// tiles of its parity; CTA 2k + p works on parity p of the same index range, so a link's second read
-// (as the down link of the other parity's neighbouring site) is an L2 hit.  One partial per CTA and
-// quantity, summed in a fixed order as before: deterministic.
-// ---------------------------------------------------------------------------------------------------
-template <typename S>
-__device__ __forceinline__ void antihermitian_parts(const typename S::Real* U, double* a, double* re_tr) {
-  // widen rows 0 and 1; row 2 is rebuilt in fp64 (12-parameter storage) or widened (18-parameter)
-  double m[18];
-#pragma unroll
-  for (int i = 0; i < 12; ++i) m[i] = (double)U[i];
-  if (S::NP == 12) {
-    reconstruct_row2(m);
-  } else {
-#pragma unroll
-    for (int i = 12; i < 18; ++i) m[i] = (double)U[i];
-  }
-  a[0] = m[CULGT_IM(0, 0)];
-  a[1] = m[CULGT_IM(1, 1)];
-  a[2] = m[CULGT_IM(2, 2)];
-  a[3] = m[CULGT_IM(0, 1)] + m[CULGT_IM(1, 0)];
-  a[4] = m[CULGT_RE(0, 1)] - m[CULGT_RE(1, 0)];
-  a[5] = m[CULGT_IM(0, 2)] + m[CULGT_IM(2, 0)];
-  a[6] = m[CULGT_RE(0, 2)] - m[CULGT_RE(2, 0)];
-  a[7] = m[CULGT_IM(1, 2)] + m[CULGT_IM(2, 1)];
-  a[8] = m[CULGT_RE(1, 2)] - m[CULGT_RE(2, 1)];
-  *re_tr = m[CULGT_RE(0, 0)] + m[CULGT_RE(1, 1)] + m[CULGT_RE(2, 2)];
-}
-
-template <typename S, int TILES, int MINB>
-__global__ void __launch_bounds__(128, MINB)
-theta_functional_tps4_kernel(const typename S::Vec* __restrict__ links, const Geom g,
-                             double* __restrict__ partial_theta, double* __restrict__ partial_F,
-                             const int* __restrict__ stop_flag) {
-  typedef typename S::Real Real;
-  if (stop_flag != nullptr && *stop_flag != 0) return;   // driver loop: this check is no longer wanted
-  __shared__ double parts[2][9][4][32];                  // [buffer][component][direction][site]
-  const int mu = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int parity = blockIdx.x & 1;
-  const int h0 = (int)(blockIdx.x >> 1) * (32 * TILES);
-  double th = 0, f = 0;
-#pragma unroll 1
-  for (int tile = 0; tile < TILES; ++tile) {
-    const int h = h0 + tile * 32 + lane;
-    double a[9];
-#pragma unroll
-    for (int c = 0; c < 9; ++c) a[c] = 0;
-    if (h < g.vh) {
-      const SiteCoord sc = decode_site(g, h, parity);
-      Real Uu[kLinkRegs], Ud[kLinkRegs];
-      load_params<S>(link_base<S>(links, g, parity, mu, h), g.pitch, Uu);
-      load_params<S>(link_base<S>(links, g, 1 - parity, mu, down_index(g, h, sc, mu)), g.pitch, Ud);
-      double b[9], tr;
-      antihermitian_parts<S>(Uu, a, &tr);
-      f += tr;
-      antihermitian_parts<S>(Ud, b, &tr);
-#pragma unroll
-      for (int c = 0; c < 9; ++c) a[c] -= b[c];
-    }
-    double(*buf)[4][32] = parts[tile & 1];
-#pragma unroll
-    for (int c = 0; c < 9; ++c) buf[c][mu][lane] = a[c];
-    __syncthreads();
-    // component group mu of this site: its four directions, added in the order mu' = 0, 1, 2, 3
-    if (mu == 0) {
-      double d[3];
-#pragma unroll
-      for (int c = 0; c < 3; ++c) d[c] = ((buf[c][0][lane] + buf[c][1][lane]) + buf[c][2][lane]) + buf[c][3][lane];
-      const double tr = (d[0] + d[1] + d[2]) * (1.0 / 3.0);
-#pragma unroll
-      for (int c = 0; c < 3; ++c) th += (d[c] - tr) * (d[c] - tr);
-    } else {
-      const int c = 1 + 2 * mu;
-      const double s = ((buf[c][0][lane] + buf[c][1][lane]) + buf[c][2][lane]) + buf[c][3][lane];
-      const double r = ((buf[c + 1][0][lane] + buf[c + 1][1][lane]) + buf[c + 1][2][lane]) + buf[c + 1][3][lane];
-      th += 0.5 * (s * s + r * r);          // |D_ab|^2 + |D_ba|^2 with D_ab = (s - i r)/2
-    }
-  }
-  const double st = block_sum<128>(th);
-  __syncthreads();                       // block_sum's shared slots are reused
-  const double sf = block_sum<128>(f);
-  if (threadIdx.x == 0) {
-    partial_theta[blockIdx.x] = st;
-    partial_F[blockIdx.x] = sf;
-  }
-}
-
-constexpr int kTps4Tiles = 4;      // 32-site tiles per CTA: one partial per 128 sites of a parity = vh/64 per quantity
 
 // Final pass of the per-slice (Coulomb) sums: block (group, quantity) sums the n partials of that group
 // in a fixed order and scales.  partial = [quantity][group][n]; quantity 0 = theta, 1 = F; group = time-slice for the
@@ -365,22 +266,12 @@ static cudaError_t launch_theta_staged(dim3 grid, const void* links, const Geom&
 // DESIGN.md 6.3); the other formats the register path with 128 sites of each parity per CTA.
 template <typename S>
 static constexpr bool theta_is_staged() { return S::NC == 3 && S::NP == 12 && sizeof(typename S::Real) == 4; }
-// Landau gauge, SU(3): four threads per site (measured)
-template <typename S>
-static constexpr bool theta_is_tps4() { return S::NC == 3; }
 
 // group_size sites of each parity per y-slot of the grid (the sublattice, or one time-slice of it);
 // the partials of quantity 1 start at p_theta + ny * blocks
 template <typename S, bool COULOMB>
 static cudaError_t launch_theta_pass(int group_size, int ny, const void* links, const Geom& g, double* p_theta,
                                      const int* stop_flag, cudaStream_t st, int* blocks_out) {
-  if constexpr (!COULOMB && theta_is_tps4<S>()) {
-    const int nb = 2 * ((group_size + 32 * kTps4Tiles - 1) / (32 * kTps4Tiles));
-    *blocks_out = nb;
-    theta_functional_tps4_kernel<S, kTps4Tiles, (sizeof(typename S::Real) == 4 ? 6 : 4)><<<nb, 128, 0, st>>>(
-        (const typename S::Vec*)links, g, p_theta, p_theta + nb, stop_flag);
-    return cudaGetLastError();
-  }
   const int nb = reduce_blocks_fused(group_size, theta_is_staged<S>() ? 64 : 128);
   *blocks_out = nb;
   double* p_F = p_theta + (size_t)ny * nb;
@@ -388,8 +279,8 @@ static cudaError_t launch_theta_pass(int group_size, int ny, const void* links, 
   if constexpr (theta_is_staged<S>()) {
     return launch_theta_staged<S, 128, COULOMB>(grid, links, g, p_theta, p_F, stop_flag, st);
   } else {
-    theta_functional_kernel<S, 256, COULOMB, false><<<grid, 256, 0, st>>>((const typename S::Vec*)links, g, p_theta, p_F,
-                                                                          stop_flag);
+    theta_functional_kernel<S, 256, COULOMB, false><<<grid, 256, 0, st>>>((const typename S::Vec*)links, g, p_theta,
+                                                                                p_F, stop_flag);
     return cudaGetLastError();
   }
 }
