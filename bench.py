@@ -404,10 +404,20 @@ def driver_loop_times(culgt, torch, rank):
                 theta = float(scal[0].item())
             return done, theta
 
+        def fix(variant):
+            # variant 34 = the production kernels launched per half-sweep (no L2 hints: irrelevant at this
+            # size), stop word on the device; variant 0 additionally takes the one-kernel loop where it applies
+            def run():
+                culgt.culgt_set_sweep_variant(variant)
+                try:
+                    return culgt.culgt_landau_fix(f.lat, f.links, f.ws, f.omega, target, max_sweeps, every)[:2]
+                finally:
+                    culgt.culgt_set_sweep_variant(0)
+            return run
+
         res = {}
-        for label, loop in (("host_sync_every_check", host_loop),
-                            ("device_stop_flag", lambda: culgt.culgt_landau_fix(f.lat, f.links, f.ws, f.omega, target,
-                                                                                max_sweeps, every)[:2])):
+        for label, loop in (("host_sync_every_check", host_loop), ("device_stop_flag_launch_per_half_sweep", fix(34)),
+                            ("device_stop_flag", fix(0))):
             best = None
             for _ in range(3):
                 culgt.culgt_pack(f.lat, f.can_dev, f.links)

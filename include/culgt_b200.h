@@ -132,8 +132,11 @@ int culgt_gauge_transform(const culgt_lattice* lat, void* links, const void* g, 
  * launch enqueued behind it into a no-op), so the host synchronises only once per batch of about 32
  * sweeps' worth of launches, not at each check; the field, sweeps_done, theta and F are exactly
  * those of the loop that stops at the first check with theta < theta_target.  A NaN theta never
- * satisfies the test (the loop then runs to max_sweeps).  SYNCHRONISES.  Outputs are HOST pointers
- * (any may be NULL). */
+ * satisfies the test (the loop then runs to max_sweeps).  SU(3) lattices with at most one site block
+ * (128 sites for fp32 12-parameter storage, 64 otherwise) per SM and parity run the WHOLE loop as one
+ * cooperative kernel (grid barriers between half-sweeps, theta and F reduced inside it); the links
+ * are the same bit for bit, theta and F agree to rounding (the partial sums are grouped differently).
+ * SYNCHRONISES.  Outputs are HOST pointers (any may be NULL). */
 int culgt_landau_fix(const culgt_lattice* lat, void* links, void* workspace, double omega,
                      double theta_target, int max_sweeps, int check_every,
                      int* sweeps_done, double* theta_out, double* F_out, void* stream);

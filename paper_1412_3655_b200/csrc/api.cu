@@ -237,8 +237,24 @@ int culgt_landau_fix(const culgt_lattice* lat, void* links, void* workspace, dou
   cudaStream_t st = (cudaStream_t)stream;
   double* ws = (double*)workspace;
   double* scal = ws + reduce_partial_doubles(d.geom);
+  cudaError_t e;
+  if (g_variant == 0) {
+    // small SU(3) lattices: the whole loop as one cooperative kernel (csrc/fix_persistent.cu)
+    PersistCtl* pc = (PersistCtl*)(ws + fix_ctl_offset_doubles(d.geom));
+    e = launch_landau_fix_persistent(d, links, omega, theta_target, max_sweeps, check_every, ws, pc, st);
+    if (e == cudaSuccess) {
+      PersistCtl h;
+      if ((e = cudaMemcpyAsync(&h, pc, sizeof(h), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+      if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+      if (sweeps_done) *sweeps_done = h.sweeps_done;
+      if (theta_out) *theta_out = h.theta;
+      if (F_out) *F_out = h.F;
+      return CULGT_OK;
+    }
+    if (e != cudaErrorNotSupported) return cuda_fail(e);
+  }
   FixCtl* ctl = (FixCtl*)(ws + fix_ctl_offset_doubles(d.geom));
-  cudaError_t e = cudaMemsetAsync(ctl, 0, sizeof(FixCtl), st);
+  e = cudaMemsetAsync(ctl, 0, sizeof(FixCtl), st);
   if (e != cudaSuccess) return cuda_fail(e);
   FixCheck chk = {ctl, theta_target, 0};
   if ((e = launch_theta_functional(d, links, ws, scal, scal + 1, st, &chk)) != cudaSuccess) return cuda_fail(e);

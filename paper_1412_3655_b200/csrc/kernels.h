@@ -50,6 +50,13 @@ struct FixCtl {
   double theta, F;     // of the last check that ran
 };
 
+// Persistent driver loop for small lattices (fix_persistent.cu); shares FixCtl's slot.
+struct PersistCtl {
+  unsigned barrier;    // grid barrier: arrivals so far (monotone)
+  int sweeps_done;
+  double theta, F;
+};
+
 // Fused full sweep (or_sweep_fused.cu; -DCULGT_MEASURE builds only -- the struct is declared
 // unconditionally so that both builds lay the workspace out the same way).
 constexpr int kFusedMaxSlices = 512;
@@ -69,7 +76,7 @@ inline size_t ctl_offset_doubles(const Geom& g) { return (reduce_workspace_doubl
 inline size_t fix_ctl_offset_doubles(const Geom& g) { return ctl_offset_doubles(g); }
 inline size_t fused_ctl_offset_doubles(const Geom& g) { return ctl_offset_doubles(g) + 16; }
 inline size_t workspace_doubles(const Geom& g) { return fused_ctl_offset_doubles(g) + sizeof(FusedCtl) / 8; }
-static_assert(sizeof(FixCtl) <= 16 * 8, "FixCtl must fit its 16-double slot");
+static_assert(sizeof(FixCtl) <= 16 * 8 && sizeof(PersistCtl) <= 16 * 8, "the driver-loop control blocks share a 16-double slot");
 static_assert(sizeof(FusedCtl) % 8 == 0, "FusedCtl is addressed in doubles");
 
 // ---- half-sweeps ----------------------------------------------------------------------------------
@@ -120,6 +127,12 @@ cudaError_t launch_or_sweep_measure(const LatticeDesc& d, void* links, int parit
 cudaError_t launch_or_sweep_measure_slabbed(const LatticeDesc& d, void* links, double omega, int slab_slices,
                                             cudaStream_t st);
 #endif
+
+// The whole driver loop as one cooperative kernel (fix_persistent.cu): SU(3) lattices with at most one
+// site block per SM and parity; cudaErrorNotSupported otherwise.  partial: 2 * (site blocks) doubles.
+cudaError_t launch_landau_fix_persistent(const LatticeDesc& d, void* links, double omega, double theta_target,
+                                         int max_sweeps, int check_every, double* partial, PersistCtl* ctl,
+                                         cudaStream_t st);
 
 // ---- layout, reductions, transform ----------------------------------------------------------------
 cudaError_t launch_pack(const LatticeDesc& d, const void* canonical, void* links, cudaStream_t st);

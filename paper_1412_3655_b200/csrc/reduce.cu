@@ -219,13 +219,17 @@ final_sum_landau_kernel(const double* __restrict__ partial, int n, double scale_
                         double* __restrict__ out_theta, double* __restrict__ out_F, FixCtl* __restrict__ ctl,
                         double theta_target, int sweeps_before) {
   if (ctl != nullptr && ctl->stop != 0) return;
-  double acc = 0;
-  for (int i = threadIdx.x; i < n; i += BLOCK) acc += partial[i];
-  const double st = block_sum<BLOCK>(acc);
+  // both quantities at once, four partials of each in flight per thread (the loads are what this
+  // kernel waits for: one block, a few thousand partials)
+  double at = 0, af = 0;
+#pragma unroll 4
+  for (int i = threadIdx.x; i < n; i += BLOCK) {
+    at += partial[i];
+    af += partial[(size_t)n + i];
+  }
+  const double st = block_sum<BLOCK>(at);
   __syncthreads();
-  acc = 0;
-  for (int i = threadIdx.x; i < n; i += BLOCK) acc += partial[(size_t)n + i];
-  const double sf = block_sum<BLOCK>(acc);
+  const double sf = block_sum<BLOCK>(af);
   if (threadIdx.x == 0) {
     const double theta = st * scale_theta, F = sf * scale_F;
     *out_theta = theta;
@@ -241,6 +245,8 @@ final_sum_landau_kernel(const double* __restrict__ partial, int n, double scale_
     }
   }
 }
+
+constexpr int kFinalBlock = 1024;      // threads of the single block that sums the Landau partials
 
 template <typename S, int BLOCK, bool COULOMB>
 static cudaError_t launch_theta_staged(dim3 grid, const void* links, const Geom& g, double* p_theta, double* p_F,
@@ -292,7 +298,7 @@ static cudaError_t run_theta_functional(const LatticeDesc& d, const void* links,
   FixCtl* ctl = fix ? fix->ctl : nullptr;
   cudaError_t e = launch_theta_pass<S, false>(d.geom.vh, 1, links, d.geom, ws, ctl ? &ctl->stop : nullptr, st, &nblk);
   if (e != cudaSuccess) return e;
-  final_sum_landau_kernel<kReduceBlock><<<1, kReduceBlock, 0, st>>>(
+  final_sum_landau_kernel<kFinalBlock><<<1, kFinalBlock, 0, st>>>(
       ws, nblk, 1.0 / ((double)S::NC * (double)d.V), 1.0 / (4.0 * S::NC * (double)d.V), out_theta, out_F, ctl,
       fix ? fix->theta_target : 0.0, fix ? fix->sweeps_before : 0);
   return cudaGetLastError();
@@ -336,7 +342,7 @@ static cudaError_t run_theta_functional_sums(const LatticeDesc& d, const void* l
   int nblk = 0;
   cudaError_t e = launch_theta_pass<S, false>(d.geom.vh, 1, links, d.geom, ws, nullptr, st, &nblk);
   if (e != cudaSuccess) return e;
-  final_sum_landau_kernel<kReduceBlock><<<1, kReduceBlock, 0, st>>>(ws, nblk, 1.0, 1.0, out2, out2 + 1, nullptr, 0.0, 0);
+  final_sum_landau_kernel<kFinalBlock><<<1, kFinalBlock, 0, st>>>(ws, nblk, 1.0, 1.0, out2, out2 + 1, nullptr, 0.0, 0);
   return cudaGetLastError();
 }
 

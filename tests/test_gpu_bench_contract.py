@@ -53,7 +53,7 @@ def test_our_arm_json_line():
         loop = d["driver_loop"][name]
         a, b = loop["host_sync_every_check"], loop["device_stop_flag"]
         assert a["sweeps"] == b["sweeps"] and a["wall_ms"] > 0 and b["wall_ms"] > 0
-        assert b["theta"] == a["theta"]                                       # the same loop, bit for bit
+        assert abs(b["theta"] - a["theta"]) <= 1e-9 * a["theta"] + 1e-29      # the same loop (sums grouped differently)
     assert d["value"] > 20 * c["value"]               # the GPU path, not a CPU fallback
 
 

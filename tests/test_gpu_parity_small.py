@@ -212,3 +212,29 @@ def test_autotuner_picks_a_result_equivalent_mapping():
             assert np.abs(f.download() - li.from_real(ref)).max() < TOL_LINK[precision]
         finally:
             culgt.culgt_set_sweep_variant(0)
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 8, 8, 8), (4, 6, 2, 8), (2, 2, 2, 2)])
+@pytest.mark.parametrize("precision,params", SU3_STORES)
+def test_one_kernel_driver_loop_is_the_same_loop(dims, precision, params):
+    """culgt_landau_fix on a small SU(3) lattice runs the whole loop as one cooperative kernel
+    (csrc/fix_persistent.cu: grid barriers between half-sweeps, theta/F reduced inside).  Against the
+    launch-per-half-sweep path (any non-zero product variant selects it): the same number of sweeps, the
+    same links bit for bit, theta and F to rounding -- when it stops on theta and when it runs to
+    max_sweeps, with theta checked every sweep and every third."""
+    u = make(dims, 3, 50)
+    for target, max_sweeps, every in ((1e-6, 300, 1), (1e-6, 300, 3), (0.0, 7, 3)):
+        res = {}
+        for variant in (34, 0):
+            culgt.culgt_set_sweep_variant(variant)
+            try:
+                f = GpuField(dims, 3, precision, params, u)
+                res[variant] = culgt.culgt_landau_fix(f.lat, f.links, f.ws, 1.7, target, max_sweeps, every) + (f.links.clone(),)
+            finally:
+                culgt.culgt_set_sweep_variant(0)
+        (d0, th0, F0, l0), (d1, th1, F1, l1) = res[34], res[0]
+        assert d0 == d1 and (d0 == 7 if target == 0.0 else 0 < d0 < 300), (d0, d1)
+        assert torch.equal(l0, l1)
+        assert abs(th0 - th1) <= 1e-12 * th0 and abs(F0 - F1) <= 1e-13 * abs(F0)
+        if target > 0:
+            assert th1 < target and d1 % every == 0
