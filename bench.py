@@ -474,6 +474,8 @@ def run_sharded(args):
     ws = culgt.alloc_workspace(local)
     sums = torch.zeros(2 * world + 2, dtype=torch.float64, device="cuda")
     scal = torch.zeros(2, dtype=torch.float64, device="cuda")
+    if os.environ.get("NCCL_DEBUG", "").upper() in ("", "VERSION", "WARN"):
+        os.environ["NCCL_DEBUG"] = "NONE"               # at VERSION and WARN NCCL prints a banner on stdout: one JSON line only
     uid = [culgt.culgt_slab_comm_unique_id() if rank == 0 else None]
     if world > 1:
         dist.broadcast_object_list(uid, src=0)

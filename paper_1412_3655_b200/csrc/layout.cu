@@ -7,27 +7,74 @@
 
 namespace culgt {
 
+// two reals as one 8- / 16-byte shared-memory access
+template <typename Real> struct HalfVec;
+template <> struct HalfVec<float> {
+  typedef float2 type;
+  __device__ static __forceinline__ float2 make(float a, float b) { return make_float2(a, b); }
+  __device__ static __forceinline__ void split(const float2& v, float& a, float& b) { a = v.x; b = v.y; }
+};
+template <> struct HalfVec<double> {
+  typedef double2 type;
+  __device__ static __forceinline__ double2 make(double a, double b) { return make_double2(a, b); }
+  __device__ static __forceinline__ void split(const double2& v, double& a, double& b) { a = v.x; b = v.y; }
+};
+
 // A CTA converts TILE consecutive canonical sites (= TILE/2 consecutive half indices h of BOTH
 // parities, 4*TILE links).  The canonical side of the tile is one contiguous run of
 // TILE*4*NFULL reals and moves with coalesced 16-byte accesses through shared memory; the internal
 // side is written / read with consecutive threads on consecutive h of one (parity, mu) plane set.
 // (A thread per link touching its 18 canonical reals directly reached 40 % of the copy rate.)
+//
+// Shared-memory layout: consecutive h are one SITE PAIR = 8*NFULL reals apart (144 reals for SU(3)),
+// a multiple of 32 four-byte banks for every format, so the link threads of a warp would all hit the
+// same banks.  Two reals of padding behind every site pair make the pair stride an odd number of
+// 8-byte (fp32) / 16-byte (fp64) units: the link threads' 64- / 128-bit accesses are conflict-free.
+// A 16-byte canonical vector never straddles a pair, so the copy side only splits it into its two
+// 8-byte halves (fp32) or moves it whole (fp64).
+template <typename S, int TILE>
+struct TileLayout {
+  static constexpr int PAIR = 8 * S::NFULL;                    // reals of one site pair
+  static constexpr int PAD = 2;                                // reals of padding behind it
+  static constexpr int REALS = (TILE / 2) * (PAIR + PAD);
+  __device__ static __forceinline__ int at(int real_index) { return real_index + PAD * (real_index / PAIR); }
+};
+
 template <typename S, bool PACK, int TILE, int BLOCK>
 __global__ void __launch_bounds__(BLOCK)
 layout_tiled_kernel(typename S::Real* __restrict__ canonical, typename S::Vec* __restrict__ links, const Geom g,
                     const long long V) {
   typedef typename S::Real Real;
   typedef typename S::Vec Vec;
+  typedef TileLayout<S, TILE> TL;
+  typedef typename HalfVec<Real>::type HV;
   constexpr int NF = S::NFULL;
+  constexpr int VL = S::VL;                                    // reals per 16-byte vector: 4 or 2
   extern __shared__ __align__(16) unsigned char tile_raw[];
-  Real* tile = reinterpret_cast<Real*>(tile_raw);          // [site in tile][mu][NF]
+  Real* tile = reinterpret_cast<Real*>(tile_raw);              // [site in tile][mu][NF], padded per site pair
   const long long s0 = (long long)blockIdx.x * TILE;
-  const int nsite = (int)((V - s0 < TILE) ? (V - s0) : TILE);   // even: every extent is even
-  const int nvec = nsite * 4 * NF * (int)sizeof(Real) / 16;
-  Vec* tile_v = reinterpret_cast<Vec*>(tile_raw);
+  const int nsite = (int)((V - s0 < TILE) ? (V - s0) : TILE);  // even: every extent is even
+  const int nvec = nsite * 4 * NF / VL;
   Vec* can_v = reinterpret_cast<Vec*>(canonical + s0 * 4 * NF);
+  // one canonical vector <-> its padded place, as 8-byte halves (fp32) or whole (fp64: VL = 2 reals = PAD)
+  auto put = [&](int i, const Vec& v) {
+    Real r[VL];
+    vec_get(v, r);
+    Real* d = tile + TL::at(i * VL);
+#pragma unroll
+    for (int k = 0; k < VL; k += 2) *reinterpret_cast<HV*>(d + k) = HalfVec<Real>::make(r[k], r[k + 1]);
+  };
+  auto get = [&](int i) {
+    Real r[VL];
+    const Real* d = tile + TL::at(i * VL);
+#pragma unroll
+    for (int k = 0; k < VL; k += 2) HalfVec<Real>::split(*reinterpret_cast<const HV*>(d + k), r[k], r[k + 1]);
+    Vec v;
+    vec_set(v, r);
+    return v;
+  };
   if (PACK) {
-    for (int i = threadIdx.x; i < nvec; i += BLOCK) tile_v[i] = can_v[i];
+    for (int i = threadIdx.x; i < nvec; i += BLOCK) put(i, can_v[i]);
     __syncthreads();
   }
   const int h0 = (int)(s0 >> 1);
@@ -39,12 +86,14 @@ layout_tiled_kernel(typename S::Real* __restrict__ canonical, typename S::Vec* _
     if (hl >= nh) continue;
     const int h = h0 + hl;
     const SiteCoord sc = decode_site(g, h, parity);
-    Real* c = tile + ((2 * hl + sc.odd) * 4 + mu) * NF;     // canonical site 2h + odd, local index
+    Real* c = tile + hl * (TL::PAIR + TL::PAD) + (sc.odd * 4 + mu) * NF;   // canonical site 2h + odd, local index
     Vec* lptr = link_base<S>(links, g, parity, mu, h);
     if (PACK) {
       Real m[kLinkRegs];
 #pragma unroll
-      for (int i = 0; i < kLinkRegs; ++i) m[i] = i < NF ? c[i] : (Real)0;   // pad reals stay 0
+      for (int i = 0; i < kLinkRegs; ++i) m[i] = (Real)0;                   // pad reals stay 0
+#pragma unroll
+      for (int i = 0; i < NF; i += 2) HalfVec<Real>::split(*reinterpret_cast<const HV*>(c + i), m[i], m[i + 1]);
       if (S::NC == 3) {
         store_params<S>(lptr, g.pitch, m);              // first NP reals = first NP/6 rows (L118)
       } else {
@@ -58,20 +107,20 @@ layout_tiled_kernel(typename S::Real* __restrict__ canonical, typename S::Vec* _
         load_params<S>(lptr, g.pitch, m);
         if (S::NP == 12) reconstruct_row2(m);
 #pragma unroll
-        for (int i = 0; i < 18; ++i) c[i] = m[i];
+        for (int i = 0; i < 18; i += 2) *reinterpret_cast<HV*>(c + i) = HalfVec<Real>::make(m[i], m[i + 1]);
       } else {
         Real a[4];
         load_params<S>(lptr, g.pitch, a);
-        c[0] = a[0];  c[1] = a[3];     // a0 + i a3
-        c[2] = a[2];  c[3] = a[1];     // a2 + i a1
-        c[4] = -a[2]; c[5] = a[1];     // -a2 + i a1
-        c[6] = a[0];  c[7] = -a[3];    // a0 - i a3
+        *reinterpret_cast<HV*>(c + 0) = HalfVec<Real>::make(a[0], a[3]);     // a0 + i a3
+        *reinterpret_cast<HV*>(c + 2) = HalfVec<Real>::make(a[2], a[1]);     // a2 + i a1
+        *reinterpret_cast<HV*>(c + 4) = HalfVec<Real>::make(-a[2], a[1]);    // -a2 + i a1
+        *reinterpret_cast<HV*>(c + 6) = HalfVec<Real>::make(a[0], -a[3]);    // a0 - i a3
       }
     }
   }
   if (!PACK) {
     __syncthreads();
-    for (int i = threadIdx.x; i < nvec; i += BLOCK) can_v[i] = tile_v[i];
+    for (int i = threadIdx.x; i < nvec; i += BLOCK) can_v[i] = get(i);
   }
 }
 
@@ -79,7 +128,7 @@ template <typename S, bool PACK>
 static cudaError_t launch_layout(void* canonical, void* links, const Geom& g, cudaStream_t st) {
   constexpr int BLOCK = 256;
   constexpr int TILE = (sizeof(typename S::Real) == 8 && S::NC == 3) ? 64 : 128;   // <= 36 KB of shared memory
-  constexpr size_t smem = (size_t)TILE * 4 * S::NFULL * sizeof(typename S::Real);
+  constexpr size_t smem = (size_t)TileLayout<S, TILE>::REALS * sizeof(typename S::Real);
   const long long V = 2ll * g.vh;
   const unsigned grid = (unsigned)((V + TILE - 1) / TILE);
   layout_tiled_kernel<S, PACK, TILE, BLOCK><<<grid, BLOCK, smem, st>>>((typename S::Real*)canonical,
