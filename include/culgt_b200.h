@@ -60,6 +60,7 @@ extern "C" {
 #define CULGT_ERR_CUDA     -7  /* CUDA runtime / launch failure (see culgt_last_cuda_error)    */
 #define CULGT_ERR_ARG      -8  /* another argument is out of range                             */
 #define CULGT_ERR_NCCL     -9  /* NCCL failure, or libnccl.so.2 not found (culgt_last_cuda_error) */
+#define CULGT_ERR_TOO_LARGE -10 /* lattice larger than the no-allocation entry point's built-in scratch */
 
 typedef struct {
   int32_t dims[4];    /* N0..N3, x fastest in the canonical site index                        */
@@ -120,6 +121,23 @@ int culgt_functional(const culgt_lattice* lat, const void* links, void* workspac
  * scalars as above, written to the DEVICE addresses theta_dev and F_dev.  Same workspace. */
 int culgt_gauge_precision_functional(const culgt_lattice* lat, const void* links, void* workspace,
                                      double* theta_dev, double* F_dev, void* stream);
+
+/* a7 + a8 for callers that CANNOT ALLOCATE device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same fused pass, the same kernels and the same bits as
+ * culgt_gauge_precision_functional, without a workspace argument -- the block partials live in a
+ * file-scope device array of the library: 2 MiB, held by every GPU that loads the library until the
+ * process exits.  Limit: V = N0*N1*N2*N3 <= CULGT_NOALLOC_MAX_SITES = 2^24 sites (64^4) in every
+ * storage format; a larger lattice returns CULGT_ERR_TOO_LARGE and launches nothing.  The call
+ * allocates nothing (no cudaMalloc, cudaFree or allocating library routine).  The first call on each
+ * device resolves the array's device address (cudaGetSymbolAddress; no allocation): make it before
+ * starting a stream capture.  All calls on a device share the array, which keeps the last call's
+ * contents; nothing in it has to start at zero (every slot read has been written by the same call).
+ * Calls on one stream are ordered and safe; calls that OVERLAP on the GPU (different streams, no event
+ * between them) race on the array -- do not do that.  theta_dev, F_dev: DEVICE addresses, as above.
+ * Asynchronous on `stream`. */
+#define CULGT_NOALLOC_MAX_SITES (1 << 24)
+int culgt_gauge_precision_functional_noalloc(const culgt_lattice* lat, const void* links, double* theta_dev,
+                                             double* F_dev, void* stream);
 
 /* a9: U_mu(x) <- g(x) U_mu(x) g(x+mu)^dagger for all x, mu (the paper's worked code
  * example P:L105-118).  g: device pointer to a canonical g field (read-only); links in place. */

@@ -24,8 +24,9 @@ CULGT_OK = 0
 ERRORS = {
     "CULGT_ERR_NULL": -1, "CULGT_ERR_DIMS": -2, "CULGT_ERR_DESC": -3, "CULGT_ERR_PARITY": -4,
     "CULGT_ERR_OMEGA": -5, "CULGT_ERR_ALIGN": -6, "CULGT_ERR_CUDA": -7, "CULGT_ERR_ARG": -8,
-    "CULGT_ERR_NCCL": -9,
+    "CULGT_ERR_NCCL": -9, "CULGT_ERR_TOO_LARGE": -10,
 }
+NOALLOC_MAX_SITES = 1 << 24   # CULGT_NOALLOC_MAX_SITES
 FLOPS_PER_SITE = {3: 2304, 2: 278}   # fixed algorithmic counts, DESIGN.md "Measurement"
 
 
@@ -72,6 +73,7 @@ def lib() -> ctypes.CDLL:
     L.culgt_gauge_precision.argtypes = [latp, vp, vp, vp, vp]
     L.culgt_functional.argtypes = [latp, vp, vp, vp, vp]
     L.culgt_gauge_precision_functional.argtypes = [latp, vp, vp, vp, vp, vp]
+    L.culgt_gauge_precision_functional_noalloc.argtypes = [latp, vp, vp, vp, vp]
     L.culgt_gauge_transform.argtypes = [latp, vp, vp, vp]
     L.culgt_landau_fix.argtypes = [latp, vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                    ctypes.c_int, ctypes.POINTER(ctypes.c_int), dp, dp, vp]
@@ -276,6 +278,15 @@ def culgt_gauge_precision_functional(lat: Lattice, links, workspace, theta_dev, 
     _check(lib().culgt_gauge_precision_functional(ctypes.byref(lat.c()), _ptr(links), _ptr(workspace),
                                                   _ptr(theta_dev), _ptr(F_dev), _stream(stream)),
            "culgt_gauge_precision_functional")
+
+
+def culgt_gauge_precision_functional_noalloc(lat: Lattice, links, theta_dev, F_dev, stream=None) -> None:
+    """theta and F without a workspace: the partials live in a 2 MiB device array of the library
+    (at most NOALLOC_MAX_SITES sites); allocates nothing."""
+    _require_cuda()
+    _check(lib().culgt_gauge_precision_functional_noalloc(ctypes.byref(lat.c()), _ptr(links), _ptr(theta_dev),
+                                                          _ptr(F_dev), _stream(stream)),
+           "culgt_gauge_precision_functional_noalloc")
 
 
 def culgt_gauge_transform(lat: Lattice, links, g, stream=None) -> None:

@@ -202,6 +202,24 @@ int culgt_gauge_precision_functional(const culgt_lattice* lat, const void* links
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
+// theta and F for callers that cannot allocate: no workspace argument, the block partials live in a 2 MiB
+// file-scope device array of the library (csrc/reduce.cu).
+int culgt_gauge_precision_functional_noalloc(const culgt_lattice* lat, const void* links, double* theta_dev,
+                                             double* F_dev, void* stream) {
+  LatticeDesc d;
+  int rc = describe(lat, &d);
+  if (rc != CULGT_OK) return rc;
+  if (!links || !theta_dev || !F_dev) return CULGT_ERR_NULL;
+  if (misaligned(links)) return CULGT_ERR_ALIGN;
+  if ((long long)d.V > (long long)CULGT_NOALLOC_MAX_SITES) return CULGT_ERR_TOO_LARGE;
+  cudaError_t e = launch_theta_functional_noalloc(d, links, theta_dev, F_dev, (cudaStream_t)stream);
+  if (e == cudaErrorMemoryAllocation) {          // the launcher's own size check (never an allocation failure)
+    cudaGetLastError();
+    return CULGT_ERR_TOO_LARGE;
+  }
+  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
+}
+
 // theta and F (one fused pass) into the first two result slots of the workspace, read back.
 static int read_theta_F(const LatticeDesc& d, const void* links, void* workspace, cudaStream_t st,
                         double* theta, double* F) {
@@ -968,6 +986,7 @@ const char* culgt_strerror(int status) {
     case CULGT_ERR_CUDA: return "CUDA error (see culgt_last_cuda_error)";
     case CULGT_ERR_ARG: return "argument out of range";
     case CULGT_ERR_NCCL: return "NCCL error (see culgt_last_cuda_error)";
+    case CULGT_ERR_TOO_LARGE: return "lattice exceeds the built-in scratch of the no-allocation entry point (at most 2^24 sites)";
     default: return "unknown status";
   }
 }

@@ -149,6 +149,11 @@ struct FixCheck {
 cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
                                     double* out_theta, double* out_F, cudaStream_t st,
                                     const FixCheck* fix = nullptr);
+// the same pass with the block partials in the library's own file-scope device array (reduce.cu): allocates
+// nothing; cudaErrorMemoryAllocation when the lattice needs more partials than the array holds
+size_t noalloc_partials_needed(const LatticeDesc& d);
+cudaError_t launch_theta_functional_noalloc(const LatticeDesc& d, const void* links, double* out_theta, double* out_F,
+                                            cudaStream_t st);
 // Coulomb gauge: per-slice theta_t, F_t (N3 doubles each)
 cudaError_t launch_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
                                             double* out_theta_t, double* out_F_t, cudaStream_t st);

@@ -356,4 +356,46 @@ cudaError_t launch_coulomb_theta_functional(const LatticeDesc& d, const void* li
   CULGT_DISPATCH(run_coulomb_theta_functional, d, links, workspace, out_theta_t, out_F_t, st)
 }
 
+// ---------------------------------------------------------------------------------------------------
+// theta + F for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses
+// that forbid cudaMalloc): the same fused pass and the same kernels as launch_theta_functional, but the
+// block partials live in a file-scope device array instead of a caller-supplied workspace.
+//   * kNoAllocPartials doubles = 2 MiB, held by every GPU that loads the library until the process
+//     exits.  It covers 2 quantities x V/128 partials (V/64 for fp32 12-parameter storage) up to
+//     V = 2^24 sites (64^4) in every storage format; larger lattices are refused.
+//   * In host code `g_noalloc_partials` is a host-side stand-in, NOT a device address: the device
+//     address is resolved once per device, with that device current, by cudaGetSymbolAddress, and that
+//     pointer is what the kernels get.
+//   * Nothing in the array has to start at zero: every slot the final sum reads has been written by
+//     the partial kernel of the same call, so the previous call's contents are simply overwritten.
+//   * Every call on a device shares the array: two calls that overlap on the GPU (different streams)
+//     race on it.  Calls on one stream are ordered and safe.
+// No cudaMalloc / cudaFree / allocating library routine is called here or below.
+// ---------------------------------------------------------------------------------------------------
+constexpr size_t kNoAllocPartials = (size_t)1 << 18;                 // doubles: 2 MiB
+static __device__ __align__(256) double g_noalloc_partials[kNoAllocPartials];
+
+size_t noalloc_partials_needed(const LatticeDesc& d) {
+  const bool staged = d.group == 3 && d.precision == 32 && d.params == 12;      // theta_is_staged
+  return 2 * (size_t)reduce_blocks_fused(d.geom.vh, staged ? 64 : 128);
+}
+
+cudaError_t launch_theta_functional_noalloc(const LatticeDesc& d, const void* links, double* out_theta, double* out_F,
+                                            cudaStream_t st) {
+  if (noalloc_partials_needed(d) > kNoAllocPartials) return cudaErrorMemoryAllocation;   // mapped to CULGT_ERR_TOO_LARGE
+  static double* scratch[kMaxDevices] = {nullptr};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  if (scratch[dev] == nullptr) {                 // set-up, once per device, with that device current
+    double* ptr = nullptr;
+    e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_partials);
+    if (e != cudaSuccess) return e;
+    if (ptr == nullptr) return cudaErrorInvalidSymbol;
+    scratch[dev] = ptr;
+  }
+  return launch_theta_functional(d, links, scratch[dev], out_theta, out_F, st, nullptr);
+}
+
 }  // namespace culgt
