@@ -215,8 +215,10 @@ int culgt_sa_anneal_micro(const culgt_lattice* lat, void* links, double T_max, d
  * culgt_or_sweep_coulomb_masked: the half-sweep over the time-slices t with slice_active_dev[t] != 0
  *   only (DEVICE array of dims[3] bytes); slices decouple, so frozen slices keep their spatial links.
  * culgt_coulomb_fix: every slice is swept until ITS theta_t < theta_target (checked every
- *   check_every sweeps; converged slices are frozen, the others go on) or max_sweeps; SYNCHRONISES
- *   at each check; sweeps_done = sweeps of the slowest slice; theta_t_out / F_t_out: HOST arrays of
+ *   check_every sweeps; converged slices are frozen, the others go on) or max_sweeps.  As in
+ *   culgt_landau_fix the decisions are taken on the device (the mask is recomputed by the check, a stop
+ *   word raised when no slice is active) and the host synchronises once per batch of checks;
+ *   SYNCHRONISES; sweeps_done = sweeps of the slowest slice; theta_t_out / F_t_out: HOST arrays of
  *   dims[3] doubles (may be NULL). */
 int culgt_or_sweep_coulomb(const culgt_lattice* lat, void* links, int parity, double omega, void* stream);
 int culgt_or_sweeps_coulomb(const culgt_lattice* lat, void* links, int n_sweeps, double omega, void* stream);

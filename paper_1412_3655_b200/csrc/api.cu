@@ -500,19 +500,9 @@ int culgt_coulomb_precision_functional(const culgt_lattice* lat, const void* lin
   return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
 }
 
-// theta_t and F_t of every slice through the result slots of the workspace into host[0..2*N3)
-// (synchronises).
-static int read_coulomb(const LatticeDesc& d, const void* links, void* workspace, cudaStream_t st, double* host) {
-  const int n3 = d.geom.n[3];
-  double* ws = (double*)workspace;
-  double* res = ws + reduce_partial_doubles(d.geom);
-  cudaError_t e = launch_coulomb_theta_functional(d, links, ws, res, res + n3, st);
-  if (e != cudaSuccess) return cuda_fail(e);
-  e = cudaMemcpyAsync(host, res, 2 * (size_t)n3 * sizeof(double), cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  return e == cudaSuccess ? CULGT_OK : cuda_fail(e);
-}
-
+// As culgt_landau_fix, the stopping decision is taken on the device: every check recomputes the per-slice
+// activity mask from theta_t (coulomb_mask_kernel) and raises the stop word when no slice is active; the
+// host reads the control block and the 2*N3 results back once per batch of rounds.
 int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, double omega,
                       double theta_target, int max_sweeps, int check_every, int* sweeps_done,
                       double* theta_t_out, double* F_t_out, void* stream) {
@@ -525,34 +515,38 @@ int culgt_coulomb_fix(const culgt_lattice* lat, void* links, void* workspace, do
   if ((rc = check_omega(omega)) != CULGT_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   const int n3 = d.geom.n[3];
+  double* ws = (double*)workspace;
+  double* res = ws + reduce_partial_doubles(d.geom);                 // theta_t[N3], F_t[N3]
+  unsigned char* mask_dev = (unsigned char*)(res + 2 * (size_t)n3);  // the per-slice activity mask behind them
+  FixCtl* ctl = (FixCtl*)(ws + fix_ctl_offset_doubles(d.geom));
+  cudaError_t e = cudaMemsetAsync(ctl, 0, sizeof(FixCtl), st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  CoulombCheck chk = {ctl, mask_dev, theta_target, 0};
+  if ((e = launch_coulomb_theta_functional(d, links, ws, res, res + n3, st, &chk)) != cudaSuccess) return cuda_fail(e);
+  LatticeDesc dm = d;
+  dm.geom.slice_active = mask_dev;
+  const int rounds_per_sync = check_every >= 32 ? 1 : 32 / check_every;
   std::vector<double> host(2 * (size_t)n3);
-  std::vector<unsigned char> active((size_t)n3, 1);
-  // the per-slice activity mask lives behind the result slots of the workspace
-  unsigned char* mask_dev = (unsigned char*)((double*)workspace + reduce_partial_doubles(d.geom) + 2 * (size_t)n3);
-  int done = 0;
+  FixCtl hc;
+  int enqueued = 0;
   for (;;) {
-    if ((rc = read_coulomb(d, links, workspace, st, host.data())) != CULGT_OK) return rc;
-    // slices decouple: a slice whose theta_t is below the target stops, the others go on
-    int n_active = 0;
-    for (int t = 0; t < n3; ++t) {
-      active[t] = !(host[t] < theta_target);          // NaN keeps a slice active until max_sweeps
-      n_active += active[t];
+    for (int r = 0; r < rounds_per_sync && enqueued < max_sweeps; ++r) {
+      int n = check_every;
+      if (enqueued + n > max_sweeps) n = max_sweeps - enqueued;
+      for (int i = 0; i < n; ++i)
+        for (int parity = 0; parity < 2; ++parity)
+          if ((e = launch_or_sweep(dm, links, parity, omega, 0, st, true, &ctl->stop)) != cudaSuccess) return cuda_fail(e);
+      enqueued += n;
+      chk.sweeps_before = enqueued;
+      if ((e = launch_coulomb_theta_functional(d, links, ws, res, res + n3, st, &chk)) != cudaSuccess) return cuda_fail(e);
     }
-    if (n_active == 0 || done >= max_sweeps) break;
-    cudaError_t e = cudaMemcpyAsync(mask_dev, active.data(), (size_t)n3, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return cuda_fail(e);
-    LatticeDesc dm = d;
-    dm.geom.slice_active = mask_dev;
-    int n = check_every;
-    if (done + n > max_sweeps) n = max_sweeps - done;
-    for (int i = 0; i < n; ++i)
-      for (int parity = 0; parity < 2; ++parity) {
-        e = launch_or_sweep(dm, links, parity, omega, 0, st, true);
-        if (e != cudaSuccess) return cuda_fail(e);
-      }
-    done += n;
+    if ((e = cudaMemcpyAsync(&hc, ctl, sizeof(FixCtl), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(host.data(), res, 2 * (size_t)n3 * sizeof(double), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+      return cuda_fail(e);
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+    if (hc.stop || enqueued >= max_sweeps) break;
   }
-  if (sweeps_done) *sweeps_done = done;
+  if (sweeps_done) *sweeps_done = hc.stop ? hc.sweeps_at_stop : enqueued;
   for (int t = 0; t < n3; ++t) {
     if (theta_t_out) theta_t_out[t] = host[t];
     if (F_t_out) F_t_out[t] = host[n3 + t];

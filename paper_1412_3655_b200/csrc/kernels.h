@@ -26,7 +26,7 @@ inline int reduce_blocks_fused(int vh, int half = 64) { return (vh + half - 1) /
 // slice/128; never below 4096) followed by 2 * N3 result slots that the *_host / *_fix paths
 // read back (Landau uses the first two).
 inline size_t reduce_partial_doubles(const Geom& g) {
-  size_t n = 2 * (size_t)reduce_blocks_fused(g.vh) + 8;      // + 8: the 4-threads-per-site kernel rounds per parity
+  size_t n = 2 * (size_t)reduce_blocks_fused(g.vh) + 8;      // + 8 spare slots
   const size_t c = 2 * (size_t)g.n[3] * (size_t)reduce_blocks_fused(g.stride[3]);
   if (c > n) n = c;
   return n > 4096 ? n : 4096;
@@ -154,9 +154,18 @@ cudaError_t launch_theta_functional(const LatticeDesc& d, const void* links, dou
 size_t noalloc_partials_needed(const LatticeDesc& d);
 cudaError_t launch_theta_functional_noalloc(const LatticeDesc& d, const void* links, double* out_theta, double* out_F,
                                             cudaStream_t st);
-// Coulomb gauge: per-slice theta_t, F_t (N3 doubles each)
+// Coulomb gauge: per-slice theta_t, F_t (N3 doubles each).  chk (may be null): driver-loop bookkeeping on
+// the device -- the per-slice activity mask is recomputed from theta_t, the stop word raised when no slice
+// is active; the pass is skipped when the stop word is already set.
+struct CoulombCheck {
+  FixCtl* ctl;
+  unsigned char* mask;   // N3 bytes, device
+  double theta_target;
+  int sweeps_before;
+};
 cudaError_t launch_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
-                                            double* out_theta_t, double* out_F_t, cudaStream_t st);
+                                            double* out_theta_t, double* out_F_t, cudaStream_t st,
+                                            const CoulombCheck* chk = nullptr);
 cudaError_t launch_gauge_transform(const LatticeDesc& d, void* links, const void* g, cudaStream_t st);
 
 // ---- time-slab decomposition (slab.cu) ------------------------------------------------------------------

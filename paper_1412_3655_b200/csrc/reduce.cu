@@ -196,7 +196,8 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
 template <int BLOCK>
 __global__ void __launch_bounds__(BLOCK)
 final_sum_kernel(const double* __restrict__ partial, int n, double scale0, double scale1,
-                 double* __restrict__ out0, double* __restrict__ out1) {
+                 double* __restrict__ out0, double* __restrict__ out1, const int* __restrict__ stop_flag) {
+  if (stop_flag != nullptr && *stop_flag != 0) return;   // driver loop has stopped: keep the last results
   const double* p = partial + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * (size_t)n;
   double acc = 0;
   for (int i = threadIdx.x; i < n; i += BLOCK) acc += p[i];
@@ -204,6 +205,31 @@ final_sum_kernel(const double* __restrict__ partial, int n, double scale0, doubl
   if (threadIdx.x == 0) {
     if (blockIdx.y == 0) out0[blockIdx.x] = s * scale0;
     else out1[blockIdx.x] = s * scale1;
+  }
+}
+
+// Coulomb driver loop on the device (culgt_coulomb_fix): after a check, slice t stays active iff NOT
+// theta_t < target (a NaN keeps it active); when no slice is active the stop word is raised and every
+// sweep and check enqueued behind it returns at entry.  Slices decouple (reading C-22), so a frozen
+// slice's theta_t never changes again.
+__global__ void coulomb_mask_kernel(const double* __restrict__ theta_t, int n3, double target,
+                                    unsigned char* __restrict__ mask, FixCtl* __restrict__ ctl, int sweeps_before) {
+  if (ctl->stop != 0) return;
+  __shared__ int any_active;
+  if (threadIdx.x == 0) any_active = 0;
+  __syncthreads();
+  for (int t = threadIdx.x; t < n3; t += blockDim.x) {
+    const bool active = !(theta_t[t] < target);
+    mask[t] = active ? 1 : 0;
+    if (active) any_active = 1;            // benign race: every writer stores 1
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    ctl->checks_done += 1;
+    if (!any_active) {
+      ctl->sweeps_at_stop = sweeps_before;
+      ctl->stop = 1;
+    }
   }
 }
 
@@ -307,14 +333,18 @@ static cudaError_t run_theta_functional(const LatticeDesc& d, const void* links,
 // Coulomb gauge: theta_t and F_t for every time-slice t (arrays of N3 doubles).
 template <typename S>
 static cudaError_t run_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* ws,
-                                                double* out_theta_t, double* out_F_t, cudaStream_t st) {
+                                                double* out_theta_t, double* out_F_t, cudaStream_t st,
+                                                const CoulombCheck* chk) {
   const int n3 = d.geom.n[3];
   int nbx = 0;
-  cudaError_t e = launch_theta_pass<S, true>(d.geom.stride[3], n3, links, d.geom, ws, nullptr, st, &nbx);
+  const int* stop = chk ? &chk->ctl->stop : nullptr;
+  cudaError_t e = launch_theta_pass<S, true>(d.geom.stride[3], n3, links, d.geom, ws, stop, st, &nbx);
   if (e != cudaSuccess) return e;
   const double vs = (double)d.V / (double)n3;
   final_sum_kernel<kReduceBlock><<<dim3(n3, 2), kReduceBlock, 0, st>>>(
-      ws, nbx, 1.0 / ((double)S::NC * vs), 1.0 / (3.0 * S::NC * vs), out_theta_t, out_F_t);
+      ws, nbx, 1.0 / ((double)S::NC * vs), 1.0 / (3.0 * S::NC * vs), out_theta_t, out_F_t, stop);
+  if ((e = cudaGetLastError()) != cudaSuccess || chk == nullptr) return e;
+  coulomb_mask_kernel<<<1, 128, 0, st>>>(out_theta_t, n3, chk->theta_target, chk->mask, chk->ctl, chk->sweeps_before);
   return cudaGetLastError();
 }
 
@@ -352,8 +382,9 @@ cudaError_t launch_theta_functional_sums(const LatticeDesc& d, const void* links
 }
 
 cudaError_t launch_coulomb_theta_functional(const LatticeDesc& d, const void* links, double* workspace,
-                                            double* out_theta_t, double* out_F_t, cudaStream_t st) {
-  CULGT_DISPATCH(run_coulomb_theta_functional, d, links, workspace, out_theta_t, out_F_t, st)
+                                            double* out_theta_t, double* out_F_t, cudaStream_t st,
+                                            const CoulombCheck* chk) {
+  CULGT_DISPATCH(run_coulomb_theta_functional, d, links, workspace, out_theta_t, out_F_t, st, chk)
 }
 
 // ---------------------------------------------------------------------------------------------------
