@@ -137,6 +137,8 @@ class ClockSampler:
             self.nv = pynvml
             self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
             self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            pynvml.nvmlDeviceGetClockInfo(self.h, pynvml.NVML_CLOCK_SM)          # warm the query path (slow the first time)
+            pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
         except Exception:
             self.nv = None
 
@@ -308,8 +310,10 @@ def time_sweep_loop(torch, field, sweeps, check, steps, warmup, check_every, bar
     check()
     barrier()
 
-    def roll_until(t_end):
-        while time.perf_counter() < t_end:
+    def roll_until(t_end, min_samples, t_cap):
+        # keep the GPU under the same load until the time has passed AND NVML has answered often enough
+        # (the first NVML queries of a process on a fresh box can take tens of milliseconds each)
+        while (time.perf_counter() < t_end or len(sampler.samples) < min_samples) and time.perf_counter() < t_cap:
             sweeps(8)
             torch.cuda.synchronize()
 
@@ -318,7 +322,7 @@ def time_sweep_loop(torch, field, sweeps, check, steps, warmup, check_every, bar
     t_start = time.perf_counter()
     if sampler is not None:
         sampler.start()
-        roll_until(t_start + 0.4e-3 * window_ms)
+        roll_until(t_start + 0.4e-3 * window_ms, 2 if sampler.nv is not None else 0, t_start + 1.5)
     ev0.record(stream)
     done = 0
     while done < steps:
@@ -333,7 +337,7 @@ def time_sweep_loop(torch, field, sweeps, check, steps, warmup, check_every, bar
     ev1.record(stream)
     if sampler is not None:
         torch.cuda.synchronize()
-        roll_until(t_start + 1e-3 * window_ms)
+        roll_until(t_start + 1e-3 * window_ms, 6 if sampler.nv is not None else 0, t_start + 4.0)
     barrier()
     clocks = sampler.stop() if sampler is not None else None
     elapsed_ms = ev0.elapsed_time(ev1)
