@@ -7,6 +7,7 @@
 // one partial per block in the workspace -> a single block per quantity sums the partials in a
 // fixed order.  Deterministic: no atomics, the same launch always produces the same bits.
 // All arithmetic is fp64 on the stored values (12-parameter storage: third row rebuilt in fp64).
+#include <stdlib.h>
 #include "lattice.cuh"
 #include "su_math.cuh"
 #include "kernels.h"
@@ -92,7 +93,8 @@ __device__ __forceinline__ double theta_from_parts(const double* a) {
 // Measured and rejected: four threads per site with the parts exchanged through shared
 // memory (commit 7e9a7e2: 72 us against 59 at 32^4 fp32-12 -- a third of the bytes in flight per SM),
 // part of the fp32 -> fp64 conversions moved from the XU to the integer pipe (no change: the kernel is
-// not bound by a pipe), staging through the L1 with cp.async.ca (82 us).
+// not bound by a pipe), staging through the L1 with cp.async.ca (82 us), a 4-D site tile per CTA in which
+// every link is fetched and converted once (theta_functional_tile_kernel below: 79 us).
 template <typename S, int BLOCK, bool COULOMB, bool STAGED>
 __global__ void __launch_bounds__(BLOCK, STAGED ? 512 / BLOCK : 0)
 theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
@@ -189,6 +191,110 @@ theta_functional_kernel(const typename S::Vec* __restrict__ links, const Geom g,
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------------
+// Landau gauge, SU(3): a 4-D SITE TILE per CTA, every link widened and reduced ONCE.
+//
+// theta needs, per site, the anti-Hermitian parts (9 reals, add_antihermitian_parts) of its 4 up links
+// minus those of its 4 down links; a link is the up link of one site and the down link of the
+// neighbouring site of the other parity.  The kernels above fetch and widen it twice.  Here a CTA owns
+// the TX x T1 x T2 x T3 block of half indices (hx, x1, x2, x3) of BOTH parities (2*NT sites, one thread
+// each): a thread loads its 4 up links, reduces each to its 9 reals, keeps them for its own sum and
+// parks them in shared memory ([component][parity*4+mu][site], conflict-free); after one barrier it
+// subtracts the parts of its down links, which its neighbours parked -- except on the tile's lower
+// faces, where the down link belongs to another tile and is fetched and reduced directly (issued with
+// the up links, before the barrier).  Link fetches per site: 4 + (1/(2 TX) + 1/T1 + 1/T2 + 1/T3)
+// instead of 8; conversions and third-row rebuilds likewise.  Threads are ordered hx-fastest, so a
+// warp reads runs of TX consecutive vectors of a plane.
+// Requires nh0 % TX == 0, N1 % T1 == 0, N2 % T2 == 0, N3 % T3 == 0 (else the kernels above).
+// ---------------------------------------------------------------------------------------------------
+#ifdef CULGT_MEASURE
+template <typename S>
+__device__ __forceinline__ double link_parts(const typename S::Real* U, double* pr) {
+#pragma unroll
+  for (int c = 0; c < 9; ++c) pr[c] = 0;
+  return add_antihermitian_parts<S>(U, 1.0, pr);
+}
+
+template <typename S, int TX, int T1, int T2, int T3, int MINB>
+__global__ void __launch_bounds__(2 * TX * T1 * T2 * T3, MINB)
+theta_functional_tile_kernel(const typename S::Vec* __restrict__ links, const Geom g, const int nbx, const int nb1,
+                             const int nb2, double* __restrict__ partial_theta, double* __restrict__ partial_F,
+                             const int* __restrict__ stop_flag) {
+  typedef typename S::Real Real;
+  constexpr int NT = TX * T1 * T2 * T3;          // sites of one parity per tile
+  if (stop_flag != nullptr && *stop_flag != 0) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* const parts = reinterpret_cast<double*>(smem_raw);      // [9][8 * NT]
+  // tile origin
+  int b = (int)blockIdx.x;
+  const int bx = b % nbx; b /= nbx;
+  const int b1 = b % nb1; b /= nb1;
+  const int b2 = b % nb2;
+  const int b3 = b / nb2;
+  // my site
+  const int p = (int)threadIdx.x / NT;
+  const int lh = (int)threadIdx.x % NT;
+  const int lhx = lh % TX, l1 = (lh / TX) % T1, l2 = (lh / (TX * T1)) % T2, l3 = lh / (TX * T1 * T2);
+  SiteCoord sc;
+  sc.hx = bx * TX + lhx;
+  sc.x1 = b1 * T1 + l1;
+  sc.x2 = b2 * T2 + l2;
+  sc.x3 = b3 * T3 + l3;
+  sc.odd = (sc.x1 + sc.x2 + sc.x3 + p) & 1;
+  const int h = sc.hx + g.nh0 * (sc.x1 + g.n[1] * (sc.x2 + g.n[2] * sc.x3));
+  // local index of the down neighbour inside the tile, or -1 when it belongs to another tile
+  int nb_local[4];
+  nb_local[0] = sc.odd ? lh : (lhx > 0 ? lh - 1 : -1);
+  nb_local[1] = l1 > 0 ? lh - TX : -1;
+  nb_local[2] = l2 > 0 ? lh - TX * T1 : -1;
+  nb_local[3] = l3 > 0 ? lh - TX * T1 * T2 : -1;
+
+  double a[9];
+#pragma unroll
+  for (int c = 0; c < 9; ++c) a[c] = 0;
+  double f = 0;
+  // all loads first: the 4 up links, and the down links that come from outside the tile
+  Real Uu[4][kLinkRegs];
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) load_params<S>(link_base<S>(links, g, p, mu, h), g.pitch, Uu[mu]);
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) {
+    if (nb_local[mu] < 0) {
+      Real Ud[kLinkRegs];
+      load_params<S>(link_base<S>(links, g, 1 - p, mu, down_index(g, h, sc, mu)), g.pitch, Ud);
+      add_antihermitian_parts<S>(Ud, -1.0, a);
+    }
+  }
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) {
+    double pr[9];
+    f += link_parts<S>(Uu[mu], pr);
+#pragma unroll
+    for (int c = 0; c < 9; ++c) {
+      a[c] += pr[c];
+      parts[(c * 8 + p * 4 + mu) * NT + lh] = pr[c];
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) {
+    if (nb_local[mu] >= 0) {
+#pragma unroll
+      for (int c = 0; c < 9; ++c) a[c] -= parts[(c * 8 + (1 - p) * 4 + mu) * NT + nb_local[mu]];
+    }
+  }
+  const double th = theta_from_parts(a);
+  __syncthreads();
+  const double st = block_sum<2 * NT>(th);
+  __syncthreads();                       // block_sum's shared slots are reused
+  const double sf = block_sum<2 * NT>(f);
+  if (threadIdx.x == 0) {
+    partial_theta[blockIdx.x] = st;
+    partial_F[blockIdx.x] = sf;
+  }
+}
+#endif  // CULGT_MEASURE
 
 // Final pass of the per-slice (Coulomb) sums: block (group, quantity) sums the n partials of that group
 // in a fixed order and scales.  partial = [quantity][group][n]; quantity 0 = theta, 1 = F; group = time-slice for the
@@ -296,6 +402,23 @@ static cudaError_t launch_theta_staged(dim3 grid, const void* links, const Geom&
 // fp32 12-parameter storage takes the staged kernel, 64 sites of each parity per 128-thread CTA, 4 CTAs
 // per SM (measured at 32^4: 67 -> 60 us per check inside the sweep loop, 91 -> 56 us back to back;
 // DESIGN.md 6.3); the other formats the register path with 128 sites of each parity per CTA.
+// The 4-D tile kernel (theta_functional_tile_kernel) was measured and rejected (78.7 us
+// against 57.5 us at 32^4 fp32-12, 697 against 482 us at 48^3 x 96): it fetches 5.3 instead of 8 links per
+// site and converts each once, but keeps only a third of the bytes in flight per SM.  It is compiled only
+// into the measurement build, where CULGT_THETA_TILE=1 selects it.
+static bool theta_tile_enabled() {
+#ifdef CULGT_MEASURE
+  static int v = -1;
+  if (v < 0) {
+    const char* e = getenv("CULGT_THETA_TILE");
+    v = e ? (e[0] != '0') : 0;
+  }
+  return v != 0;
+#else
+  return false;
+#endif
+}
+
 template <typename S>
 static constexpr bool theta_is_staged() { return S::NC == 3 && S::NP == 12 && sizeof(typename S::Real) == 4; }
 
@@ -304,6 +427,29 @@ static constexpr bool theta_is_staged() { return S::NC == 3 && S::NP == 12 && si
 template <typename S, bool COULOMB>
 static cudaError_t launch_theta_pass(int group_size, int ny, const void* links, const Geom& g, double* p_theta,
                                      const int* stop_flag, cudaStream_t st, int* blocks_out) {
+#ifdef CULGT_MEASURE
+  if constexpr (!COULOMB && S::NC == 3 && sizeof(typename S::Real) == 4 && S::NP == 12) {
+    constexpr int TX = 8, T1 = 4, T2 = 2, T3 = 2, NT = TX * T1 * T2 * T3, MINB = 2;
+    if (theta_tile_enabled() && g.nh0 % TX == 0 && g.n[1] % T1 == 0 && g.n[2] % T2 == 0 && g.n[3] % T3 == 0) {
+      auto kern = theta_functional_tile_kernel<S, TX, T1, T2, T3, MINB>;
+      constexpr size_t smem = (size_t)9 * 8 * NT * sizeof(double);
+      static bool configured[kMaxDevices] = {false};
+      int dev = 0;
+      cudaError_t e = cudaGetDevice(&dev);
+      if (e != cudaSuccess) return e;
+      if (dev < 0 || dev >= kMaxDevices || !configured[dev]) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < kMaxDevices) configured[dev] = true;
+      }
+      const int nbx = g.nh0 / TX, nb1 = g.n[1] / T1, nb2 = g.n[2] / T2, nb3 = g.n[3] / T3;
+      const int nb = nbx * nb1 * nb2 * nb3;             // = vh / NT
+      *blocks_out = nb;
+      kern<<<nb, 2 * NT, smem, st>>>((const typename S::Vec*)links, g, nbx, nb1, nb2, p_theta, p_theta + nb, stop_flag);
+      return cudaGetLastError();
+    }
+  }
+#endif
   const int nb = reduce_blocks_fused(group_size, theta_is_staged<S>() ? 64 : 128);
   *blocks_out = nb;
   double* p_F = p_theta + (size_t)ny * nb;
