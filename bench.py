@@ -387,6 +387,34 @@ def other_kernels(culgt, torch, f, peak):
     return out
 
 
+def sweep_variants(culgt, torch, f, peak, steps):
+    """The widening steps of the path at the workload of `f`: us per half-sweep of the
+    Coulomb-gauge, truncated-series, microcanonical and simulated-annealing sweeps (same loads, stores and
+    link products as the overrelaxation sweep; only the per-subgroup update differs), algorithmic GB/s."""
+    lat, links, omega = f.lat, f.links, f.omega
+    runs = {
+        "coulomb": lambda n: culgt.culgt_or_sweeps_coulomb(lat, links, n, omega),
+        "series_order_4": lambda n: culgt.culgt_or_sweeps_series(lat, links, n, omega, 4),
+        "microcanonical": lambda n: culgt.culgt_micro_sweeps(lat, links, n),
+        "annealing_T_0.1": lambda n: culgt.culgt_sa_anneal(lat, links, 0.1, 0.1, n, 2024),
+        "annealing_T_2": lambda n: culgt.culgt_sa_anneal(lat, links, 2.0, 2.0, n, 2024),
+    }
+    out = {}
+    stream = torch.cuda.current_stream()
+    for name, run in runs.items():
+        culgt.culgt_pack(lat, f.can_dev, links)           # every variant starts from the same stored field
+        run(3)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        run(steps)
+        b.record(stream)
+        torch.cuda.synchronize()
+        us = 1e3 * a.elapsed_time(b) / (2 * steps)
+        gbs = 2 * f.field_bytes / (us * 1e-6) / 1e9
+        out[name] = {"half_sweep_us": us, "value": f.V * steps / (a.elapsed_time(b) * 1e-3), "gbs": gbs, "frac": gbs / peak}
+    return out
+
+
 def driver_loop_times(culgt, torch, rank):
     """The paper's driver loop on the latency-bound BASELINE.json configs[0..2]: wall time of
     culgt_landau_fix (stopping decision on the device, one host synchronisation per batch of checks)
@@ -671,10 +699,12 @@ def main():
                "theta": th_e, "F": F_e}
 
     # ---- the other kernels of the path at this workload; the other BASELINE.json workloads; the driver loop
-    kernels = extra = loops = None
+    kernels = extra = loops = variants = None
     extra_names = (args.extra_workloads.split(",") if args.extra_workloads
                    else ["cfg3_fp64", "cfg4_fp32", "cfg4_fp64"] if args.workload == "cfg3_fp32" else [])
     if world == 1 and not args.no_extra and plain_or and extra_names:
+        culgt.culgt_unpack(lat, links, f.can_dev)        # the gauge-fixed field, as the canonical input of what follows
+        variants = sweep_variants(culgt, torch, f, peak, max(args.extra_steps, 10))
         kernels = other_kernels(culgt, torch, f, peak)
         del f, links, ws
         torch.cuda.empty_cache()
@@ -697,6 +727,7 @@ def main():
                 "theta_F": {"us": chk_us, "gbs": fx.field_bytes / (chk_us * 1e-6) / 1e9,
                             "frac": fx.field_bytes / (chk_us * 1e-6) / 1e9 / peak},
                 "clocks": tx["clocks"], "final": {"theta": float(sx[0].item()), "F": float(sx[1].item())},
+                "kernels": other_kernels(culgt, torch, fx, peak) if fx.V <= 32 ** 4 else None,
             })
             del fx, sx
             torch.cuda.empty_cache()
@@ -748,7 +779,7 @@ def main():
             "clocks": clocks,
             "final": {"theta": theta, "F": F},
             "check_ms_total": check_ms, "variant": args.variant,
-            "kernels": kernels, "extra_workloads": extra, "driver_loop": loops,
+            "kernels": kernels, "sweep_variants": variants, "extra_workloads": extra, "driver_loop": loops,
             "context": {"paper": "470 GFlops at 80% of peak bandwidth on a GeForce GTX 580 (PAPER.md L7), context only"},
         }
         print(json.dumps(line), flush=True)

@@ -46,6 +46,8 @@ def test_our_arm_json_line():
     # the other kernels of the path, the other workloads and the driver loop ride on the same line
     for k in ("theta_F", "pack", "unpack", "gauge_transform"):
         assert d["kernels"][k]["us"] > 0 and 0 < d["kernels"][k]["frac"] < 2
+    for k in ("coulomb", "series_order_4", "microcanonical", "annealing_T_0.1", "annealing_T_2"):
+        assert d["sweep_variants"][k]["half_sweep_us"] > 0 and d["sweep_variants"][k]["value"] > 0
     (x,) = d["extra_workloads"]
     assert x["workload"].startswith("cfg1") and x["value"] > 0 and x["launch_us"] > 0 and x["steps"] == 4
     assert x["roofline"]["frac"] == x["roofline"]["achieved"] / x["roofline"]["peak"] and "clocks" in x
