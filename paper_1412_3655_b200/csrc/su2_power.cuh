@@ -17,7 +17,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <math.h>
-#include "heatbath.cuh"
+#include <stdint.h>
 
 namespace culgt {
 
@@ -77,6 +77,12 @@ __device__ __forceinline__ double rsqrt_newton(double x) {
   }
   return y;
 }
+
+}  // namespace culgt
+
+#include "heatbath.cuh"   // needs kSinCoef / kCosCoef and rsqrt_newton above
+
+namespace culgt {
 
 // atan2(y, x) for y >= 0 and x^2 + y^2 = 1, in fp32, absolute error < 3e-6 (degree-11 odd
 // polynomial on [0,1] plus octant fix-up).  It only seeds the fp64 correction below.
