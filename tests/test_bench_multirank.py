@@ -78,3 +78,24 @@ def test_reference_arm_prints_on_rank0_only():
     assert line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
     assert line["n_gpus"] == 2 and line["steps"] == 2
+
+
+def test_committed_traffic_rows_are_stamped_and_stale_rows_are_refused():
+    """roofline.traffic* comes from committed ncu captures (profiles/roofline_traffic.csv), which cannot
+    be measured live: every row carries the commit and the kernel instantiation it was taken on, and
+    bench.py uses a row only for the kernel it names."""
+    rows = [l.strip().split(";") for l in open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) if l.strip()]
+    assert rows[0] == ["workload", "capture", "dram_read_bytes", "dram_write_bytes", "commit", "kernel", "source"]
+    for r in rows[1:]:
+        assert len(r) == 7 and int(r[2]) > 0 and int(r[3]) > 0 and len(r[4]) >= 7
+        assert os.path.exists(os.path.join(ROOT, r[6]))
+    import paper_1412_3655_b200 as culgt
+    kernel = culgt.culgt_sweep_kernel_name(culgt.Lattice((32, 32, 32, 32), 3, 32, 12))
+    total, info = bench.committed_traffic("cfg3_fp32", "steady_state", kernel)
+    assert total is not None and 3.0e8 < total < 4.1e8 and info["kernel"] == kernel and "stale" not in info
+    # the steady-state DRAM traffic never exceeds the algorithmic bytes of a half-sweep (no re-reads)
+    assert total <= 2 * 4 * 32 ** 4 * 48
+    total, info = bench.committed_traffic("cfg3_fp32", "steady_state", "some_other_kernel<...>")
+    assert total is None and "stale" in info
+    total, info = bench.committed_traffic("cfg2", "steady_state", kernel)
+    assert total is None and "stale" in info
