@@ -34,7 +34,7 @@ __device__ __forceinline__ void grid_barrier(unsigned* counter, unsigned& target
     target += gridDim.x;
     __threadfence();                       // my CTA's stores are visible before I arrive
     atomicAdd(counter, 1u);
-    while (ld_acquire_u32(counter) < target) {}
+    while ((int)(ld_acquire_u32(counter) - target) < 0) {}     // wrap-safe: the counter is monotone mod 2^32
   }
   __syncthreads();
 }
